@@ -1,0 +1,303 @@
+// C ABI of libsw (include/sw.h): host-side validation and dispatch.  Nothing here computes.
+#include <stdarg.h>
+#include <string.h>
+
+#include "common.cuh"
+
+namespace sw {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+int32_t fail(int32_t code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+static int g_sms = 0;
+
+int32_t check_arch() {
+  static int cached_dev = -1;
+  static int32_t cached = SW_ERR_ARCH;
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) {
+    cudaGetLastError();
+    return fail(SW_ERR_ARCH, "no CUDA device is available (libsw has no CPU fallback)");
+  }
+  if (dev == cached_dev) return cached;
+  int major = 0, minor = 0, sms = 0;
+  cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cached_dev = dev;
+  g_sms = sms;
+  cached = (major == 10) ? SW_OK : SW_ERR_ARCH;
+  if (cached != SW_OK) set_error("device %d is sm_%d%d; libsw is built for sm_100a only", dev, major, minor);
+  return cached;
+}
+
+int num_sms() { return g_sms > 0 ? g_sms : 148; }
+
+int32_t check_launch(const char* what) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(SW_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+  return SW_OK;
+}
+
+int32_t validate_layout(const sw_layout* L) {
+  SW_REQUIRE(L != nullptr, SW_ERR_INVALID_ARG, "layout is NULL");
+  SW_REQUIRE(L->batch >= 0 && L->total_tokens >= 0 && L->total_blocks >= 0 && L->max_blocks >= 0,
+             SW_ERR_INVALID_ARG, "layout: negative size");
+  SW_REQUIRE(L->block == 64 || L->block == 128, SW_ERR_UNSUPPORTED, "layout: block size %d not in {64,128}",
+             L->block);
+  if (L->batch > 0) {
+    SW_REQUIRE(L->cu_seqlens && L->cu_blocks && L->cu_sq, SW_ERR_INVALID_ARG, "layout: NULL cu_* array");
+    SW_REQUIRE(L->max_blocks <= L->total_blocks, SW_ERR_INVALID_ARG, "layout: max_blocks > total_blocks");
+    SW_REQUIRE((int64_t)L->total_blocks * L->block >= L->total_tokens, SW_ERR_INVALID_ARG,
+               "layout: total_blocks*block < total_tokens");
+  }
+  return SW_OK;
+}
+
+int32_t validate_tensor(const sw_tensor* t, const char* name) {
+  SW_REQUIRE(t != nullptr, SW_ERR_INVALID_ARG, "%s is NULL", name);
+  SW_REQUIRE(t->ptr != nullptr, SW_ERR_INVALID_ARG, "%s.ptr is NULL", name);
+  SW_REQUIRE(aligned16(t->ptr), SW_ERR_INVALID_ARG, "%s.ptr is not 16-byte aligned", name);
+  SW_REQUIRE(t->dtype == SW_BF16 || t->dtype == SW_F32, SW_ERR_UNSUPPORTED, "%s.dtype %d", name, t->dtype);
+  SW_REQUIRE(t->d == 64 || t->d == 128, SW_ERR_UNSUPPORTED, "%s.d = %d not in {64,128}", name, t->d);
+  SW_REQUIRE(t->heads >= 1, SW_ERR_INVALID_ARG, "%s.heads = %d", name, t->heads);
+  SW_REQUIRE(t->stride_tok % 8 == 0 && t->stride_head % 8 == 0 && t->stride_head >= t->d,
+             SW_ERR_INVALID_ARG, "%s: strides must be multiples of 8 elements and stride_head >= d", name);
+  return SW_OK;
+}
+
+static int32_t validate_sketch_params(const sw_tensor* x, const int32_t* cols, int r) {
+  SW_REQUIRE(cols != nullptr, SW_ERR_INVALID_ARG, "cols is NULL");
+  SW_REQUIRE(is_pow2(r) && r <= x->d, SW_ERR_INVALID_ARG, "r = %d must be a power of two <= d = %d", r, x->d);
+  return SW_OK;
+}
+
+}  // namespace sw
+
+using namespace sw;
+
+#define SW_TRY(expr)                  \
+  do {                                \
+    int32_t _s = (expr);              \
+    if (_s != SW_OK) return _s;       \
+  } while (0)
+
+extern "C" {
+
+SW_API const char* sw_last_error(void) { return g_err; }
+SW_API int32_t sw_version(void) { return SW_VERSION; }
+
+SW_API int32_t sw_sketch(const sw_layout* L, const sw_tensor* x, const int8_t* signs, const int32_t* cols,
+                  int32_t r, float scale, float* sketch, float* mean, sw_stream_t stream) {
+  SW_TRY(validate_layout(L));
+  SW_TRY(validate_tensor(x, "x"));
+  SW_TRY(validate_sketch_params(x, cols, r));
+  SW_REQUIRE(sketch != nullptr, SW_ERR_INVALID_ARG, "sketch is NULL");
+  SW_TRY(check_arch());
+  return launch_sketch(*L, *x, signs, cols, r, scale, sketch, mean, (cudaStream_t)stream);
+}
+
+SW_API int32_t sw_sketch_append(int32_t batch, int32_t block, int32_t max_blocks, const sw_tensor* x,
+                         const int32_t* seqlens, const int8_t* signs, const int32_t* cols, int32_t r,
+                         float scale, float* mean, float* sketch, float* tok_sketch, sw_stream_t stream) {
+  SW_REQUIRE(batch >= 0 && max_blocks >= 1, SW_ERR_INVALID_ARG, "batch %d / max_blocks %d", batch, max_blocks);
+  SW_REQUIRE(block == 64 || block == 128, SW_ERR_UNSUPPORTED, "block size %d not in {64,128}", block);
+  SW_TRY(validate_tensor(x, "x"));
+  SW_TRY(validate_sketch_params(x, cols, r));
+  SW_REQUIRE(seqlens != nullptr, SW_ERR_INVALID_ARG, "seqlens is NULL");
+  SW_REQUIRE((mean && sketch) || tok_sketch, SW_ERR_INVALID_ARG, "nothing to write");
+  SW_REQUIRE((mean != nullptr) == (sketch != nullptr), SW_ERR_INVALID_ARG, "mean and sketch go together");
+  SW_TRY(check_arch());
+  return launch_sketch_append(batch, block, max_blocks, *x, seqlens, signs, cols, r, scale, mean, sketch,
+                              tok_sketch, (cudaStream_t)stream);
+}
+
+SW_API int32_t sw_block_scores(const sw_layout* L, const float* qs, const float* ks, int32_t r, int32_t s,
+                        uint32_t flags, float* W, float* A, sw_stream_t stream) {
+  SW_TRY(validate_layout(L));
+  SW_REQUIRE(qs && ks && W, SW_ERR_INVALID_ARG, "qs / ks / W is NULL");
+  SW_REQUIRE(r >= 1 && r <= 128, SW_ERR_INVALID_ARG, "r = %d out of [1,128]", r);
+  SW_REQUIRE(s >= 1, SW_ERR_INVALID_ARG, "s = %d must be >= 1", s);
+  SW_TRY(check_arch());
+  return launch_block_scores(*L, qs, ks, r, s, flags, W, A, (cudaStream_t)stream);
+}
+
+SW_API int32_t sw_block_scores_row(int32_t batch, int32_t block, int32_t max_blocks, const float* q_tok,
+                            const float* ks, const int32_t* seqlens, int32_t r, int32_t s, uint32_t flags,
+                            float* w_row, sw_stream_t stream) {
+  SW_REQUIRE(batch >= 0 && max_blocks >= 1, SW_ERR_INVALID_ARG, "batch %d / max_blocks %d", batch, max_blocks);
+  SW_REQUIRE(block == 64 || block == 128, SW_ERR_UNSUPPORTED, "block size %d not in {64,128}", block);
+  SW_REQUIRE(q_tok && ks && seqlens && w_row, SW_ERR_INVALID_ARG, "NULL argument");
+  SW_REQUIRE(r >= 1 && r <= 128 && s >= 1, SW_ERR_INVALID_ARG, "r = %d / s = %d", r, s);
+  SW_REQUIRE(!(flags & SW_POW_MATRIX), SW_ERR_UNSUPPORTED, "row mode needs the element-wise power (P4)");
+  SW_TRY(check_arch());
+  return launch_block_scores_row(batch, block, max_blocks, q_tok, ks, seqlens, r, s, flags, w_row,
+                                 (cudaStream_t)stream);
+}
+
+SW_API int32_t sw_walk_update(const sw_layout* L, const float* R_prev, const float* W, int32_t s, uint32_t flags,
+                       float* R_out, void* ws, size_t ws_bytes, sw_stream_t stream) {
+  SW_TRY(validate_layout(L));
+  SW_REQUIRE(W && R_out, SW_ERR_INVALID_ARG, "W / R_out is NULL");
+  SW_REQUIRE(R_out != R_prev && R_out != W, SW_ERR_INVALID_ARG, "R_out must not alias its inputs");
+  SW_REQUIRE(s >= 1, SW_ERR_INVALID_ARG, "s = %d must be >= 1", s);
+  if ((flags & SW_POW_MATRIX) && s > 1) {
+    const size_t need = sw_workspace_bytes(SW_OP_WALK_UPDATE, L, 0, 0, 0, 0, SW_F32);
+    SW_REQUIRE(ws != nullptr && ws_bytes >= need, SW_ERR_WORKSPACE,
+               "sw_walk_update: workspace %zu < %zu bytes", ws_bytes, need);
+  }
+  SW_TRY(check_arch());
+  return launch_walk(*L, R_prev, W, s, flags, R_out, ws, ws_bytes, (cudaStream_t)stream);
+}
+
+SW_API int32_t sw_walk_update_row(int32_t batch, int32_t block, int32_t max_blocks, const float* r_prev,
+                           const float* W_cache, int64_t stride_seq, const float* w_row,
+                           const int32_t* seqlens, uint32_t flags, float* r_out, sw_stream_t stream) {
+  SW_REQUIRE(batch >= 0 && max_blocks >= 1, SW_ERR_INVALID_ARG, "batch %d / max_blocks %d", batch, max_blocks);
+  SW_REQUIRE(block == 64 || block == 128, SW_ERR_UNSUPPORTED, "block size %d not in {64,128}", block);
+  SW_REQUIRE(W_cache && w_row && seqlens && r_out, SW_ERR_INVALID_ARG, "NULL argument");
+  SW_REQUIRE(r_out != r_prev, SW_ERR_INVALID_ARG, "r_out must not alias r_prev");
+  SW_TRY(check_arch());
+  return launch_walk_row(batch, block, max_blocks, r_prev, W_cache, stride_seq, w_row, seqlens, flags,
+                         r_out, (cudaStream_t)stream);
+}
+
+SW_API int32_t sw_select_topk(const sw_layout* L, const float* R, const int32_t* tau, int32_t tau_max,
+                       uint32_t flags, int32_t* idx, int32_t* count, sw_stream_t stream) {
+  SW_TRY(validate_layout(L));
+  SW_REQUIRE(R && tau && idx && count, SW_ERR_INVALID_ARG, "NULL argument");
+  SW_REQUIRE(tau_max >= 1, SW_ERR_INVALID_ARG, "tau_max = %d", tau_max);
+  SW_TRY(check_arch());
+  return launch_select(*L, R, tau, tau_max, flags, idx, count, (cudaStream_t)stream);
+}
+
+SW_API int32_t sw_select_topk_row(int32_t batch, int32_t block, int32_t max_blocks, const float* r,
+                           const int32_t* seqlens, const int32_t* tau, int32_t tau_max, uint32_t flags,
+                           int32_t* idx, int32_t* count, sw_stream_t stream) {
+  SW_REQUIRE(batch >= 0 && max_blocks >= 1, SW_ERR_INVALID_ARG, "batch %d / max_blocks %d", batch, max_blocks);
+  SW_REQUIRE(block == 64 || block == 128, SW_ERR_UNSUPPORTED, "block size %d not in {64,128}", block);
+  SW_REQUIRE(r && seqlens && tau && idx && count, SW_ERR_INVALID_ARG, "NULL argument");
+  SW_REQUIRE(tau_max >= 1, SW_ERR_INVALID_ARG, "tau_max = %d", tau_max);
+  SW_TRY(check_arch());
+  return launch_select_row(batch, block, max_blocks, r, seqlens, tau, tau_max, flags, idx, count,
+                           (cudaStream_t)stream);
+}
+
+static size_t cast_bytes(int64_t tokens, int heads, int d) {
+  return ((size_t)tokens * heads * d * 2 + 255) & ~(size_t)255;
+}
+
+SW_API size_t sw_workspace_bytes(int32_t op, const sw_layout* L, int32_t h_q, int32_t h_kv, int32_t d,
+                          int32_t tau_max, int32_t dtype) {
+  switch (op) {
+    case SW_OP_WALK_UPDATE:
+      return L ? (size_t)L->batch * L->max_blocks * L->max_blocks * sizeof(float) : 0;
+    case SW_OP_ATTN_PREFILL:
+      if (!L || dtype != SW_F32) return 0;
+      return cast_bytes(L->total_tokens, h_q, d) + 2 * cast_bytes(L->total_tokens, h_kv, d);
+    case SW_OP_ATTN_DECODE:
+      return L ? sw_decode_workspace_bytes(L->batch, h_q, h_kv, d, tau_max) : 0;
+    default:
+      return 0;
+  }
+}
+
+SW_API int32_t sw_decode_num_splits(int32_t batch, int32_t h_kv, int32_t tau_max) {
+  check_arch();
+  return decode_num_splits(batch, h_kv, tau_max);
+}
+
+SW_API size_t sw_decode_workspace_bytes(int32_t batch, int32_t h_q, int32_t h_kv, int32_t d, int32_t tau_max) {
+  check_arch();
+  return decode_ws_bytes(batch, h_q, d, decode_num_splits(batch, h_kv, tau_max));
+}
+
+SW_API int32_t sw_sparse_attn_prefill(const sw_layout* L, const sw_tensor* q, const sw_tensor* k, const sw_tensor* v,
+                               const int32_t* idx, const int32_t* count, int32_t tau_max, float softmax_scale,
+                               uint32_t flags, void* out, float* lse, void* ws, size_t ws_bytes,
+                               sw_stream_t stream) {
+  SW_TRY(validate_layout(L));
+  SW_TRY(validate_tensor(q, "q"));
+  SW_TRY(validate_tensor(k, "k"));
+  SW_TRY(validate_tensor(v, "v"));
+  SW_REQUIRE(idx && count && out, SW_ERR_INVALID_ARG, "idx / count / out is NULL");
+  SW_REQUIRE(aligned16(out), SW_ERR_INVALID_ARG, "out is not 16-byte aligned");
+  SW_REQUIRE(tau_max >= 1, SW_ERR_INVALID_ARG, "tau_max = %d", tau_max);
+  SW_REQUIRE(q->dtype == k->dtype && k->dtype == v->dtype, SW_ERR_UNSUPPORTED, "q/k/v dtypes differ");
+  SW_REQUIRE(q->d == k->d && k->d == v->d, SW_ERR_UNSUPPORTED, "q/k/v head_dim differ");
+  SW_REQUIRE(k->heads == v->heads && q->heads % k->heads == 0, SW_ERR_INVALID_ARG,
+             "h_q = %d must be a multiple of h_kv = %d", q->heads, k->heads);
+  SW_TRY(check_arch());
+  cudaStream_t st = (cudaStream_t)stream;
+
+  AttnPrefillArgs a;
+  a.L = L;
+  a.h_q = q->heads; a.h_kv = k->heads; a.d = q->d;
+  a.idx = idx; a.count = count; a.tau_max = tau_max;
+  a.softmax_scale = softmax_scale; a.flags = flags;
+  a.out = out; a.out_dtype = q->dtype; a.lse = lse;
+  if (q->dtype == SW_F32) {
+    // P17: attention operands are rounded to bf16 by a cast pre-pass
+    const size_t need = sw_workspace_bytes(SW_OP_ATTN_PREFILL, L, q->heads, k->heads, q->d, tau_max, SW_F32);
+    SW_REQUIRE(ws != nullptr && ws_bytes >= need && aligned16(ws), SW_ERR_WORKSPACE,
+               "sw_sparse_attn_prefill: fp32 inputs need %zu bytes of workspace, got %zu", need, ws_bytes);
+    uint8_t* p = reinterpret_cast<uint8_t*>(ws);
+    __nv_bfloat16* qb = reinterpret_cast<__nv_bfloat16*>(p);
+    p += cast_bytes(L->total_tokens, q->heads, q->d);
+    __nv_bfloat16* kb = reinterpret_cast<__nv_bfloat16*>(p);
+    p += cast_bytes(L->total_tokens, k->heads, k->d);
+    __nv_bfloat16* vb = reinterpret_cast<__nv_bfloat16*>(p);
+    SW_TRY(launch_cast_f32_to_bf16((const float*)q->ptr, qb, L->total_tokens, q->heads, q->d, q->stride_tok, q->stride_head, st));
+    SW_TRY(launch_cast_f32_to_bf16((const float*)k->ptr, kb, L->total_tokens, k->heads, k->d, k->stride_tok, k->stride_head, st));
+    SW_TRY(launch_cast_f32_to_bf16((const float*)v->ptr, vb, L->total_tokens, v->heads, v->d, v->stride_tok, v->stride_head, st));
+    a.q = qb; a.k = kb; a.v = vb;
+    a.q_stride_head = q->d; a.q_stride_tok = (int64_t)q->heads * q->d;
+    a.k_stride_head = k->d; a.k_stride_tok = (int64_t)k->heads * k->d;
+    a.v_stride_head = v->d; a.v_stride_tok = (int64_t)v->heads * v->d;
+  } else {
+    a.q = (const __nv_bfloat16*)q->ptr; a.k = (const __nv_bfloat16*)k->ptr; a.v = (const __nv_bfloat16*)v->ptr;
+    a.q_stride_tok = q->stride_tok; a.q_stride_head = q->stride_head;
+    a.k_stride_tok = k->stride_tok; a.k_stride_head = k->stride_head;
+    a.v_stride_tok = v->stride_tok; a.v_stride_head = v->stride_head;
+  }
+  if (attn_prefill_sm100_supported(a)) return launch_attn_prefill_sm100(a, st);
+  return launch_attn_prefill_generic(a, st);
+}
+
+SW_API int32_t sw_sparse_attn_decode(int32_t batch, int32_t block, const sw_tensor* q, const sw_tensor* kcache,
+                              const sw_tensor* vcache, int64_t stride_batch, const int32_t* seqlens,
+                              const int32_t* idx, const int32_t* count, int32_t tau_max, float softmax_scale,
+                              void* out, float* lse, void* ws, size_t ws_bytes, sw_stream_t stream) {
+  SW_REQUIRE(batch >= 0, SW_ERR_INVALID_ARG, "batch = %d", batch);
+  SW_REQUIRE(block == 64 || block == 128, SW_ERR_UNSUPPORTED, "block size %d not in {64,128}", block);
+  SW_TRY(validate_tensor(q, "q"));
+  SW_TRY(validate_tensor(kcache, "kcache"));
+  SW_TRY(validate_tensor(vcache, "vcache"));
+  SW_REQUIRE(q->dtype == SW_BF16 && kcache->dtype == SW_BF16 && vcache->dtype == SW_BF16, SW_ERR_UNSUPPORTED,
+             "decode attention takes bf16 q and caches");
+  SW_REQUIRE(q->d == kcache->d && q->d == vcache->d, SW_ERR_UNSUPPORTED, "head_dim mismatch");
+  SW_REQUIRE(kcache->heads == vcache->heads && q->heads % kcache->heads == 0 &&
+                 q->heads / kcache->heads <= 16,
+             SW_ERR_UNSUPPORTED, "GQA group h_q/h_kv = %d/%d must be an integer <= 16", q->heads, kcache->heads);
+  SW_REQUIRE(seqlens && idx && count && out, SW_ERR_INVALID_ARG, "NULL argument");
+  SW_REQUIRE(tau_max >= 1 && stride_batch % 8 == 0, SW_ERR_INVALID_ARG, "tau_max / stride_batch");
+  SW_TRY(check_arch());
+  return launch_attn_decode(batch, block, *q, *kcache, *vcache, stride_batch, seqlens, idx, count, tau_max,
+                            softmax_scale, out, lse, ws, ws_bytes, (cudaStream_t)stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,127 @@
+// Shared host/device helpers of libsw (sm_100a only).  No arithmetic of the method lives
+// here: error plumbing, launch checks, small device utilities.
+#pragma once
+
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/sw.h"
+
+namespace sw {
+
+// ---- thread-local error text ---------------------------------------------------------
+void set_error(const char* fmt, ...);
+int32_t fail(int32_t code, const char* fmt, ...);
+int32_t check_arch();                      // SW_OK or SW_ERR_ARCH (cached per device)
+int32_t check_launch(const char* what);    // cudaGetLastError -> SW_ERR_CUDA
+int num_sms();
+
+#define SW_REQUIRE(cond, code, ...)            \
+  do {                                         \
+    if (!(cond)) return sw::fail((code), __VA_ARGS__); \
+  } while (0)
+
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+static inline bool is_pow2(int x) { return x > 0 && (x & (x - 1)) == 0; }
+static inline int cdiv(int a, int b) { return (a + b - 1) / b; }
+
+int32_t validate_layout(const sw_layout* L);
+int32_t validate_tensor(const sw_tensor* t, const char* name);
+
+// ---- kernel launchers (one per translation unit) ---------------------------------------
+int32_t launch_sketch(const sw_layout& L, const sw_tensor& x, const int8_t* signs, const int32_t* cols,
+                      int r, float scale, float* sketch, float* mean, cudaStream_t st);
+int32_t launch_sketch_append(int batch, int block, int max_blocks, const sw_tensor& x,
+                             const int32_t* seqlens, const int8_t* signs, const int32_t* cols, int r,
+                             float scale, float* mean, float* sketch, float* tok_sketch, cudaStream_t st);
+int32_t launch_block_scores(const sw_layout& L, const float* qs, const float* ks, int r, int s,
+                            uint32_t flags, float* W, float* A, cudaStream_t st);
+int32_t launch_block_scores_row(int batch, int block, int max_blocks, const float* q_tok, const float* ks,
+                                const int32_t* seqlens, int r, int s, uint32_t flags, float* w_row,
+                                cudaStream_t st);
+int32_t launch_walk(const sw_layout& L, const float* R_prev, const float* W, int s, uint32_t flags,
+                    float* R_out, void* ws, size_t ws_bytes, cudaStream_t st);
+int32_t launch_walk_row(int batch, int block, int max_blocks, const float* r_prev, const float* W_cache,
+                        int64_t stride_seq, const float* w_row, const int32_t* seqlens, uint32_t flags,
+                        float* r_out, cudaStream_t st);
+int32_t launch_select(const sw_layout& L, const float* R, const int32_t* tau, int tau_max,
+                      uint32_t flags, int32_t* idx, int32_t* count, cudaStream_t st);
+int32_t launch_select_row(int batch, int block, int max_blocks, const float* r, const int32_t* seqlens,
+                          const int32_t* tau, int tau_max, uint32_t flags, int32_t* idx, int32_t* count,
+                          cudaStream_t st);
+
+struct AttnPrefillArgs {
+  const sw_layout* L;
+  const __nv_bfloat16 *q, *k, *v;           // bf16 operands (possibly the cast copies in ws)
+  int64_t q_stride_tok, q_stride_head, k_stride_tok, k_stride_head, v_stride_tok, v_stride_head;
+  int h_q, h_kv, d;
+  const int32_t *idx, *count;
+  int tau_max;
+  float softmax_scale;
+  uint32_t flags;
+  void* out;                                // [total_tokens, h_q, d] contiguous
+  int out_dtype;                            // SW_BF16 | SW_F32
+  float* lse;
+};
+int32_t launch_attn_prefill_generic(const AttnPrefillArgs& a, cudaStream_t st);
+bool attn_prefill_sm100_supported(const AttnPrefillArgs& a);
+int32_t launch_attn_prefill_sm100(const AttnPrefillArgs& a, cudaStream_t st);
+int32_t launch_cast_f32_to_bf16(const float* src, __nv_bfloat16* dst, int64_t tokens, int heads, int d,
+                                int64_t stride_tok, int64_t stride_head, cudaStream_t st);
+
+int decode_num_splits(int batch, int h_kv, int tau_max);
+size_t decode_ws_bytes(int batch, int h_q, int d, int nsplit);
+int32_t launch_attn_decode(int batch, int block, const sw_tensor& q, const sw_tensor& kc,
+                           const sw_tensor& vc, int64_t stride_batch, const int32_t* seqlens,
+                           const int32_t* idx, const int32_t* count, int tau_max, float softmax_scale,
+                           void* out, float* lse, void* ws, size_t ws_bytes, cudaStream_t st);
+
+}  // namespace sw
+
+// ---- device utilities ------------------------------------------------------------------
+#ifdef __CUDACC__
+namespace swd {
+
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ int warp_sum_i(int v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// sequence that owns global block index gb: largest s with cu_blocks[s] <= gb
+__device__ __forceinline__ int find_seq(const int32_t* __restrict__ cu, int batch, int gb) {
+  int lo = 0, hi = batch - 1;
+  while (lo < hi) {
+    int mid = (lo + hi + 1) >> 1;
+    if (__ldg(cu + mid) <= gb) lo = mid; else hi = mid - 1;
+  }
+  return lo;
+}
+
+__device__ __forceinline__ uint4 ld_nc_v4(const void* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+
+__device__ __forceinline__ float powi(float x, int s) {
+  float r = 1.f, b = x;
+  while (s) { if (s & 1) r *= b; b *= b; s >>= 1; }
+  return r;
+}
+
+}  // namespace swd
+#endif

@@ -1,0 +1,220 @@
+// sw_sketch: Small-World Sketching, Alg. 1 Steps 1-4, sec 2.2.
+// One fused pass: head mean + block mean (token-space sketch) -> sign flip D -> fast
+// Walsh-Hadamard transform in registers / warp shuffles -> column sampling S -> scale.
+// HBM-bound: every element of x is read exactly once with 128-bit loads; H_d is never
+// materialised.
+#include "common.cuh"
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kUnroll = 8;
+
+template <typename T> struct Chunk;          // 8 consecutive elements of one row
+template <> struct Chunk<__nv_bfloat16> {
+  uint4 v;
+  __device__ __forceinline__ void load(const __nv_bfloat16* p) { v = swd::ld_nc_v4(p); }
+  __device__ __forceinline__ void add_to(float* acc) const {
+    const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&v);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      float2 f = __bfloat1622float2(h[i]);
+      acc[2 * i] += f.x;
+      acc[2 * i + 1] += f.y;
+    }
+  }
+};
+template <> struct Chunk<float> {
+  uint4 a, b;
+  __device__ __forceinline__ void load(const float* p) {
+    a = swd::ld_nc_v4(p);
+    b = swd::ld_nc_v4(p + 4);
+  }
+  __device__ __forceinline__ void add_to(float* acc) const {
+    const float* fa = reinterpret_cast<const float*>(&a);
+    const float* fb = reinterpret_cast<const float*>(&b);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { acc[i] += fa[i]; acc[4 + i] += fb[i]; }
+  }
+};
+
+// In-warp FWHT of a d-vector held as EPL = d/32 consecutive elements per lane
+// (element x = lane*EPL + e), natural (Sylvester) order: y[x] = sum_z v[z] (-1)^popcount(x&z).
+template <int EPL>
+__device__ __forceinline__ void fwht_warp(float (&v)[EPL], int lane) {
+#pragma unroll
+  for (int h = 1; h < EPL; h <<= 1) {
+#pragma unroll
+    for (int e = 0; e < EPL; ++e) {
+      if ((e & h) == 0) {
+        float a = v[e], b = v[e | h];
+        v[e] = a + b;
+        v[e | h] = a - b;
+      }
+    }
+  }
+#pragma unroll
+  for (int m = 1; m < 32; m <<= 1) {
+#pragma unroll
+    for (int e = 0; e < EPL; ++e) {
+      float other = __shfl_xor_sync(0xffffffffu, v[e], m);
+      v[e] = (lane & m) ? (other - v[e]) : (v[e] + other);
+    }
+  }
+}
+
+// Shared tail: warp 0 turns the d-vector in s_vec into the r-vector of the sketch.
+template <int D>
+__device__ __forceinline__ void sketch_tail(float* s_vec, const int8_t* __restrict__ signs,
+                                            const int32_t* __restrict__ cols, int r, float scale,
+                                            float* __restrict__ out_row) {
+  constexpr int EPL = D / 32;
+  const int lane = threadIdx.x & 31;
+  if (threadIdx.x < 32) {
+    float v[EPL];
+#pragma unroll
+    for (int e = 0; e < EPL; ++e) {
+      int x = lane * EPL + e;
+      float sg = signs ? (float)signs[x] : 1.f;
+      v[e] = s_vec[x] * sg;
+    }
+    fwht_warp<EPL>(v, lane);
+    __syncwarp();
+#pragma unroll
+    for (int e = 0; e < EPL; ++e) s_vec[lane * EPL + e] = v[e];
+    __syncwarp();
+    for (int c = lane; c < r; c += 32) out_row[c] = s_vec[__ldg(cols + c)] * scale;
+  }
+}
+
+template <typename T, int D>
+__global__ void __launch_bounds__(kThreads)
+sketch_kernel(const T* __restrict__ x, int64_t stride_tok, int64_t stride_head, int heads,
+              const int32_t* __restrict__ cu_seqlens, const int32_t* __restrict__ cu_blocks, int batch,
+              int B, const int8_t* __restrict__ signs, const int32_t* __restrict__ cols, int r,
+              float scale, float* __restrict__ sketch, float* __restrict__ mean) {
+  constexpr int D8 = D / 8;                      // 8-element chunks per head row
+  __shared__ float s_part[kThreads][9];          // +1 pad
+  __shared__ float s_vec[D];
+
+  const int gb = blockIdx.x;
+  const int seq = swd::find_seq(cu_blocks, batch, gb);
+  const int bi = gb - __ldg(cu_blocks + seq);
+  const int tok0 = __ldg(cu_seqlens + seq) + bi * B;
+  const int tok_end = min(tok0 + B, __ldg(cu_seqlens + seq + 1));
+  const int ntok = tok_end - tok0;
+
+  const int tid = threadIdx.x;
+  const int chunk = tid % D8;                    // constant per thread: kThreads % D8 == 0
+  const int rows_per_pass = kThreads / D8;       // (token, head) rows covered per pass
+  const int total_rows = ntok * heads;
+  float acc[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) acc[i] = 0.f;
+
+  int row = tid / D8;
+  // main loop: kUnroll independent 128-bit loads in flight per thread
+  for (; row + (kUnroll - 1) * rows_per_pass < total_rows; row += kUnroll * rows_per_pass) {
+    Chunk<T> c[kUnroll];
+#pragma unroll
+    for (int u = 0; u < kUnroll; ++u) {
+      int rr = row + u * rows_per_pass;
+      int tok = rr / heads, hd = rr - tok * heads;
+      c[u].load(x + (int64_t)(tok0 + tok) * stride_tok + (int64_t)hd * stride_head + chunk * 8);
+    }
+#pragma unroll
+    for (int u = 0; u < kUnroll; ++u) c[u].add_to(acc);
+  }
+  for (; row < total_rows; row += rows_per_pass) {
+    int tok = row / heads, hd = row - tok * heads;
+    Chunk<T> c;
+    c.load(x + (int64_t)(tok0 + tok) * stride_tok + (int64_t)hd * stride_head + chunk * 8);
+    c.add_to(acc);
+  }
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s_part[tid][i] = acc[i];
+  __syncthreads();
+  if (tid < D) {
+    const int ch = tid / 8, e = tid % 8;
+    float s = 0.f;
+    for (int k = 0; k < rows_per_pass; ++k) s += s_part[k * D8 + ch][e];
+    const float m = s / (float)(ntok * heads);   // P12: divide by the number of valid tokens
+    s_vec[tid] = m;
+    if (mean) mean[(int64_t)gb * D + tid] = m;
+  }
+  __syncthreads();
+  sketch_tail<D>(s_vec, signs, cols, r, scale, sketch + (int64_t)gb * r);
+}
+
+// Decode (Alg. 2 Steps 2-3): one token per sequence; one CTA per sequence.
+template <typename T, int D>
+__global__ void __launch_bounds__(128)
+sketch_append_kernel(const T* __restrict__ x, int64_t stride_seq, int64_t stride_head, int heads,
+                     const int32_t* __restrict__ seqlens, int B, int max_blocks,
+                     const int8_t* __restrict__ signs, const int32_t* __restrict__ cols, int r, float scale,
+                     float* __restrict__ mean, float* __restrict__ sketch, float* __restrict__ tok_sketch) {
+  __shared__ float s_vec[D];
+  __shared__ float s_tok[D];
+  const int seq = blockIdx.x;
+  const int t = __ldg(seqlens + seq);
+  const int bcur = (t - 1) / B;
+  const int c = (t - 1) % B;                      // tokens already in block b_curr
+  const int tid = threadIdx.x;
+  if (tid < D) {
+    float s = 0.f;
+    for (int h = 0; h < heads; ++h)
+      s += (float)x[(int64_t)seq * stride_seq + (int64_t)h * stride_head + tid];
+    const float avg = s / (float)heads;           // PAPER.md:810 / 815
+    s_tok[tid] = avg;
+    if (mean) {
+      float* mp = mean + ((int64_t)seq * max_blocks + bcur) * D + tid;
+      const float m = (c == 0) ? avg : ((float)c * (*mp) + avg) / (float)(c + 1);
+      *mp = m;
+      s_vec[tid] = m;
+    }
+  }
+  __syncthreads();
+  if (mean && sketch)
+    sketch_tail<D>(s_vec, signs, cols, r, scale, sketch + ((int64_t)seq * max_blocks + bcur) * r);
+  if (tok_sketch) sketch_tail<D>(s_tok, signs, cols, r, scale, tok_sketch + (int64_t)seq * r);
+}
+
+}  // namespace
+
+namespace sw {
+
+int32_t launch_sketch(const sw_layout& L, const sw_tensor& x, const int8_t* signs, const int32_t* cols,
+                      int r, float scale, float* sketch, float* mean, cudaStream_t st) {
+  if (L.total_blocks == 0) return SW_OK;
+  dim3 grid(L.total_blocks), block(kThreads);
+#define SW_LAUNCH(T, D)                                                                              \
+  sketch_kernel<T, D><<<grid, block, 0, st>>>((const T*)x.ptr, x.stride_tok, x.stride_head, x.heads, \
+                                              L.cu_seqlens, L.cu_blocks, L.batch, L.block, signs,    \
+                                              cols, r, scale, sketch, mean)
+  if (x.dtype == SW_BF16 && x.d == 128) SW_LAUNCH(__nv_bfloat16, 128);
+  else if (x.dtype == SW_BF16 && x.d == 64) SW_LAUNCH(__nv_bfloat16, 64);
+  else if (x.dtype == SW_F32 && x.d == 128) SW_LAUNCH(float, 128);
+  else if (x.dtype == SW_F32 && x.d == 64) SW_LAUNCH(float, 64);
+  else return fail(SW_ERR_UNSUPPORTED, "sw_sketch: dtype %d / d %d", x.dtype, x.d);
+#undef SW_LAUNCH
+  return check_launch("sw_sketch");
+}
+
+int32_t launch_sketch_append(int batch, int block, int max_blocks, const sw_tensor& x,
+                             const int32_t* seqlens, const int8_t* signs, const int32_t* cols, int r,
+                             float scale, float* mean, float* sketch, float* tok_sketch, cudaStream_t st) {
+  if (batch == 0) return SW_OK;
+#define SW_LAUNCH(T, D)                                                                          \
+  sketch_append_kernel<T, D><<<batch, 128, 0, st>>>((const T*)x.ptr, x.stride_tok, x.stride_head, \
+                                                    x.heads, seqlens, block, max_blocks, signs,   \
+                                                    cols, r, scale, mean, sketch, tok_sketch)
+  if (x.dtype == SW_BF16 && x.d == 128) SW_LAUNCH(__nv_bfloat16, 128);
+  else if (x.dtype == SW_BF16 && x.d == 64) SW_LAUNCH(__nv_bfloat16, 64);
+  else if (x.dtype == SW_F32 && x.d == 128) SW_LAUNCH(float, 128);
+  else if (x.dtype == SW_F32 && x.d == 64) SW_LAUNCH(float, 64);
+  else return fail(SW_ERR_UNSUPPORTED, "sw_sketch_append: dtype %d / d %d", x.dtype, x.d);
+#undef SW_LAUNCH
+  return check_launch("sw_sketch_append");
+}
+
+}  // namespace sw

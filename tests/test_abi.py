@@ -1,0 +1,89 @@
+"""Host-side checks that need no GPU: libsw builds/loads, exports every symbol include/sw.h declares,
+and validates arguments before touching the device."""
+import ctypes as C
+import os
+import re
+
+import pytest
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    from paper_2602_07397_b200 import build as b
+    b.build()
+    import paper_2602_07397_b200 as p
+    return p
+
+
+def header_symbols():
+    text = open(os.path.join(ROOT, "include", "sw.h")).read()
+    return sorted(set(re.findall(r"SW_API\s+[\w\s\*]+?\b(sw_\w+)\s*\(", text)))
+
+
+def test_header_declares_the_six_calls():
+    syms = header_symbols()
+    for name in ["sw_sketch", "sw_block_scores", "sw_walk_update", "sw_select_topk", "sw_sparse_attn_prefill",
+                 "sw_sparse_attn_decode"]:
+        assert name in syms
+
+
+def test_library_exports_every_declared_symbol(pkg):
+    lib = C.CDLL(pkg.LIB_PATH)
+    syms = header_symbols()
+    assert len(syms) >= 15
+    for name in syms:
+        assert getattr(lib, name) is not None
+    assert sorted(pkg.EXPORTS) == syms
+    assert pkg.sw_version() == 100
+
+
+def test_flag_values_match_header(pkg):
+    text = open(os.path.join(ROOT, "include", "sw.h")).read()
+    for name in ["SW_CAUSAL", "SW_SCORE_SOFTMAX", "SW_POW_MATRIX", "SW_FORCE_FIRST", "SW_FORCE_LAST", "SW_ROWNORM"]:
+        val = int(re.search(name + r"\s*=\s*(\d+)", text).group(1))
+        assert getattr(pkg, name) == val
+    from oracle import sw_oracle as O        # the oracle restates the same contract values independently
+    assert (O.CAUSAL, O.SCORE_SOFTMAX, O.POW_MATRIX, O.FORCE_FIRST, O.FORCE_LAST, O.ROWNORM) == (1, 2, 4, 8, 16, 32)
+
+
+def test_validation_happens_before_any_device_work(pkg):
+    lib = pkg.binding._lib
+    # NULL layout -> INVALID_ARG regardless of the device
+    assert lib.sw_sketch(None, None, None, None, 64, 0.125, None, None, None) == pkg.SW_ERR_INVALID_ARG
+    assert b"layout" in lib.sw_last_error()
+    lay = pkg.binding._Layout(1, 48, 10, 1, 1, 1, 1, 1)
+    assert lib.sw_block_scores(C.byref(lay), 1, 1, 64, 2, 0, 1, None, None) == pkg.SW_ERR_UNSUPPORTED
+    lay = pkg.binding._Layout(1, 64, 10, 1, 1, 16, 16, 16)
+    assert lib.sw_block_scores(C.byref(lay), 16, 16, 64, 0, 0, 16, None, None) == pkg.SW_ERR_INVALID_ARG   # s = 0
+    t = pkg.binding._Tensor(16, pkg.SW_BF16, 8, 96, 768, 96)
+    assert lib.sw_sketch(C.byref(lay), C.byref(t), None, 16, 64, 0.125, 16, None, None) == pkg.SW_ERR_UNSUPPORTED
+    t = pkg.binding._Tensor(16, pkg.SW_BF16, 8, 128, 1024, 128)
+    assert lib.sw_sketch(C.byref(lay), C.byref(t), None, 16, 48, 0.125, 16, None, None) == pkg.SW_ERR_INVALID_ARG  # r
+    t = pkg.binding._Tensor(8, pkg.SW_BF16, 8, 128, 1024, 128)     # misaligned pointer
+    assert lib.sw_sketch(C.byref(lay), C.byref(t), None, 16, 64, 0.125, 16, None, None) == pkg.SW_ERR_INVALID_ARG
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU behaviour")
+def test_no_cpu_fallback_without_gpu(pkg):
+    """Valid arguments but no device: the call must fail loudly (SW_ERR_ARCH), never compute on the host."""
+    lib = pkg.binding._lib
+    lay = pkg.binding._Layout(1, 64, 10, 1, 1, 16, 16, 16)
+    assert lib.sw_block_scores(C.byref(lay), 16, 16, 64, 2, 0, 16, None, None) == pkg.SW_ERR_ARCH
+    with pytest.raises(pkg.SwError):
+        pkg.binding._check(pkg.SW_ERR_ARCH)
+
+
+def test_host_only_helpers(pkg):
+    assert pkg.sw_decode_num_splits(8, 8, 410) >= 1
+    assert pkg.sw_decode_workspace_bytes(8, 32, 8, 128, 410) > 0
+    assert pkg.tau_from_density(0.2, 512) == 103 and pkg.tau_from_density(0.25, 16) == 4
+
+
+def test_make_layout_offsets(pkg):
+    L = pkg.make_layout([130, 64, 257], 64, device="cpu")
+    assert L.blocks == [3, 1, 5] and L.total_blocks == 9 and L.max_blocks == 5 and L.total_tokens == 451
+    assert L.cu_seqlens.tolist() == [0, 130, 194, 451] and L.cu_blocks.tolist() == [0, 3, 4, 9]
+    assert L.cu_sq.tolist() == [0, 9, 10, 35] and L.total_sq == 35

@@ -1,0 +1,416 @@
+"""GPU parity: every C-ABI call of libsw against the CPU oracle on the same seeded inputs.
+Tolerances are the ones BASELINE.json's north_star states:
+  * selected block indices bit-exact when the GPU selector is fed the oracle's scores;
+  * sketch / score / walk values within 1e-3 relative (row-norm-wise: |d| <= 1e-3 max_j |ref[i,j]|);
+  * end-to-end block sets overlap >= 99 %, differences only at near-ties (<= 1e-3 of the row max);
+  * attention outputs within max-abs 2e-2 and mean-abs 2e-3 (bf16 I/O, fp32 accumulation).
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import sw_oracle as O
+from synth import gen
+
+pytestmark = pytest.mark.gpu
+
+REL = 1e-3
+ATT_MAX, ATT_MEAN = 2e-2, 2e-3
+
+
+@pytest.fixture(scope="module")
+def sw():
+    import paper_2602_07397_b200 as pkg
+    return pkg
+
+
+def rowwise_close(got, ref, rel=REL):
+    got = np.asarray(got, np.float64); ref = np.asarray(ref, np.float64)
+    scale = np.abs(ref).max(axis=-1, keepdims=True)
+    return bool((np.abs(got - ref) <= rel * scale + 1e-30).all())
+
+
+def dev(x, dtype=None):
+    t = torch.as_tensor(np.ascontiguousarray(x))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda()
+
+
+def H_of(d, r, seed=5):
+    signs, cols = gen.srht_params(seed, d, r)
+    return signs, cols, O.srht_matrix(d, signs, cols, 1 / math.sqrt(r))
+
+
+# ------------------------------------------------------------------------------ sketch
+@pytest.mark.parametrize("seqlens,heads,d,r,B,dtype", [
+    ((1024,), 1, 64, 16, 64, torch.float32),          # cfg 1
+    ((1000,), 32, 128, 64, 64, torch.bfloat16),       # ragged tail, Llama Q heads
+    ((333,), 8, 128, 64, 64, torch.bfloat16),         # K heads
+    ((130, 64, 257), 8, 128, 32, 128, torch.bfloat16),  # varlen, B = 128
+    ((70,), 4, 64, 64, 64, torch.bfloat16),           # r = d
+    ((5,), 2, 128, 1, 64, torch.float32),             # single partial block, r = 1
+])
+def test_sketch(sw, seqlens, heads, d, r, B, dtype):
+    torch.manual_seed(0)
+    T = sum(seqlens)
+    x = (torch.randn(T, heads, d) * 2 + 0.3).to(dtype)
+    signs, cols, H = H_of(d, r)
+    L = sw.make_layout(seqlens, B)
+    sk = torch.empty(L.total_blocks, r, device="cuda"); mean = torch.empty(L.total_blocks, d, device="cuda")
+    sw.sw_sketch(L, x.cuda(), dev(signs), dev(cols), r, 1 / math.sqrt(r), sk, mean)
+    xn = gen.to_numpy_f64(x)
+    ref_mean, ref_sk, lo = [], [], 0
+    for n in seqlens:
+        m = O.block_mean(O.head_mean(xn[lo:lo + n]), B)
+        ref_mean.append(m); ref_sk.append(O.sketch(m, H)); lo += n
+    ref_mean, ref_sk = np.concatenate(ref_mean), np.concatenate(ref_sk)
+    assert rowwise_close(mean.cpu().numpy(), ref_mean)
+    assert rowwise_close(sk.cpu().numpy(), ref_sk)
+
+
+def test_sketch_strided_and_nosigns(sw):
+    torch.manual_seed(1)
+    T, heads, d, r, B = 200, 4, 128, 64, 64
+    big = torch.randn(T, heads + 2, d + 8, dtype=torch.float32).to(torch.bfloat16).cuda()
+    x = big[:, 1:1 + heads, 8:]                          # non-compact strides, 16-byte aligned
+    _, cols, _ = H_of(d, r)
+    H = O.srht_matrix(d, np.ones(d), cols, 1 / math.sqrt(r))
+    L = sw.make_layout((T,), B)
+    sk = torch.empty(L.total_blocks, r, device="cuda")
+    sw.sw_sketch(L, x, None, dev(cols), r, 1 / math.sqrt(r), sk, None)
+    ref = O.sketch(O.block_mean(O.head_mean(gen.to_numpy_f64(x)), B), H)
+    assert rowwise_close(sk.cpu().numpy(), ref)
+
+
+# ------------------------------------------------------------------------------ block scores
+FLAG_SETS = [O.DEFAULT_FLAGS, O.DEFAULT_FLAGS & ~O.SCORE_SOFTMAX, O.DEFAULT_FLAGS & ~O.CAUSAL,
+             O.DEFAULT_FLAGS | O.POW_MATRIX, 0]
+
+
+@pytest.mark.parametrize("blocks", [(16,), (100,), (37, 130, 64)])
+@pytest.mark.parametrize("flags", FLAG_SETS)
+@pytest.mark.parametrize("s", [1, 2, 3])
+def test_block_scores(sw, blocks, flags, s):
+    rng = np.random.RandomState(3)
+    r, B = 64, 64
+    L = sw.make_layout([b * B for b in blocks], B)
+    qs = rng.randn(L.total_blocks, r).astype(np.float32) * 1.5
+    ks = rng.randn(L.total_blocks, r).astype(np.float32) * 1.5
+    W = torch.full((L.total_sq,), float("nan"), device="cuda"); A = torch.full_like(W, float("nan"))
+    sw.sw_block_scores(L, dev(qs), dev(ks), r, s, flags, W, A)
+    Wn, An = W.cpu().numpy(), A.cpu().numpy()
+    lo = off = 0
+    for b in blocks:
+        S = O.block_scores(qs[lo:lo + b].astype(np.float64), ks[lo:lo + b].astype(np.float64))
+        A_ref = O.masked_softmax(S, flags)
+        W_ref = A_ref if (flags & O.POW_MATRIX) else O.power(A_ref, s, flags)
+        assert rowwise_close(An[off:off + b * b].reshape(b, b), A_ref)
+        assert rowwise_close(Wn[off:off + b * b].reshape(b, b), W_ref)
+        lo += b; off += b * b
+
+
+# ------------------------------------------------------------------------------ walk
+@pytest.mark.parametrize("blocks", [(16,), (100,), (300,), (37, 130, 64)])
+@pytest.mark.parametrize("flags", [O.DEFAULT_FLAGS, O.DEFAULT_FLAGS & ~O.ROWNORM, O.DEFAULT_FLAGS & ~O.CAUSAL,
+                                   O.DEFAULT_FLAGS | O.POW_MATRIX])
+def test_walk_update(sw, blocks, flags):
+    rng = np.random.RandomState(4)
+    B, s = 64, 3
+    L = sw.make_layout([b * B for b in blocks], B)
+    As, Rs = [], []
+    for b in blocks:
+        As.append(O.masked_softmax(rng.randn(b, b) * 2, flags))
+        Rs.append(O.masked_softmax(rng.randn(b, b) * 2, flags))
+    mat = bool(flags & O.POW_MATRIX)
+    Wsrc = [a if mat else O.power(a, s, flags) for a in As]
+    Wd = dev(np.concatenate([w.ravel() for w in Wsrc]), torch.float32)
+    Rp = dev(np.concatenate([r.ravel() for r in Rs]), torch.float32)
+    ws = torch.empty(sw.sw_workspace_bytes(sw.SW_OP_WALK_UPDATE, L), dtype=torch.uint8, device="cuda")
+    for prev in (None, Rp):
+        out = torch.full((L.total_sq,), float("nan"), device="cuda")
+        sw.sw_walk_update(L, prev, Wd, s, flags, out, ws)
+        on = out.cpu().numpy(); off = 0
+        for k, b in enumerate(blocks):
+            # the oracle gets the fp32-rounded operands the GPU saw
+            A32 = Wsrc[k].astype(np.float32).astype(np.float64) if mat else None
+            if mat:
+                ref = O.walk_update(None if prev is None else Rs[k].astype(np.float32).astype(np.float64),
+                                    A32, s, flags)
+            else:
+                W32 = Wsrc[k].astype(np.float32).astype(np.float64)
+                R0 = np.eye(b) if prev is None else Rs[k].astype(np.float32).astype(np.float64)
+                ref = R0 @ W32
+                if flags & O.ROWNORM:
+                    ref = O.row_rescale(ref)
+            assert rowwise_close(on[off:off + b * b].reshape(b, b), ref)
+            off += b * b
+
+
+def test_walk_s1_identity_is_block_scores(sw):
+    # north_star: s = 1, R^0 = I  =>  R == A (one-hop)
+    rng = np.random.RandomState(8)
+    b, B = 80, 64
+    L = sw.make_layout([b * B], B)
+    A = O.masked_softmax(rng.randn(b, b), O.DEFAULT_FLAGS).astype(np.float32)
+    out = torch.empty(b * b, device="cuda")
+    sw.sw_walk_update(L, None, dev(A.ravel()), 1, O.DEFAULT_FLAGS & ~O.ROWNORM, out, None)
+    assert np.array_equal(out.cpu().numpy().reshape(b, b), A)
+
+
+# ------------------------------------------------------------------------------ select
+@pytest.mark.parametrize("blocks,taus", [((16,), (4,)), ((100,), (20,)), ((300,), (60,)), ((37, 130, 64), (8, 26, 13)),
+                                         ((50,), (1,)), ((50,), (2,)), ((20,), (64,))])
+@pytest.mark.parametrize("flags", [O.DEFAULT_FLAGS, O.DEFAULT_FLAGS & ~O.CAUSAL, O.CAUSAL, O.CAUSAL | O.FORCE_FIRST,
+                                   O.CAUSAL | O.FORCE_LAST])
+def test_select_topk_bit_exact_given_oracle_scores(sw, blocks, taus, flags):
+    rng = np.random.RandomState(6)
+    B = 64
+    L = sw.make_layout([b * B for b in blocks], B)
+    Rs = []
+    for b in blocks:
+        R = rng.rand(b, b).astype(np.float32)
+        R[rng.rand(b, b) < 0.3] = 0.25                        # deliberate ties
+        R[rng.rand(b, b) < 0.05] = 0.0
+        if flags & O.CAUSAL:
+            R = np.tril(R)
+        Rs.append(R)
+    tau_max = max(taus) + 3
+    idx = torch.full((L.total_blocks, tau_max), -7, dtype=torch.int32, device="cuda")
+    cnt = torch.full((L.total_blocks,), -7, dtype=torch.int32, device="cuda")
+    sw.sw_select_topk(L, dev(np.concatenate([r.ravel() for r in Rs])), dev(np.asarray(taus, np.int32)), tau_max,
+                      flags, idx, cnt)
+    idx, cnt = idx.cpu().numpy(), cnt.cpu().numpy()
+    lo = 0
+    for b, tau, R in zip(blocks, taus, Rs):
+        ref_idx, ref_cnt = O.select_topk(R.astype(np.float64), tau, flags)
+        assert np.array_equal(cnt[lo:lo + b], ref_cnt)
+        assert np.array_equal(idx[lo:lo + b, :tau], ref_idx)
+        assert (idx[lo:lo + b, tau:] == -1).all()
+        lo += b
+
+
+def test_select_topk_negative_nan_inf(sw):
+    rng = np.random.RandomState(9)
+    b, B, tau = 70, 64, 9
+    R = rng.randn(b, b).astype(np.float32)
+    R[5, 2] = np.nan; R[9, 1] = -np.inf; R[11, 3] = np.inf; R[20, :8] = -0.0; R[20, 8:12] = 0.0
+    flags = O.CAUSAL
+    L = sw.make_layout([b * B], B)
+    idx = torch.empty(b, tau, dtype=torch.int32, device="cuda"); cnt = torch.empty(b, dtype=torch.int32, device="cuda")
+    sw.sw_select_topk(L, dev(R.ravel()), dev(np.asarray([tau], np.int32)), tau, flags, idx, cnt)
+    ref_idx, ref_cnt = O.select_topk(R.astype(np.float64), tau, flags)
+    assert np.array_equal(idx.cpu().numpy(), ref_idx) and np.array_equal(cnt.cpu().numpy(), ref_cnt)
+
+
+# ------------------------------------------------------------------------------ prefill attention
+def random_lists(rng, b, tau, causal=True):
+    R = rng.rand(b, b)
+    return O.select_topk(np.tril(R) if causal else R, tau, O.DEFAULT_FLAGS if causal else (O.DEFAULT_FLAGS & ~O.CAUSAL))
+
+
+def attn_case(sw, seqlens, h_q, h_kv, d, B, tau_frac, dtype, causal=True, seed=0, heads_checked=None):
+    rng = np.random.RandomState(seed)
+    torch.manual_seed(seed)
+    T = sum(seqlens)
+    q = torch.randn(T, h_q, d).to(dtype); k = torch.randn(T, h_kv, d).to(dtype); v = torch.randn(T, h_kv, d).to(dtype)
+    L = sw.make_layout(seqlens, B)
+    flags = O.DEFAULT_FLAGS if causal else (O.DEFAULT_FLAGS & ~O.CAUSAL)
+    taus = [max(1, int(math.ceil(tau_frac * b))) for b in L.blocks]
+    tau_max = max(taus)
+    idx_all = np.full((L.total_blocks, tau_max), -1, np.int32); cnt_all = np.zeros(L.total_blocks, np.int32)
+    lo = 0
+    for b, tau in zip(L.blocks, taus):
+        i, c = random_lists(rng, b, tau, causal)
+        idx_all[lo:lo + b, :tau] = i; cnt_all[lo:lo + b] = c; lo += b
+    out = torch.full((T, h_q, d), float("nan"), dtype=dtype, device="cuda")
+    lse = torch.empty(T, h_q, device="cuda")
+    ws = torch.empty(sw.sw_workspace_bytes(sw.SW_OP_ATTN_PREFILL, L, h_q, h_kv, d, tau_max,
+                                           sw.SW_F32 if dtype == torch.float32 else sw.SW_BF16) + 16,
+                     dtype=torch.uint8, device="cuda")
+    scale = 1 / math.sqrt(d)
+    sw.sw_sparse_attn_prefill(L, q.cuda(), k.cuda(), v.cuda(), dev(idx_all), dev(cnt_all), tau_max, scale, flags, out,
+                              lse, ws)
+    # the oracle sees what the tensor cores see: operands rounded to bf16 (P17)
+    qn, kn, vn = (gen.to_numpy_f64(t.to(torch.bfloat16)) for t in (q, k, v))
+    got, got_lse = out.float().cpu().numpy(), lse.cpu().numpy()
+    assert np.isfinite(got).all()
+    tlo = blo = 0
+    for n, b in zip(seqlens, L.blocks):
+        ref, ref_lse = O.sparse_attention(qn[tlo:tlo + n], kn[tlo:tlo + n], vn[tlo:tlo + n], idx_all[blo:blo + b],
+                                          cnt_all[blo:blo + b], B, scale, flags, q_heads=heads_checked, return_lse=True)
+        hs = list(range(h_q)) if heads_checked is None else heads_checked
+        err = np.abs(got[tlo:tlo + n][:, hs] - ref[:, hs])
+        assert err.max() <= ATT_MAX and err.mean() <= ATT_MEAN, (err.max(), err.mean())
+        assert np.abs(got_lse[tlo:tlo + n][:, hs] - ref_lse[:, hs]).max() <= 2e-2
+        tlo += n; blo += b
+
+
+@pytest.mark.parametrize("case", [
+    dict(seqlens=(1024,), h_q=1, h_kv=1, d=64, B=64, tau_frac=0.25, dtype=torch.float32),      # cfg 1 shape
+    dict(seqlens=(1000,), h_q=8, h_kv=2, d=128, B=64, tau_frac=0.2, dtype=torch.bfloat16),     # GQA 4, ragged
+    dict(seqlens=(700,), h_q=4, h_kv=4, d=128, B=128, tau_frac=0.5, dtype=torch.bfloat16),     # B = 128, MHA
+    dict(seqlens=(130, 64, 257), h_q=4, h_kv=1, d=64, B=64, tau_frac=0.5, dtype=torch.bfloat16),  # varlen
+    dict(seqlens=(515,), h_q=8, h_kv=2, d=128, B=64, tau_frac=1.0, dtype=torch.bfloat16),      # 100 % density
+    dict(seqlens=(320,), h_q=2, h_kv=1, d=128, B=64, tau_frac=0.6, dtype=torch.bfloat16, causal=False),
+    dict(seqlens=(40,), h_q=2, h_kv=2, d=64, B=64, tau_frac=1.0, dtype=torch.bfloat16),        # one partial block
+])
+def test_sparse_attn_prefill(sw, case):
+    attn_case(sw, **case)
+
+
+def test_sparse_attn_prefill_full_density_is_dense_causal(sw):
+    # north_star pin, on the GPU path: 100 % density == dense causal softmax attention (torch SDPA fp64)
+    torch.manual_seed(3)
+    n, h_q, h_kv, d, B = 448, 8, 2, 128, 64
+    q = torch.randn(n, h_q, d).bfloat16(); k = torch.randn(n, h_kv, d).bfloat16(); v = torch.randn(n, h_kv, d).bfloat16()
+    b = n // B
+    L = sw.make_layout((n,), B)
+    idx = np.tile(np.arange(b, dtype=np.int32), (b, 1)); cnt = np.arange(1, b + 1, dtype=np.int32)
+    idx = np.where(np.arange(b)[None, :] <= np.arange(b)[:, None], idx, -1).astype(np.int32)
+    out = torch.empty(n, h_q, d, dtype=torch.bfloat16, device="cuda")
+    sw.sw_sparse_attn_prefill(L, q.cuda(), k.cuda(), v.cuda(), dev(idx), dev(cnt), b, 1 / math.sqrt(d),
+                              O.DEFAULT_FLAGS, out, None, None)
+    qq = q.double().permute(1, 0, 2)[None]
+    kk = k.double().permute(1, 0, 2).repeat_interleave(4, 0)[None]
+    vv = v.double().permute(1, 0, 2).repeat_interleave(4, 0)[None]
+    ref = torch.nn.functional.scaled_dot_product_attention(qq, kk, vv, is_causal=True)[0].permute(1, 0, 2).numpy()
+    err = np.abs(out.float().cpu().numpy() - ref)
+    assert err.max() <= ATT_MAX and err.mean() <= ATT_MEAN
+
+
+# ------------------------------------------------------------------------------ decode attention
+@pytest.mark.parametrize("ts,h_q,h_kv,d,B,tau", [
+    ((64 * 9 + 1, 64 * 9 + 32, 64 * 10), 32, 8, 128, 64, 5),      # t mod B in {1, B/2, 0}
+    ((700,), 8, 2, 128, 64, 11),                                     # all blocks selected
+    ((300, 90), 4, 4, 64, 64, 3),
+    ((1000, 513), 16, 2, 128, 128, 4),                               # B = 128, group 8
+])
+def test_sparse_attn_decode(sw, ts, h_q, h_kv, d, B, tau):
+    rng = np.random.RandomState(2)
+    torch.manual_seed(2)
+    batch, tmax = len(ts), max(ts)
+    q = torch.randn(batch, h_q, d).bfloat16()
+    kc = torch.randn(batch, tmax, h_kv, d).bfloat16(); vc = torch.randn(batch, tmax, h_kv, d).bfloat16()
+    idx = np.full((batch, tau), -1, np.int32); cnt = np.zeros(batch, np.int32)
+    for s_, t in enumerate(ts):
+        bq = (t - 1) // B
+        sel = O.select_topk_row(rng.rand(bq + 1), bq, tau, O.DEFAULT_FLAGS)
+        idx[s_, :len(sel)] = sel; cnt[s_] = len(sel)
+    out = torch.full((batch, h_q, d), float("nan"), dtype=torch.bfloat16, device="cuda")
+    lse = torch.empty(batch, h_q, device="cuda")
+    ws = torch.empty(sw.sw_decode_workspace_bytes(batch, h_q, h_kv, d, tau), dtype=torch.uint8, device="cuda")
+    scale = 1 / math.sqrt(d)
+    sw.sw_sparse_attn_decode(batch, B, q.cuda(), kc.cuda(), vc.cuda(), dev(np.asarray(ts, np.int32)), dev(idx),
+                             dev(cnt), tau, scale, out, lse, ws)
+    got = out.float().cpu().numpy()
+    for s_, t in enumerate(ts):
+        ref = O.decode_attention(gen.to_numpy_f64(q[s_]), gen.to_numpy_f64(kc[s_, :t]), gen.to_numpy_f64(vc[s_, :t]),
+                                 idx[s_, :cnt[s_]], B, scale)
+        err = np.abs(got[s_] - ref)
+        assert err.max() <= ATT_MAX and err.mean() <= ATT_MEAN, (err.max(), err.mean())
+
+
+# ------------------------------------------------------------------------------ decode selection path
+@pytest.mark.parametrize("t", [64 * 5 + 1, 64 * 5 + 32, 64 * 6])
+def test_decode_selection_matches_literal_alg2(sw, t):
+    """Row-vector GPU path (sketch_append, block_scores_row, walk_update_row, select_topk_row) against the
+    oracle's literal full-matrix Alg. 2, three layers, caches built by the GPU prefill path."""
+    cfg = gen.CONFIGS[2]
+    B, r, s, d, h_q, h_kv = cfg.B, cfg.r, cfg.s, cfg.d, 8, 2
+    signs, cols, H = H_of(d, r, seed=3)
+    flags = O.DEFAULT_FLAGS
+    n_pre = t - 1
+    b_pre, mb = O.num_blocks(n_pre, B), O.num_blocks(t, B)
+    tau = 4
+    dp = sw.DecodePipeline(1, mb, h_q, h_kv, d, B, r, s, [tau], signs, cols, flags)
+    R_full = None
+    for layer in range(3):
+        torch.manual_seed(100 + layer)
+        Q = (torch.randn(t, h_q, d) + 0.5).bfloat16(); K = (torch.randn(t, h_kv, d) + 0.5).bfloat16()
+        # caches from the GPU prefill selection path over the first t-1 tokens
+        pp = sw.PrefillPipeline([n_pre], h_q, h_kv, d, B, r, s, 0.5, signs, cols, flags)
+        pp.select(Q[:n_pre].cuda(), K[:n_pre].cuda())
+        kbar = torch.zeros(1, mb, d, device="cuda"); ks = torch.zeros(1, mb, r, device="cuda")
+        kbar[0, :b_pre] = pp.kbar; ks[0, :b_pre] = pp.ks
+        Wc = torch.zeros(1, mb, mb, device="cuda")
+        Wc[0, :b_pre, :b_pre] = pp.W.view(b_pre, b_pre)
+        seqlens = dev(np.asarray([t], np.int32))
+        dp.select(Q[t - 1:t].cuda(), K[t - 1:t].cuda(), seqlens, kbar, ks, Wc)
+        torch.cuda.synchronize()
+        # oracle, literal
+        Qn, Kn = gen.to_numpy_f64(Q), gen.to_numpy_f64(K)
+        pre = O.prefill_selection(Qn[:n_pre], Kn[:n_pre], None, B=B, H_d=H, s=s, tau=tau, flags=flags)
+        sel, R_full, cache2 = O.decode_layer_literal(Qn[t - 1], Kn[t - 1], O.DecodeCache(pre.qbar, pre.kbar, pre.S), t,
+                                                     R_full, B=B, H_d=H, s=s, tau=tau, flags=flags)
+        bq = (t - 1) // B
+        assert rowwise_close(kbar[0].cpu().numpy(), cache2.kbar)
+        assert rowwise_close(dp.rvec[dp.cur][0, :bq + 1].cpu().numpy()[None], R_full[bq][None, :bq + 1], rel=2e-3)
+        got = dp.idx[0, :dp.count[0].item()].cpu().numpy()
+        ref_r = R_full[bq]
+        if not np.array_equal(got, sel):                     # only near-ties may differ
+            diff = set(got.tolist()) ^ set(sel.tolist())
+            thr = np.sort(ref_r[1:bq])[::-1][tau - 3]        # (tau-2)-th largest non-forced candidate
+            assert all(abs(ref_r[j] - thr) <= 1e-3 * np.abs(ref_r).max() for j in diff)
+        assert bq in got
+
+
+# ------------------------------------------------------------------------------ end to end
+def check_overlap(idx_gpu, cnt_gpu, sel, R_ref):
+    b = R_ref.shape[0]
+    inter = tot = 0
+    for i in range(b):
+        g_ = set(idx_gpu[i, :cnt_gpu[i]].tolist()); o_ = set(sel.idx[i, :sel.count[i]].tolist())
+        assert cnt_gpu[i] == sel.count[i]
+        inter += len(g_ & o_); tot += len(o_)
+        if g_ != o_:                                           # differences only at near-ties
+            row = R_ref[i]; scale = np.abs(row).max()
+            free = [j for j in o_ if j not in (0, i)]
+            kth = min(row[free]) if free else 0.0
+            for j in g_ ^ o_:
+                assert abs(row[j] - kth) <= 1e-3 * scale, (i, j, row[j], kth)
+    return inter / tot
+
+
+@pytest.mark.parametrize("cfg_idx,seqlens,layers", [(0, None, 2), (1, (2048 + 19,), 4), (4, (192, 700, 1024), 3)])
+def test_end_to_end_prefill_stack(sw, cfg_idx, seqlens, layers):
+    """Whole hot path, several layers with the walk carried across them; cfg 1 in full, cfg 2 / cfg 5 recipes
+    at reduced length (full-size samples live in test_gpu_fullsize.py)."""
+    cfg = gen.CONFIGS[cfg_idx]
+    seqlens = tuple(cfg.seqlens if seqlens is None else seqlens)
+    signs, cols, H = H_of(cfg.d, cfg.r, seed=cfg_idx + 1)
+    dtype = torch.float32 if cfg.dtype == "f32" else torch.bfloat16
+    pipe = sw.PrefillPipeline(seqlens, cfg.h_q, cfg.h_kv, cfg.d, cfg.B, cfg.r, cfg.s, cfg.density, signs, cols,
+                              dtype=dtype, keep_A=True)
+    plans = gen.make_plans(cfg_idx, seqlens) if cfg.planted else None
+    R_ref = [None] * len(seqlens)
+    for layer in range(layers):
+        li = gen.layer_inputs(cfg_idx, layer, device="cuda", seqlens=seqlens, plans=plans)
+        out = pipe.layer(li.Q, li.K, li.V)
+        torch.cuda.synchronize()
+        Qn, Kn, Vn = (gen.to_numpy_f64(x) for x in (li.Q, li.K, li.V))
+        idx_gpu, cnt_gpu = pipe.idx.cpu().numpy(), pipe.count.cpu().numpy()
+        R_gpu = pipe.R_cur.cpu().numpy()
+        got = out.float().cpu().numpy()
+        tlo = blo = qlo = 0
+        for si, n in enumerate(seqlens):
+            b = O.num_blocks(n, cfg.B)
+            tau = O.tau_from_density(cfg.density, b)
+            sel = O.prefill_selection(Qn[tlo:tlo + n], Kn[tlo:tlo + n], R_ref[si], B=cfg.B, H_d=H, s=cfg.s, tau=tau)
+            R_ref[si] = sel.R
+            assert rowwise_close(pipe.qs[blo:blo + b].cpu().numpy(), sel.qs)
+            assert rowwise_close(pipe.W[qlo:qlo + b * b].cpu().numpy().reshape(b, b), sel.W)
+            assert rowwise_close(R_gpu[qlo:qlo + b * b].reshape(b, b), sel.R)
+            ov = check_overlap(idx_gpu[blo:blo + b], cnt_gpu[blo:blo + b], sel, sel.R)
+            assert ov >= 0.99, ov
+            heads = sorted(set([0, cfg.h_q // 2, cfg.h_q - 1]))
+            qb = torch.as_tensor(Qn[tlo:tlo + n]).bfloat16().double().numpy()
+            kb = torch.as_tensor(Kn[tlo:tlo + n]).bfloat16().double().numpy()
+            vb = torch.as_tensor(Vn[tlo:tlo + n]).bfloat16().double().numpy()
+            ref = O.sparse_attention(qb, kb, vb, idx_gpu[blo:blo + b], cnt_gpu[blo:blo + b], cfg.B,
+                                     1 / math.sqrt(cfg.d), q_heads=heads)
+            err = np.abs(got[tlo:tlo + n][:, heads] - ref[:, heads])
+            assert err.max() <= ATT_MAX and err.mean() <= ATT_MEAN, (err.max(), err.mean())
+            tlo += n; blo += b; qlo += b * b

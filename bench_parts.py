@@ -1,0 +1,288 @@
+"""Timed regions of bench.py (prefill stack = the headline; decode step = extra keys)."""
+from __future__ import annotations
+
+import math
+import os
+import statistics
+import time
+
+import numpy as np
+import torch
+
+from synth import gen
+
+CFG_IDX = 1
+METRIC = "prefill_tokens_per_s_per_layer_at_20pct_density"
+UNIT = "tokens/s"
+KERNELS = ["sketch_q", "sketch_k", "block_scores", "walk", "select", "attn"]
+ROOT = os.path.dirname(os.path.abspath(__file__))
+
+
+def tile_pairs(b: int, tau: int) -> int:
+    return sum(min(tau, i + 1) for i in range(b))
+
+
+def _ncu_traffic(kernel: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu summary, or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        import json
+        return json.load(open(p)).get(kernel)
+    except Exception:
+        return None
+
+
+def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
+    cfg = gen.CONFIGS[CFG_IDX]
+    n = args.seqlen or cfg.seqlens[0]
+    layers = args.layers or cfg.layers
+    dev = torch.device("cuda", torch.cuda.current_device())
+    signs, cols = gen.srht_params(CFG_IDX + 1, cfg.d, cfg.r)
+    pipe = pkg.PrefillPipeline([n], cfg.h_q, cfg.h_kv, cfg.d, cfg.B, cfg.r, cfg.s, cfg.density, signs, cols)
+    b = pipe.L.blocks[0]
+    tau = pipe.tau_max
+    pairs = tile_pairs(b, tau)
+
+    # inputs: all layers resident in HBM (32 x 403 MB), each rank its own seeds (weak scaling)
+    plans = gen.make_plans(CFG_IDX, (n,))
+    Qs, Ks, Vs = [], [], []
+    for layer in range(layers):
+        g = torch.Generator(device=dev)  # noqa: F841  (generator lives inside gen.planted_qkv)
+        q, k, v = gen.planted_qkv(1000 * (CFG_IDX + 1) + layer + 100003 * rank, n, cfg.h_q, cfg.h_kv, cfg.d, cfg.B,
+                                  torch.bfloat16, plans[0].queries[layer], plans[0].targets[layer], device=str(dev))
+        Qs.append(q); Ks.append(k); Vs.append(v)
+    outs = [torch.empty(n, cfg.h_q, cfg.d, dtype=torch.bfloat16, device=dev) for _ in range(2)]
+    torch.cuda.synchronize()
+    stream = torch.cuda.current_stream()
+
+    def step(events=None):
+        pipe.reset()
+        L = pipe.L
+        for layer in range(layers):
+            Q, K, V = Qs[layer], Ks[layer], Vs[layer]
+            ev = events[layer] if events is not None else None
+            if ev is not None: ev[0].record(stream)
+            pkg.sw_sketch(L, Q, pipe.signs, pipe.cols, pipe.r, pipe.sketch_scale, pipe.qs, pipe.qbar)
+            if ev is not None: ev[1].record(stream)
+            pkg.sw_sketch(L, K, pipe.signs, pipe.cols, pipe.r, pipe.sketch_scale, pipe.ks, pipe.kbar)
+            if ev is not None: ev[2].record(stream)
+            pkg.sw_block_scores(L, pipe.qs, pipe.ks, pipe.r, pipe.s, pipe.flags, pipe.W, None)
+            if ev is not None: ev[3].record(stream)
+            nxt = 0 if pipe.cur < 0 else 1 - pipe.cur
+            pkg.sw_walk_update(L, pipe.R_cur, pipe.W, pipe.s, pipe.flags, pipe.R[nxt], pipe.walk_ws)
+            pipe.cur = nxt
+            if ev is not None: ev[4].record(stream)
+            pkg.sw_select_topk(L, pipe.R[nxt], pipe.tau, pipe.tau_max, pipe.flags, pipe.idx, pipe.count)
+            if ev is not None: ev[5].record(stream)
+            pkg.sw_sparse_attn_prefill(L, Q, K, V, pipe.idx, pipe.count, pipe.tau_max, pipe.softmax_scale,
+                                       pipe.flags, outs[layer & 1], None, pipe.attn_ws)
+            if ev is not None: ev[6].record(stream)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    events = [[[torch.cuda.Event(enable_timing=True) for _ in range(7)] for _ in range(layers)]
+              for _ in range(args.steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    e0.record(stream)
+    for k in range(args.steps):
+        step(events[k])
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms_total], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * n * layers / (ms_step * 1e-3)
+
+    # per-kernel device times (CUDA events on the launching stream, inside the timed region)
+    per = {k: [] for k in KERNELS}
+    for st in events:
+        for ev in st:
+            for i, k in enumerate(KERNELS):
+                per[k].append(ev[i].elapsed_time(ev[i + 1]))
+    kern_ms = {k: statistics.mean(v) for k, v in per.items()}
+    attn_ms = kern_ms["attn"]
+    attn_flops = 4.0 * cfg.B * cfg.B * cfg.d * cfg.h_q * pairs          # full tile counted for the diagonal
+    achieved = attn_flops / (attn_ms * 1e-3) / 1e12
+    peak = peaks.get("bf16_tflops_sustained", peaks.get("bf16_tflops"))
+    sel_ms = sum(kern_ms[k] for k in KERNELS[:5])
+    layer_ms = ms_step / layers
+    sketch_bytes = n * (cfg.h_q + cfg.h_kv) * cfg.d * 2
+    sketch_gbs = sketch_bytes / ((kern_ms["sketch_q"] + kern_ms["sketch_k"]) * 1e-3) / 1e9
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic",
+        "config": {"workload": cfg.name if (n, layers) == (cfg.seqlens[0], cfg.layers) else f"DEBUG n={n} L={layers}",
+                   "layers": layers, "seq_len": n, "h_q": cfg.h_q, "h_kv": cfg.h_kv, "head_dim": cfg.d,
+                   "block": cfg.B, "blocks": b, "tau": tau, "sketch_dim": cfg.r, "walk_power_s": cfg.s,
+                   "density": cfg.density, "tile_pairs_per_layer": pairs,
+                   "l2": "inputs larger than L2: 32 distinct layers x 403 MB cycle through the 126 MB L2",
+                   "generator": {"coherence_a": gen.COHERENCE_A, "plant_cos": gen.PLANT_COS,
+                                 "plant_frac": gen.PLANT_FRAC, "chain_frac": gen.CHAIN_FRAC, "sink_a": gen.SINK_A}},
+        "ms_per_layer": layer_ms,
+        "kernel_ms_per_layer": kern_ms,
+        "selection_overhead_share": sel_ms / (sel_ms + attn_ms),
+        "sketch_hbm": {"achieved_gbs": sketch_gbs, "peak_gbs": peaks.get("hbm_gbs"),
+                       "frac": sketch_gbs / peaks.get("hbm_gbs")},
+        "roofline": {"kernel": "sw_sparse_attn_prefill", "bound": "tensor", "achieved": achieved, "peak": peak,
+                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": _ncu_traffic("sw_sparse_attn_prefill"),
+                     "peak_source": f"{peaks['_source']} bf16 sustained (kernel timed inside a long step)",
+                     "flops_per_launch": attn_flops, "ms_per_launch": attn_ms,
+                     "whole_layer_frac": (attn_flops / peak / 1e12) / (layer_ms * 1e-3)},
+        "clocks": clocks,
+        "gpu_launches": args.steps * layers * 7,   # 2 sketch + scores + (walk gemm | copy) + rownorm + select + attn
+    }
+    res = {"line": line, "n": n, "pipe": pipe, "Qs": Qs, "Ks": Ks, "Vs": Vs, "outs": outs}
+
+    # ---- e2e: the same stack through the public API with HOST buffers (pinned), H2D of every layer's
+    # Q/K/V and D2H of every layer's output inside the timed region, copies overlapped on a second stream
+    if not args.no_e2e:
+        nh = min(2, layers)
+        hQ = [torch.empty(Qs[0].shape, dtype=torch.bfloat16).pin_memory() for _ in range(nh)]
+        hK = [torch.empty(Ks[0].shape, dtype=torch.bfloat16).pin_memory() for _ in range(nh)]
+        hV = [torch.empty(Vs[0].shape, dtype=torch.bfloat16).pin_memory() for _ in range(nh)]
+        for i in range(nh):
+            hQ[i].copy_(Qs[i]); hK[i].copy_(Ks[i]); hV[i].copy_(Vs[i])
+        hO = torch.empty(outs[0].shape, dtype=torch.bfloat16).pin_memory()
+        dQ = [torch.empty_like(Qs[0]) for _ in range(2)]
+        dK = [torch.empty_like(Ks[0]) for _ in range(2)]
+        dV = [torch.empty_like(Vs[0]) for _ in range(2)]
+        copy_s = torch.cuda.Stream()
+        ready = [torch.cuda.Event() for _ in range(2)]
+        freed = [torch.cuda.Event() for _ in range(2)]
+        odone = [torch.cuda.Event() for _ in range(2)]
+
+        def e2e_step():
+            pipe.reset()
+            for layer in range(layers):
+                sl = layer & 1
+                with torch.cuda.stream(copy_s):
+                    if layer >= 2:
+                        copy_s.wait_event(freed[sl])
+                    dQ[sl].copy_(hQ[layer % nh], non_blocking=True)
+                    dK[sl].copy_(hK[layer % nh], non_blocking=True)
+                    dV[sl].copy_(hV[layer % nh], non_blocking=True)
+                    ready[sl].record(copy_s)
+                stream.wait_event(ready[sl])
+                if layer >= 2:
+                    stream.wait_event(odone[sl])
+                pipe.layer(dQ[sl], dK[sl], dV[sl], out=outs[sl])
+                freed[sl].record(stream)
+                with torch.cuda.stream(copy_s):
+                    copy_s.wait_event(freed[sl])
+                    hO.copy_(outs[sl], non_blocking=True)
+                    odone[sl].record(copy_s)
+            copy_s.synchronize()
+
+        e2e_steps = max(1, min(args.steps, 2))
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            e2e_step()
+        barrier()
+        dt = (time.perf_counter() - t0) / e2e_steps
+        if dist is not None:
+            t = torch.tensor([dt], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        h2d = layers * (Qs[0].numel() + Ks[0].numel() + Vs[0].numel()) * 2
+        d2h = layers * outs[0].numel() * 2
+        line["e2e"] = {"value": world * n * layers / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                       "d2h_bytes_per_step": d2h, "ms_per_step": dt * 1e3, "steps": e2e_steps,
+                       "note": "pinned host Q/K/V -> device, every layer's output -> host; copies overlap compute"}
+    return res
+
+
+def decode_bench(pkg, args, peaks, n_layer_bufs: int = 4, steps: int = 20):
+    """cfg 3: batch 8 x 131072-token KV cache, one new token per sequence, 20 % density.  Reports the
+    per-layer decode time (selection + attention) and the attention kernel's HBM fraction over the
+    selected K/V bytes.  ``n_layer_bufs`` distinct layer caches (4.3 GB each >> L2) are cycled."""
+    cfg = gen.CONFIGS[2]
+    dev = torch.device("cuda", torch.cuda.current_device())
+    batch, t = len(cfg.seqlens), cfg.seqlens[0]
+    B, d, r = cfg.B, cfg.d, cfg.r
+    mb = (t + B - 1) // B
+    tau = pkg.tau_from_density(cfg.density, mb)
+    signs, cols = gen.srht_params(3, d, r)
+    free, _ = torch.cuda.mem_get_info()
+    per_layer = batch * t * cfg.h_kv * d * 2 * 2 + batch * mb * mb * 4
+    n_layer_bufs = max(1, min(n_layer_bufs, int(free * 0.6 // per_layer)))
+    dp = pkg.DecodePipeline(batch, mb, cfg.h_q, cfg.h_kv, d, B, r, cfg.s, [tau] * batch, signs, cols)
+    seqlens = torch.full((batch,), t, dtype=torch.int32, device=dev)
+    layers = []
+    for l in range(n_layer_bufs):
+        kc = torch.empty(batch, t, cfg.h_kv, d, dtype=torch.bfloat16, device=dev)
+        vc = torch.empty_like(kc)
+        Wc = torch.empty(batch, mb, mb, dtype=torch.float32, device=dev)
+        kbar = torch.empty(batch, mb, d, dtype=torch.float32, device=dev)
+        ks = torch.empty(batch, mb, r, dtype=torch.float32, device=dev)
+        q_new = torch.empty(batch, cfg.h_q, d, dtype=torch.bfloat16, device=dev)
+        k_new = torch.empty(batch, cfg.h_kv, d, dtype=torch.bfloat16, device=dev)
+        for s_ in range(batch):
+            plan = gen.plant_plan(3000 + 7919 * s_, cfg.layers, mb)
+            q, k, v = gen.planted_qkv(3000 + l + 7919 * s_, t, cfg.h_q, cfg.h_kv, d, B, torch.bfloat16,
+                                      plan.queries[l], plan.targets[l], device=str(dev))
+            kc[s_].copy_(k); vc[s_].copy_(v)
+            q_new[s_].copy_(q[t - 1]); k_new[s_].copy_(k[t - 1])
+            # caches from the prefill selection path over the first t-1 tokens (untimed set-up)
+            pp = pkg.PrefillPipeline([t - 1], cfg.h_q, cfg.h_kv, d, B, r, cfg.s, cfg.density, signs, cols)
+            pp.select(q[:t - 1], k[:t - 1])
+            Wc[s_].copy_(pp.W.view(mb, mb)); kbar[s_].copy_(pp.kbar); ks[s_].copy_(pp.ks)
+            del q, k, v, pp
+        layers.append((kc, vc, Wc, kbar, ks, q_new, k_new))
+    torch.cuda.synchronize()
+    stream = torch.cuda.current_stream()
+    out = torch.empty(batch, cfg.h_q, d, dtype=torch.bfloat16, device=dev)
+    n_model_layers = cfg.layers
+
+    def one_layer(l, ev=None):
+        kc, vc, Wc, kbar, ks, q_new, k_new = layers[l % n_layer_bufs]
+        if ev is not None: ev[0].record(stream)
+        dp.select(q_new, k_new, seqlens, kbar, ks, Wc)
+        if ev is not None: ev[1].record(stream)
+        dp.attend(q_new, kc, vc, seqlens, out)
+        if ev is not None: ev[2].record(stream)
+
+    def decode_step(evs=None):
+        dp.reset()
+        for l in range(n_model_layers):
+            one_layer(l, None if evs is None else evs[l])
+
+    for _ in range(3):
+        decode_step()
+    torch.cuda.synchronize()
+    evs = [[[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(n_model_layers)]
+           for _ in range(steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for k in range(steps):
+        decode_step(evs[k])
+    e1.record(stream)
+    torch.cuda.synchronize()
+    us_layer = e0.elapsed_time(e1) * 1e3 / (steps * n_model_layers)
+    sel_us = statistics.mean(e[0].elapsed_time(e[1]) * 1e3 for st in evs for e in st)
+    att_us = statistics.mean(e[1].elapsed_time(e[2]) * 1e3 for st in evs for e in st)
+    kv_bytes = batch * tau * B * cfg.h_kv * d * 2 * 2
+    gbs = kv_bytes / (att_us * 1e-6) / 1e9
+    return {"workload": cfg.name, "metric": "decode_us_per_step_per_layer_at_20pct_density",
+            "us_per_layer": us_layer, "selection_us": sel_us, "attention_us": att_us,
+            "selection_overhead_share": sel_us / (sel_us + att_us), "batch": batch, "kv_len": t, "tau": tau,
+            "splits": pkg.sw_decode_num_splits(batch, cfg.h_kv, tau), "layer_buffers_cycled": n_layer_bufs,
+            "roofline": {"kernel": "sw_sparse_attn_decode", "bound": "hbm", "achieved": gbs,
+                         "peak": peaks.get("hbm_gbs"), "unit": "GB/s", "frac": gbs / peaks.get("hbm_gbs"),
+                         "bytes_per_launch": kv_bytes, "traffic": _ncu_traffic("sw_sparse_attn_decode")}}

@@ -225,6 +225,20 @@ SW_API size_t sw_decode_workspace_bytes(int32_t batch, int32_t h_q, int32_t h_kv
 /* Number of KV splits sw_sparse_attn_decode will use (host-only; for reporting). */
 SW_API int32_t sw_decode_num_splits(int32_t batch, int32_t h_kv, int32_t tau_max);
 
+/* Kernel choice of sw_sparse_attn_prefill (process-wide; for tests and benchmarks -- both kernels
+ * are CUDA kernels of this library, there is no non-GPU path).
+ *   SW_PREFILL_AUTO (default): the tcgen05/TMEM/TMA kernel when the problem fits it (d = 128, bf16
+ *                    or cast fp32 operands, h_q = 4 h_kv), else the generic mma.sync kernel.
+ *   SW_PREFILL_GENERIC: always the generic kernel.
+ *   SW_PREFILL_TCGEN05: the tcgen05 kernel; sw_sparse_attn_prefill returns SW_ERR_UNSUPPORTED when
+ *                    the problem does not fit it.
+ * Returns the previous setting, or SW_ERR_INVALID_ARG for an unknown value (setting unchanged).
+ * sw_get_prefill_kernel_used(): which kernel the last sw_sparse_attn_prefill of this thread launched
+ * (SW_PREFILL_GENERIC / SW_PREFILL_TCGEN05; 0 = none yet). */
+enum sw_prefill_kernel { SW_PREFILL_AUTO = 0, SW_PREFILL_GENERIC = 1, SW_PREFILL_TCGEN05 = 2 };
+SW_API int32_t sw_set_prefill_kernel(int32_t which);
+SW_API int32_t sw_get_prefill_kernel_used(void);
+
 SW_API const char* sw_last_error(void);
 SW_API int32_t sw_version(void);
 

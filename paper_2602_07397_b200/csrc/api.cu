@@ -96,6 +96,9 @@ using namespace sw;
     if (_s != SW_OK) return _s;       \
   } while (0)
 
+static int32_t g_prefill_kernel = SW_PREFILL_AUTO;
+static thread_local int32_t g_prefill_used = 0;
+
 extern "C" {
 
 SW_API const char* sw_last_error(void) { return g_err; }
@@ -274,9 +277,25 @@ SW_API int32_t sw_sparse_attn_prefill(const sw_layout* L, const sw_tensor* q, co
     a.k_stride_tok = k->stride_tok; a.k_stride_head = k->stride_head;
     a.v_stride_tok = v->stride_tok; a.v_stride_head = v->stride_head;
   }
-  if (attn_prefill_sm100_supported(a)) return launch_attn_prefill_sm100(a, st);
+  const bool fits = attn_prefill_sm100_supported(a);
+  if (g_prefill_kernel == SW_PREFILL_TCGEN05 && !fits)
+    return fail(SW_ERR_UNSUPPORTED, "sw_sparse_attn_prefill: SW_PREFILL_TCGEN05 needs d = 128 and h_q = 4 h_kv");
+  if (fits && g_prefill_kernel != SW_PREFILL_GENERIC) {
+    g_prefill_used = SW_PREFILL_TCGEN05;
+    return launch_attn_prefill_sm100(a, st);
+  }
+  g_prefill_used = SW_PREFILL_GENERIC;
   return launch_attn_prefill_generic(a, st);
 }
+
+SW_API int32_t sw_set_prefill_kernel(int32_t which) {
+  SW_REQUIRE(which >= SW_PREFILL_AUTO && which <= SW_PREFILL_TCGEN05, SW_ERR_INVALID_ARG,
+             "sw_set_prefill_kernel: unknown value %d", which);
+  const int32_t prev = g_prefill_kernel;
+  g_prefill_kernel = which;
+  return prev;
+}
+SW_API int32_t sw_get_prefill_kernel_used(void) { return g_prefill_used; }
 
 SW_API int32_t sw_sparse_attn_decode(int32_t batch, int32_t block, const sw_tensor* q, const sw_tensor* kcache,
                               const sw_tensor* vcache, int64_t stride_batch, const int32_t* seqlens,

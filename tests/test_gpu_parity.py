@@ -211,7 +211,19 @@ def random_lists(rng, b, tau, causal=True):
     return O.select_topk(np.tril(R) if causal else R, tau, O.DEFAULT_FLAGS if causal else (O.DEFAULT_FLAGS & ~O.CAUSAL))
 
 
-def attn_case(sw, seqlens, h_q, h_kv, d, B, tau_frac, dtype, causal=True, seed=0, heads_checked=None):
+def attn_case(sw, seqlens, h_q, h_kv, d, B, tau_frac, dtype, causal=True, seed=0, heads_checked=None,
+              kernel=None):
+    kernel = sw.SW_PREFILL_AUTO if kernel is None else kernel
+    prev = sw.sw_set_prefill_kernel(kernel)
+    try:
+        _attn_case(sw, seqlens, h_q, h_kv, d, B, tau_frac, dtype, causal, seed, heads_checked)
+        if kernel != sw.SW_PREFILL_AUTO:
+            assert sw.sw_get_prefill_kernel_used() == kernel
+    finally:
+        sw.sw_set_prefill_kernel(prev)
+
+
+def _attn_case(sw, seqlens, h_q, h_kv, d, B, tau_frac, dtype, causal, seed, heads_checked):
     rng = np.random.RandomState(seed)
     torch.manual_seed(seed)
     T = sum(seqlens)
@@ -259,6 +271,37 @@ def attn_case(sw, seqlens, h_q, h_kv, d, B, tau_frac, dtype, causal=True, seed=0
 ])
 def test_sparse_attn_prefill(sw, case):
     attn_case(sw, **case)
+
+
+# the same problems through each kernel explicitly: shapes that fit the tcgen05 kernel (d = 128, GQA 4)
+TC_CASES = [
+    dict(seqlens=(1000,), h_q=8, h_kv=2, d=128, B=64, tau_frac=0.2, dtype=torch.bfloat16),     # ragged tail
+    dict(seqlens=(1100,), h_q=4, h_kv=1, d=128, B=128, tau_frac=0.4, dtype=torch.bfloat16),    # B = 128
+    dict(seqlens=(130, 64, 257, 1), h_q=8, h_kv=2, d=128, B=64, tau_frac=0.5, dtype=torch.bfloat16),  # varlen
+    dict(seqlens=(515,), h_q=8, h_kv=2, d=128, B=64, tau_frac=1.0, dtype=torch.bfloat16),      # 100 % density
+    dict(seqlens=(320,), h_q=4, h_kv=1, d=128, B=64, tau_frac=0.6, dtype=torch.bfloat16, causal=False),
+    dict(seqlens=(40,), h_q=4, h_kv=1, d=128, B=64, tau_frac=1.0, dtype=torch.bfloat16),       # one partial block
+    dict(seqlens=(700,), h_q=4, h_kv=1, d=128, B=64, tau_frac=0.1, dtype=torch.bfloat16),      # odd chunk counts
+    dict(seqlens=(600,), h_q=8, h_kv=2, d=128, B=64, tau_frac=0.3, dtype=torch.float32),       # P17 cast pre-pass
+    dict(seqlens=(4096 + 33,), h_q=8, h_kv=2, d=128, B=64, tau_frac=0.2, dtype=torch.bfloat16,
+         heads_checked=[0, 3, 6]),                                                             # long rows
+]
+
+
+@pytest.mark.parametrize("kernel", ["generic", "tcgen05"])
+@pytest.mark.parametrize("case", TC_CASES)
+def test_sparse_attn_prefill_each_kernel(sw, case, kernel):
+    attn_case(sw, kernel=sw.SW_PREFILL_TCGEN05 if kernel == "tcgen05" else sw.SW_PREFILL_GENERIC, **case)
+
+
+def test_prefill_tcgen05_rejects_unfit_shapes(sw):
+    prev = sw.sw_set_prefill_kernel(sw.SW_PREFILL_TCGEN05)
+    try:
+        with pytest.raises(sw.SwError) as e:
+            _attn_case(sw, (128,), 2, 2, 64, 64, 1.0, torch.bfloat16, True, 0, None)
+        assert e.value.code == sw.SW_ERR_UNSUPPORTED
+    finally:
+        sw.sw_set_prefill_kernel(prev)
 
 
 def test_sparse_attn_prefill_full_density_is_dense_causal(sw):

@@ -282,7 +282,7 @@ def decode_bench(pkg, args, peaks, n_layer_bufs: int = 4, steps: int = 20):
     return {"workload": cfg.name, "metric": "decode_us_per_step_per_layer_at_20pct_density",
             "us_per_layer": us_layer, "selection_us": sel_us, "attention_us": att_us,
             "selection_overhead_share": sel_us / (sel_us + att_us), "batch": batch, "kv_len": t, "tau": tau,
-            "splits": pkg.sw_decode_num_splits(batch, cfg.h_kv, tau), "layer_buffers_cycled": n_layer_bufs,
+            "splits": pkg.sw_decode_num_splits(batch, cfg.h_kv, d, tau), "layer_buffers_cycled": n_layer_bufs,
             "roofline": {"kernel": "sw_sparse_attn_decode", "bound": "hbm", "achieved": gbs,
                          "peak": peaks.get("hbm_gbs"), "unit": "GB/s", "frac": gbs / peaks.get("hbm_gbs"),
                          "bytes_per_launch": kv_bytes, "traffic": _ncu_traffic("sw_sparse_attn_decode")}}

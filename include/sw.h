@@ -223,7 +223,7 @@ SW_API size_t sw_workspace_bytes(int32_t op, const sw_layout* L, int32_t h_q, in
 SW_API size_t sw_decode_workspace_bytes(int32_t batch, int32_t h_q, int32_t h_kv, int32_t d, int32_t tau_max);
 
 /* Number of KV splits sw_sparse_attn_decode will use (host-only; for reporting). */
-SW_API int32_t sw_decode_num_splits(int32_t batch, int32_t h_kv, int32_t tau_max);
+SW_API int32_t sw_decode_num_splits(int32_t batch, int32_t h_kv, int32_t d, int32_t tau_max);
 
 /* Kernel choice of sw_sparse_attn_prefill (process-wide; for tests and benchmarks -- both kernels
  * are CUDA kernels of this library, there is no non-GPU path).

@@ -71,7 +71,7 @@ def _load() -> C.CDLL:
         "sw_sparse_attn_decode": (i32, [i32, i32, TP, TP, TP, i64, vp, vp, vp, i32, f32, vp, vp, vp, sz, vp]),
         "sw_workspace_bytes": (sz, [i32, LP, i32, i32, i32, i32, i32]),
         "sw_decode_workspace_bytes": (sz, [i32, i32, i32, i32, i32]),
-        "sw_decode_num_splits": (i32, [i32, i32, i32]),
+        "sw_decode_num_splits": (i32, [i32, i32, i32, i32]),
         "sw_set_prefill_kernel": (i32, [i32]),
         "sw_get_prefill_kernel_used": (i32, []),
         "sw_last_error": (C.c_char_p, []),
@@ -228,8 +228,8 @@ def sw_decode_workspace_bytes(batch, h_q, h_kv, d, tau_max) -> int:
     return _lib.sw_decode_workspace_bytes(batch, h_q, h_kv, d, tau_max)
 
 
-def sw_decode_num_splits(batch, h_kv, tau_max) -> int:
-    return _lib.sw_decode_num_splits(batch, h_kv, tau_max)
+def sw_decode_num_splits(batch, h_kv, d, tau_max) -> int:
+    return _lib.sw_decode_num_splits(batch, h_kv, d, tau_max)
 
 
 def sw_sparse_attn_prefill(L: Layout, q, k, v, idx, count, tau_max, softmax_scale, flags, out, lse=None,

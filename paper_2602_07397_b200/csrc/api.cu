@@ -219,14 +219,14 @@ SW_API size_t sw_workspace_bytes(int32_t op, const sw_layout* L, int32_t h_q, in
   }
 }
 
-SW_API int32_t sw_decode_num_splits(int32_t batch, int32_t h_kv, int32_t tau_max) {
+SW_API int32_t sw_decode_num_splits(int32_t batch, int32_t h_kv, int32_t d, int32_t tau_max) {
   check_arch();
-  return decode_num_splits(batch, h_kv, tau_max);
+  return decode_num_splits(batch, h_kv, tau_max, d);
 }
 
 SW_API size_t sw_decode_workspace_bytes(int32_t batch, int32_t h_q, int32_t h_kv, int32_t d, int32_t tau_max) {
   check_arch();
-  return decode_ws_bytes(batch, h_q, d, decode_num_splits(batch, h_kv, tau_max));
+  return decode_ws_bytes(batch, h_q, d, decode_num_splits(batch, h_kv, tau_max, d));
 }
 
 SW_API int32_t sw_sparse_attn_prefill(const sw_layout* L, const sw_tensor* q, const sw_tensor* k, const sw_tensor* v,

@@ -257,16 +257,28 @@ attn_decode_merge_kernel(const float* __restrict__ Opart, const float* __restric
 
 namespace sw {
 
-int decode_num_splits(int batch, int h_kv, int tau_max) {
-  // aim for ~4 CTAs per SM so that every SM keeps several cp.async rings in flight
+int decode_num_splits(int batch, int h_kv, int tau_max, int d) {
+  // Split-KV factor.  The grid (batch * h_kv * ns CTAs) runs in waves of slots = (CTAs resident per
+  // SM) * (SMs); a wave that is mostly empty costs as much as a full one, so pick the ns that
+  // minimises  waves * ceil(tau_max / ns)  (time in key blocks per CTA slot), with a 1 % penalty per
+  // split for the merge pass.
   const int base = batch * h_kv;
   if (base <= 0 || tau_max <= 0) return 1;
-  int target = 4 * num_sms();
-  int ns = (target + base - 1) / base;
-  if (ns < 1) ns = 1;
-  if (ns > tau_max) ns = tau_max;
-  if (ns > 64) ns = 64;
-  return ns;
+  const int ring = kStages * 2 * KT * d * 2;                   // bytes of shared memory per CTA
+  int occ = (227 * 1024) / (ring + 1024);
+  if (occ < 1) occ = 1;
+  if (occ > 8) occ = 8;
+  const int slots = occ * num_sms();
+  const int ns_max = tau_max < 64 ? tau_max : 64;
+  int best = 1;
+  double best_cost = 1e30;
+  for (int ns = 1; ns <= ns_max; ++ns) {
+    const int waves = (base * ns + slots - 1) / slots;
+    const int blocks = (tau_max + ns - 1) / ns;
+    const double cost = (double)waves * (blocks + 1) * (1.0 + 0.01 * ns);
+    if (cost < best_cost) { best_cost = cost; best = ns; }
+  }
+  return best;
 }
 
 size_t decode_ws_bytes(int batch, int h_q, int d, int nsplit) {
@@ -303,7 +315,7 @@ int32_t launch_attn_decode(int batch, int block, const sw_tensor& q, const sw_te
                            const int32_t* idx, const int32_t* count, int tau_max, float softmax_scale,
                            void* out, float* lse, void* ws, size_t ws_bytes, cudaStream_t st) {
   if (batch == 0) return SW_OK;
-  const int nsplit = decode_num_splits(batch, kc.heads, tau_max);
+  const int nsplit = decode_num_splits(batch, kc.heads, tau_max, q.d);
   if (ws == nullptr || ws_bytes < decode_ws_bytes(batch, q.heads, q.d, nsplit))
     return fail(SW_ERR_WORKSPACE, "sw_sparse_attn_decode: workspace %zu < %zu bytes", ws_bytes,
                 decode_ws_bytes(batch, q.heads, q.d, nsplit));

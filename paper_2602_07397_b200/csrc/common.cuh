@@ -71,7 +71,7 @@ int32_t launch_attn_prefill_sm100(const AttnPrefillArgs& a, cudaStream_t st);
 int32_t launch_cast_f32_to_bf16(const float* src, __nv_bfloat16* dst, int64_t tokens, int heads, int d,
                                 int64_t stride_tok, int64_t stride_head, cudaStream_t st);
 
-int decode_num_splits(int batch, int h_kv, int tau_max);
+int decode_num_splits(int batch, int h_kv, int tau_max, int d);
 size_t decode_ws_bytes(int batch, int h_q, int d, int nsplit);
 int32_t launch_attn_decode(int batch, int block, const sw_tensor& q, const sw_tensor& kc,
                            const sw_tensor& vc, int64_t stride_batch, const int32_t* seqlens,

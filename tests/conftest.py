@@ -8,7 +8,16 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 
+def _ensure_libsw():
+    """Compile libsw.so in-tree when it is absent (fresh checkout): building is not a fallback."""
+    lib = os.path.join(ROOT, "paper_2602_07397_b200", "libsw.so")
+    if not os.path.exists(lib):
+        import __graft_entry__
+        __graft_entry__.build()
+
+
 def pytest_configure(config):
+    _ensure_libsw()
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu")
 
 

@@ -4,17 +4,22 @@
 //
 // Work unit (one CTA): a 64-token query tile of one KV-head group (4 q-heads) = 256 query rows, row =
 // 4*token + head, processed as two 128-row MMA tiles t = 0, 1.  The selected key blocks of the query
-// block are cut into 64-key chunks and consumed two at a time (a 128-key tile):
-//     S_t = Q_t K^T      tcgen05.mma  M=128 N=128 K=16 x8   A, B from shared memory (K-major, SW128)
-//     P_t = exp2(S_t*c - m)  fp32 online softmax in registers, one thread per row, P written back to
-//                            TMEM as bf16 over the S columns
-//     O_t += P_t V       tcgen05.mma  M=128 N=128 K=16 x8   A from TMEM, B from shared memory (MN-major)
-// TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512).
+// block are cut into 64-key chunks k = 0..n-1; per tile and chunk:
+//     S_t(k) = Q_t K(k)^T     tcgen05.mma  M=128 N=64  K=16 x8   A, B from shared memory (K-major, SW128)
+//     P_t(k) = exp2(S*c - m)  fp32 online softmax in registers, one thread per row, P written back to
+//                             TMEM as bf16 over the first half of the S columns
+//     O_t   += P_t(k) V(k)    tcgen05.mma  M=128 N=128 K=16 x4   A from TMEM, B from shared memory (MN-major)
+// TMEM (512 columns): S_t[buf] at t*128 + buf*64 (two S buffers per tile), O_t at 256 + t*128.
+// The S buffers decouple the tensor pipe from the softmax warps: QK(k+1) is issued before the softmax
+// of chunk k finishes, so a softmax warp never waits for its next S while the tensor pipe works on
+// PV(k) / QK(k+2), and the two tiles' softmax warps (one of each per SM sub-partition) run
+// concurrently, interleaving their MUFU and FMA work.
 // Warps: 0 = TMA producer, 1 = MMA issuer, 2 = TMEM allocator, 3 = chunk-list builder,
 //        4-7 = softmax/epilogue of tile 0, 8-11 = softmax/epilogue of tile 1.
-// The MMA order  PV0(j) QK0(j+1) PV1(j) QK1(j+1)  lets the softmax of one tile overlap the tensor work
-// of the other.  The O rescale is lazy: the running max is only raised (and O multiplied) when it grew
-// by more than 2^8, which keeps P within bf16/fp32 range and is exact after the final 1/l.
+// MMA issue order per chunk k:  PV0(k) QK0(k+2) PV1(k) QK1(k+2).
+// The O rescale is lazy: the running max is only raised (and O multiplied) when it grew by more than
+// 2^8, which keeps P within bf16/fp32 range and is exact after the final 1/l; a rescale first waits
+// for PV(k-1) of its tile (o_ready barrier).
 #include "common.cuh"
 #include "sm100.cuh"
 
@@ -23,12 +28,22 @@ namespace {
 using namespace sm100;
 
 constexpr int kThreads = 384;
-constexpr int kStages = 4;                    // ring of 128-key K or V tiles
-constexpr int kTileBytes = 128 * 128 * 2;     // 32 KB: [d-half][128 keys][128 B]
+constexpr int kStages = 8;                    // ring of 64-key K or V tiles
+constexpr int kTileBytes = 64 * 128 * 2;      // 16 KB: [d-half][64 keys][128 B]
 constexpr int kQBytes = 256 * 128 * 2;        // 64 KB: [d-half][256 rows][128 B]
 constexpr int kMaxChunks = 4096;              // 64-key chunks per query row the list buffer holds
-constexpr int kSmemBytes = kQBytes + kStages * kTileBytes + kMaxChunks * 4 + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int kSmemBytes = kQBytes + kStages * kTileBytes + kMaxChunks * 4 + 1024 /*align*/ + 512 /*barriers*/;
 constexpr float kRescaleThreshold = 8.0f;     // log2 units
+
+// barrier map
+constexpr int kBarQ = 0;                      // Q tile landed
+constexpr int kBarFull = 1;                   // [kStages] K/V tile landed
+constexpr int kBarEmpty = kBarFull + kStages; // [kStages] K/V tile consumed
+constexpr int kBarS = kBarEmpty + kStages;    // [t][buf] S ready          (tcgen05.commit)
+constexpr int kBarP = kBarS + 4;              // [t][buf] P written         (4 warps arrive)
+constexpr int kBarO = kBarP + 4;              // [t] PV(k) done             (tcgen05.commit)
+constexpr int kBarDone = kBarO + 2;           // all MMAs done
+constexpr int kNumBars = kBarDone + 1;
 
 struct Params {
   const int32_t* cu_seqlens;
@@ -72,11 +87,10 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   const uint32_t sKV = sQ + kQBytes;
   int32_t* s_list = reinterpret_cast<int32_t*>(base + kQBytes + kStages * kTileBytes);
   uint64_t* bars = reinterpret_cast<uint64_t*>(base + kQBytes + kStages * kTileBytes + kMaxChunks * 4);
-  // barrier map: 0 q_full | 1..4 full[stage] | 5..8 empty[stage] | 9,10 s_full[t] | 11,12 p_full[t] | 13 o_full
   const uint32_t bar0 = smem_u32(bars);
   auto BAR = [&](int i) { return bar0 + 8u * i; };
-  volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(bars + 16);
-  volatile int32_t* s_nchunks = reinterpret_cast<volatile int32_t*>(bars + 17);
+  volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(bars + kNumBars);
+  volatile int32_t* s_nchunks = reinterpret_cast<volatile int32_t*>(bars + kNumBars + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -96,11 +110,11 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   // ---- one-time setup ------------------------------------------------------------------------
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&map_q); prefetch_tmap(&map_k); prefetch_tmap(&map_v);
-    mbar_init(BAR(0), 1);
-    for (int s = 0; s < kStages; ++s) { mbar_init(BAR(1 + s), 1); mbar_init(BAR(5 + s), 1); }
-    mbar_init(BAR(9), 1); mbar_init(BAR(10), 1);
-    mbar_init(BAR(11), 4); mbar_init(BAR(12), 4);
-    mbar_init(BAR(13), 1);
+    mbar_init(BAR(kBarQ), 1);
+    for (int s = 0; s < kStages; ++s) { mbar_init(BAR(kBarFull + s), 1); mbar_init(BAR(kBarEmpty + s), 1); }
+    for (int i = 0; i < 4; ++i) { mbar_init(BAR(kBarS + i), 1); mbar_init(BAR(kBarP + i), 4); }
+    mbar_init(BAR(kBarO), 1); mbar_init(BAR(kBarO + 1), 1);
+    mbar_init(BAR(kBarDone), 1);
     fence_barrier_init();
   } else if (warp == 2) {
     tmem_alloc<512>(smem_u32((const void*)s_tmem));
@@ -132,94 +146,114 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tm = *s_tmem;
-  const int n_chunks = *s_nchunks;
-  const int n_iter = (n_chunks + 1) >> 1;
+  // warp-uniform copies (shfl from lane 0) so that the compiler keeps descriptors and TMA / MMA
+  // operands in uniform registers instead of broadcasting them per instruction
+  const uint32_t tm = __shfl_sync(0xffffffffu, *s_tmem, 0);
+  const int n = __shfl_sync(0xffffffffu, *s_nchunks, 0);
 
   if (warp < 4) {
-  reg_dealloc<64>();                                          // 128*64 + 256*216 <= 64 K registers
+  reg_dealloc<64>();
   if (warp == 0) {
     // ===================== TMA producer =====================
-    if (lane == 0 && n_iter > 0) {
-      mbar_arrive_expect_tx(BAR(0), kQBytes);
-      tma_load_3d(sQ, &map_q, BAR(0), 0, kvh * 4, q_tok0);
-      tma_load_3d(sQ + kQBytes / 2, &map_q, BAR(0), 64, kvh * 4, q_tok0);
-      for (int it = 0; it < n_iter; ++it) {
-        const int nblk = min(2, n_chunks - 2 * it);
-#pragma unroll
-        for (int kv = 0; kv < 2; ++kv) {
-          const int qn = 2 * it + kv;
-          const int st = qn % kStages;
-          mbar_wait(BAR(5 + st), ((qn / kStages) & 1) ^ 1);
-          mbar_arrive_expect_tx(BAR(1 + st), nblk * (kTileBytes / 2));
-          const CUtensorMap* m = kv ? &map_v : &map_k;
+    // tile order = consumption order of the MMA warp: K0 K1 V0 K2 V1 K3 ... V(n-1)
+    // (the whole warp runs the loop; one elected lane issues the copies)
+    if (n > 0) {
+      const bool leader = elect_one();
+      if (leader) {
+        mbar_arrive_expect_tx(BAR(kBarQ), kQBytes);
+        tma_load_3d(sQ, &map_q, BAR(kBarQ), 0, kvh * 4, q_tok0);
+        tma_load_3d(sQ + kQBytes / 2, &map_q, BAR(kBarQ), 64, kvh * 4, q_tok0);
+      }
+      int c = 0;
+      auto push = [&](const CUtensorMap* m, int chunk) {
+        const int st = c % kStages;
+        mbar_wait(BAR(kBarEmpty + st), ((c / kStages) & 1) ^ 1);
+        const int k0 = __shfl_sync(0xffffffffu, s_list[chunk], 0);
+        if (leader) {
+          mbar_arrive_expect_tx(BAR(kBarFull + st), kTileBytes);
           const uint32_t dst = sKV + st * kTileBytes;
-          for (int h = 0; h < nblk; ++h) {
-            const int k0 = s_list[2 * it + h];
-            tma_load_3d(dst + h * 8192, m, BAR(1 + st), 0, kvh, k0);
-            tma_load_3d(dst + 16384 + h * 8192, m, BAR(1 + st), 64, kvh, k0);
-          }
+          tma_load_3d(dst, m, BAR(kBarFull + st), 0, kvh, k0);
+          tma_load_3d(dst + kTileBytes / 2, m, BAR(kBarFull + st), 64, kvh, k0);
         }
+        __syncwarp();
+        ++c;
+      };
+      push(&map_k, 0);
+      if (n > 1) push(&map_k, 1);
+      for (int k = 0; k < n; ++k) {
+        push(&map_v, k);
+        if (k + 2 < n) push(&map_k, k + 2);
       }
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
-    if (lane == 0 && n_iter > 0) {
-      const uint32_t id_full = idesc_bf16(128, 128, 0, 0), id_half = idesc_bf16(128, 64, 0, 0);
+    // warp-uniform control flow; one elected lane issues tcgen05.mma / tcgen05.commit
+    if (n > 0) {
+      const bool leader = elect_one();
+      const uint32_t id_qk = idesc_bf16(128, 64, 0, 0);
       const uint32_t id_pv = idesc_bf16(128, 128, 0, 1);
-      auto issue_qk = [&](int t, uint32_t sK, int nblk) {
-        const uint32_t id = nblk == 2 ? id_full : id_half;
+      int c = 0;
+      auto next_tile = [&](int& stage) -> uint32_t {       // waits for the next tile of the ring
+        stage = c % kStages;
+        mbar_wait(BAR(kBarFull + stage), (c / kStages) & 1);
+        tc_fence_after();
+        ++c;
+        return sKV + stage * kTileBytes;
+      };
+      auto issue_qk = [&](int t, int buf, uint32_t sK, int release_stage) {
+        if (leader) {
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk) {
-          const uint32_t a = sQ + (kk >> 2) * (kQBytes / 2) + t * 16384 + (kk & 3) * 32;
-          const uint32_t b = sK + (kk >> 2) * 16384 + (kk & 3) * 32;
-          mma_ss(tm + t * 128, desc_kmajor_sw128(a), desc_kmajor_sw128(b), id, kk > 0);
+          for (int kk = 0; kk < 8; ++kk) {
+            const uint32_t a = sQ + (kk >> 2) * (kQBytes / 2) + t * 16384 + (kk & 3) * 32;
+            const uint32_t b = sK + (kk >> 2) * (kTileBytes / 2) + (kk & 3) * 32;
+            mma_ss(tm + t * 128 + buf * 64, desc_kmajor_sw128(a), desc_kmajor_sw128(b), id_qk, kk > 0);
+          }
+          mma_commit(BAR(kBarS + t * 2 + buf));
+          if (release_stage >= 0) mma_commit(BAR(kBarEmpty + release_stage));
         }
-        mma_commit(BAR(9 + t));
+        __syncwarp();
       };
-      auto issue_pv = [&](int t, uint32_t sV, int nblk, bool acc) {
-        for (int kk = 0; kk < 4 * nblk; ++kk)
-          mma_ts(tm + 256 + t * 128, tm + t * 128 + kk * 8, desc_mnmajor_sw128(sV + kk * 2048, 16384, 1024), id_pv,
-                 (acc || kk > 0) ? 1u : 0u);
+      auto issue_pv = [&](int t, int buf, uint32_t sV, bool acc, int release_stage) {
+        if (leader) {
+#pragma unroll
+          for (int kk = 0; kk < 4; ++kk)
+            mma_ts(tm + 256 + t * 128, tm + t * 128 + buf * 64 + kk * 8,
+                   desc_mnmajor_sw128(sV + kk * 2048, kTileBytes / 2, 1024), id_pv, (acc || kk > 0) ? 1u : 0u);
+          mma_commit(BAR(kBarO + t));
+          if (release_stage >= 0) mma_commit(BAR(kBarEmpty + release_stage));
+        }
+        __syncwarp();
       };
-      mbar_wait(BAR(0), 0);
-      mbar_wait(BAR(1 + 0), 0);
-      tc_fence_after();
-      {
-        const int nblk = min(2, n_chunks);
-        issue_qk(0, sKV, nblk);
-        issue_qk(1, sKV, nblk);
-        mma_commit(BAR(5 + 0));
+      mbar_wait(BAR(kBarQ), 0);
+      for (int k = 0; k < 2 && k < n; ++k) {
+        int st;
+        const uint32_t sK = next_tile(st);
+        issue_qk(0, k, sK, -1);
+        issue_qk(1, k, sK, st);
       }
-      for (int j = 0; j < n_iter; ++j) {
-        const int nblk = min(2, n_chunks - 2 * j);
-        const int qv = 2 * j + 1, sv = qv % kStages;
-        const int qk = 2 * j + 2, sk = qk % kStages;
-        const bool more = (j + 1 < n_iter);
-        const int nblk_next = more ? min(2, n_chunks - 2 * (j + 1)) : 0;
-        mbar_wait(BAR(1 + sv), (qv / kStages) & 1);
-        mbar_wait(BAR(11), j & 1);
-        tc_fence_after();
-        issue_pv(0, sKV + sv * kTileBytes, nblk, j > 0);
+      for (int k = 0; k < n; ++k) {
+        const int buf = k & 1, ph = (k >> 1) & 1;
+        const bool more = k + 2 < n;
+        int sv, sk = 0;
+        uint32_t sK = 0;
+        mbar_wait(BAR(kBarP + buf), ph);
+        const uint32_t sV = next_tile(sv);
+        issue_pv(0, buf, sV, k > 0, -1);
         if (more) {
-          mbar_wait(BAR(1 + sk), (qk / kStages) & 1);
-          tc_fence_after();
-          issue_qk(0, sKV + sk * kTileBytes, nblk_next);
+          sK = next_tile(sk);
+          issue_qk(0, buf, sK, -1);
         }
-        mbar_wait(BAR(12), j & 1);
+        mbar_wait(BAR(kBarP + 2 + buf), ph);
         tc_fence_after();
-        issue_pv(1, sKV + sv * kTileBytes, nblk, j > 0);
-        mma_commit(BAR(5 + sv));
-        if (more) {
-          issue_qk(1, sKV + sk * kTileBytes, nblk_next);
-          mma_commit(BAR(5 + sk));
-        }
+        issue_pv(1, buf, sV, k > 0, sv);
+        if (more) issue_qk(1, buf, sK, sk);
       }
-      mma_commit(BAR(13));
+      if (leader) mma_commit(BAR(kBarDone));
+      __syncwarp();
     }
   }
   } else {
-    reg_alloc<216>();
+    reg_alloc<200>();
     // ===================== softmax + epilogue: one thread per query row =====================
     const int t = (warp - 4) >> 2;                       // MMA tile
     const int w4 = warp & 3;                             // TMEM lane quadrant of this warp
@@ -230,51 +264,45 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     const uint32_t t_o = tm + ((uint32_t)(w4 * 32) << 16) + 256 + t * 128;
     float m_run = -INFINITY, l_run = 0.f;
     const float c = p.scale_log2;
+    const float2 c2 = make_float2(c, c);
 
-    for (int j = 0; j < n_iter; ++j) {
-      const int nblk = min(2, n_chunks - 2 * j);
-      mbar_wait(BAR(9 + t), j & 1);
+    for (int k = 0; k < n; ++k) {
+      const int buf = k & 1, ph = (k >> 1) & 1;
+      mbar_wait(BAR(kBarS + t * 2 + buf), ph);
       tc_fence_after();
-      uint32_t s[128];
-      tmem_ld32(t_s + 0, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
-      tmem_ld32(t_s + 32, *reinterpret_cast<uint32_t(*)[32]>(&s[32]));
-      if (nblk == 2) {
-        tmem_ld32(t_s + 64, *reinterpret_cast<uint32_t(*)[32]>(&s[64]));
-        tmem_ld32(t_s + 96, *reinterpret_cast<uint32_t(*)[32]>(&s[96]));
-      }
+      uint32_t s[64];
+      tmem_ld32(t_s + buf * 64, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
+      tmem_ld32(t_s + buf * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&s[32]));
       tmem_wait_ld();
-      if (nblk < 2) {
-#pragma unroll
-        for (int i = 64; i < 128; ++i) s[i] = 0xff800000u;   // -inf
-      }
       // masks: only chunks that touch the diagonal or the end of the sequence
+      {
+        const int k0 = s_list[k];
+        const bool need = (p.causal && k0 + 63 > q_tok0) || (k0 + 64 > seq_hi);
+        if (need) {
+          const int lim = min(p.causal ? q_pos : 0x7fffffff, seq_hi - 1) - k0;   // visible iff col <= lim
 #pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        if (h < nblk) {
-          const int k0 = s_list[2 * j + h];
-          const bool need = (p.causal && k0 + 63 > q_tok0) || (k0 + 64 > seq_hi);
-          if (need) {
-            const int lim = min(p.causal ? q_pos : 0x7fffffff, seq_hi - 1) - k0;   // visible iff col <= lim
-#pragma unroll
-            for (int i = 0; i < 64; ++i)
-              if (i > lim) s[h * 64 + i] = 0xff800000u;
-          }
+          for (int i = 0; i < 64; ++i)
+            if (i > lim) s[i] = 0xff800000u;
         }
       }
-      float mx0 = -INFINITY, mx1 = -INFINITY;
+      float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
 #pragma unroll
-      for (int i = 0; i < 128; i += 4) {
+      for (int i = 0; i < 64; i += 8) {
         mx0 = fmax3(mx0, __uint_as_float(s[i]), __uint_as_float(s[i + 1]));
         mx1 = fmax3(mx1, __uint_as_float(s[i + 2]), __uint_as_float(s[i + 3]));
+        mx2 = fmax3(mx2, __uint_as_float(s[i + 4]), __uint_as_float(s[i + 5]));
+        mx3 = fmax3(mx3, __uint_as_float(s[i + 6]), __uint_as_float(s[i + 7]));
       }
-      const float m_tile = fmaxf(mx0, mx1) * c;           // c > 0
+      const float m_tile = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c;      // c > 0
       // lazy rescale
       float m_new = m_run;
       const bool grow = m_tile > m_run + kRescaleThreshold;   // also true for the first finite tile
       if (grow) m_new = m_tile;
-      if (j > 0 && __any_sync(0xffffffffu, grow)) {
+      if (k > 0 && __any_sync(0xffffffffu, grow)) {
         const float f = (m_new == m_run) ? 1.f : ex2(m_run - m_new);   // m_run = -inf -> 0
         l_run *= f;
+        mbar_wait(BAR(kBarO + t), (k - 1) & 1);           // PV(k-1) of this tile has landed in O
+        tc_fence_after();
 #pragma unroll
         for (int ch = 0; ch < 4; ++ch) {
           uint32_t o[32];
@@ -287,29 +315,34 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
       }
       m_run = m_new;
       const float m_use = (m_run == -INFINITY) ? 0.f : m_run;
-      float sum0 = 0.f, sum1 = 0.f;
-      uint32_t pk[64];
+      const float2 nm2 = make_float2(-m_use, -m_use);
+      float2 sum0 = make_float2(0.f, 0.f), sum1 = make_float2(0.f, 0.f);
+      uint32_t pk[32];
 #pragma unroll
-      for (int i = 0; i < 64; ++i) {
-        const float a = ex2(fmaf(__uint_as_float(s[2 * i]), c, -m_use));
-        const float b = ex2(fmaf(__uint_as_float(s[2 * i + 1]), c, -m_use));
-        sum0 += a; sum1 += b;
-        pk[i] = pack_bf16(a, b);
+      for (int i = 0; i < 32; i += 2) {
+        const float2 x0 = __ffma2_rn(make_float2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), c2, nm2);
+        const float2 x1 = __ffma2_rn(make_float2(__uint_as_float(s[2 * i + 2]), __uint_as_float(s[2 * i + 3])), c2, nm2);
+        const float2 e0 = make_float2(ex2(x0.x), ex2(x0.y));
+        const float2 e1 = make_float2(ex2(x1.x), ex2(x1.y));
+        sum0 = __fadd2_rn(sum0, e0);
+        sum1 = __fadd2_rn(sum1, e1);
+        pk[i] = pack_bf16(e0.x, e0.y);
+        pk[i + 1] = pack_bf16(e1.x, e1.y);
       }
-      l_run += sum0 + sum1;
-      tmem_st32(t_s + 0, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
-      if (nblk == 2) tmem_st32(t_s + 32, *reinterpret_cast<uint32_t(*)[32]>(&pk[32]));
+      l_run += (sum0.x + sum0.y) + (sum1.x + sum1.y);
+      tmem_st32(t_s + buf * 64, pk);
       tmem_wait_st();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(BAR(11 + t));
+      if (lane == 0) mbar_arrive(BAR(kBarP + t * 2 + buf));
     }
 
     // epilogue: O / l -> bf16 -> global
-    if (n_iter > 0) {
-      mbar_wait(BAR(13), 0);
+    if (n > 0) {
+      mbar_wait(BAR(kBarDone), 0);
       tc_fence_after();
     }
+    const int n_iter = n;
     const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
     const bool valid = q_pos <= q_last;
     const int64_t o_off = ((int64_t)q_pos * p.h_q + head) * 128;

@@ -14,9 +14,9 @@
 // of chunk k finishes, so a softmax warp never waits for its next S while the tensor pipe works on
 // PV(k) / QK(k+2), and the two tiles' softmax warps (one of each per SM sub-partition) run
 // concurrently, interleaving their MUFU and FMA work.
-// Warps: 0 = TMA producer, 1 = MMA issuer, 2 = TMEM allocator, 3 = chunk-list builder,
-//        4-7 = softmax/epilogue of tile 0, 8-11 = softmax/epilogue of tile 1.
-// MMA issue order per chunk k:  PV0(k) QK0(k+2) PV1(k) QK1(k+2).
+// Warps: 0 = TMA producer, 1 = MMA issuer of tile 0, 2 = TMEM allocator, 3 = chunk-list builder, then
+//        MMA issuer of tile 1, 4-7 = softmax/epilogue of tile 0, 8-11 = softmax/epilogue of tile 1.
+// MMA issue order per tile and chunk k:  PV(k) QK(k+2); the two tiles' streams interleave on the pipe.
 // The O rescale is lazy: the running max is only raised (and O multiplied) when it grew by more than
 // 2^8, which keeps P within bf16/fp32 range and is exact after the final 1/l; a rescale first waits
 // for PV(k-1) of its tile (o_ready barrier).
@@ -44,6 +44,13 @@ constexpr int kBarP = kBarS + 4;              // [t][buf] P written         (4 w
 constexpr int kBarO = kBarP + 4;              // [t] PV(k) done             (tcgen05.commit)
 constexpr int kBarDone = kBarO + 2;           // all MMAs done
 constexpr int kNumBars = kBarDone + 1;
+
+#ifdef SW_TRACE
+__device__ long long g_trace[8][4096];          // [stream][event]
+#define TRACE(stream, slot) do { if (blockIdx.x == gridDim.x / 2 && blockIdx.y == 0 && lane == 0 && (slot) < 4096) g_trace[stream][slot] = clock64(); } while (0)
+#else
+#define TRACE(stream, slot) do {} while (0)
+#endif
 
 struct Params {
   const int32_t* cu_seqlens;
@@ -111,10 +118,10 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&map_q); prefetch_tmap(&map_k); prefetch_tmap(&map_v);
     mbar_init(BAR(kBarQ), 1);
-    for (int s = 0; s < kStages; ++s) { mbar_init(BAR(kBarFull + s), 1); mbar_init(BAR(kBarEmpty + s), 1); }
+    for (int s = 0; s < kStages; ++s) { mbar_init(BAR(kBarFull + s), 1); mbar_init(BAR(kBarEmpty + s), 2); }
     for (int i = 0; i < 4; ++i) { mbar_init(BAR(kBarS + i), 1); mbar_init(BAR(kBarP + i), 4); }
     mbar_init(BAR(kBarO), 1); mbar_init(BAR(kBarO + 1), 1);
-    mbar_init(BAR(kBarDone), 1);
+    mbar_init(BAR(kBarDone), 2);
     fence_barrier_init();
   } else if (warp == 2) {
     tmem_alloc<512>(smem_u32((const void*)s_tmem));
@@ -185,42 +192,46 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
         if (k + 2 < n) push(&map_k, k + 2);
       }
     }
-  } else if (warp == 1) {
-    // ===================== MMA issuer =====================
-    // warp-uniform control flow; one elected lane issues tcgen05.mma / tcgen05.commit
+  } else if (warp == 1 || warp == 3) {
+    // ===================== MMA issuers: warp 1 -> tile 0, warp 3 -> tile 1 =====================
+    // One issuing warp per tile: the barrier waits of one tile overlap the tensor work of the other
+    // (tcgen05.mma issue blocks while the pipe's short queue is full, so a single issuing warp exposes
+    // every wait).  Warp-uniform control flow; one elected lane issues tcgen05.mma / tcgen05.commit.
     if (n > 0) {
+      const int t = warp >> 1;
       const bool leader = elect_one();
       const uint32_t id_qk = idesc_bf16(128, 64, 0, 0);
       const uint32_t id_pv = idesc_bf16(128, 128, 0, 1);
+      const uint32_t t_sp = tm + t * 128, t_acc = tm + 256 + t * 128;
+      const uint32_t sQt = sQ + t * 16384;
       int c = 0;
       auto next_tile = [&](int& stage) -> uint32_t {       // waits for the next tile of the ring
         stage = c % kStages;
         mbar_wait(BAR(kBarFull + stage), (c / kStages) & 1);
-        tc_fence_after();
         ++c;
         return sKV + stage * kTileBytes;
       };
-      auto issue_qk = [&](int t, int buf, uint32_t sK, int release_stage) {
+      auto issue_qk = [&](int buf, uint32_t sK, int stage) {
         if (leader) {
 #pragma unroll
           for (int kk = 0; kk < 8; ++kk) {
-            const uint32_t a = sQ + (kk >> 2) * (kQBytes / 2) + t * 16384 + (kk & 3) * 32;
+            const uint32_t a = sQt + (kk >> 2) * (kQBytes / 2) + (kk & 3) * 32;
             const uint32_t b = sK + (kk >> 2) * (kTileBytes / 2) + (kk & 3) * 32;
-            mma_ss(tm + t * 128 + buf * 64, desc_kmajor_sw128(a), desc_kmajor_sw128(b), id_qk, kk > 0);
+            mma_ss(t_sp + buf * 64, desc_kmajor_sw128(a), desc_kmajor_sw128(b), id_qk, kk > 0);
           }
           mma_commit(BAR(kBarS + t * 2 + buf));
-          if (release_stage >= 0) mma_commit(BAR(kBarEmpty + release_stage));
+          mma_commit(BAR(kBarEmpty + stage));
         }
         __syncwarp();
       };
-      auto issue_pv = [&](int t, int buf, uint32_t sV, bool acc, int release_stage) {
+      auto issue_pv = [&](int buf, uint32_t sV, bool acc, int stage) {
         if (leader) {
 #pragma unroll
           for (int kk = 0; kk < 4; ++kk)
-            mma_ts(tm + 256 + t * 128, tm + t * 128 + buf * 64 + kk * 8,
-                   desc_mnmajor_sw128(sV + kk * 2048, kTileBytes / 2, 1024), id_pv, (acc || kk > 0) ? 1u : 0u);
+            mma_ts(t_acc, t_sp + buf * 64 + kk * 8, desc_mnmajor_sw128(sV + kk * 2048, kTileBytes / 2, 1024),
+                   id_pv, (acc || kk > 0) ? 1u : 0u);
           mma_commit(BAR(kBarO + t));
-          if (release_stage >= 0) mma_commit(BAR(kBarEmpty + release_stage));
+          mma_commit(BAR(kBarEmpty + stage));
         }
         __syncwarp();
       };
@@ -228,25 +239,36 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
       for (int k = 0; k < 2 && k < n; ++k) {
         int st;
         const uint32_t sK = next_tile(st);
-        issue_qk(0, k, sK, -1);
-        issue_qk(1, k, sK, st);
+        tc_fence_after();
+        issue_qk(k, sK, st);
       }
       for (int k = 0; k < n; ++k) {
         const int buf = k & 1, ph = (k >> 1) & 1;
         const bool more = k + 2 < n;
-        int sv, sk = 0;
-        uint32_t sK = 0;
-        mbar_wait(BAR(kBarP + buf), ph);
-        const uint32_t sV = next_tile(sv);
-        issue_pv(0, buf, sV, k > 0, -1);
-        if (more) {
-          sK = next_tile(sk);
-          issue_qk(0, buf, sK, -1);
+        // one combined wait: lane 0 on P(k), lane 1 on the V(k) tile, lane 2 on the K(k+2) tile, so the
+        // three barrier latencies overlap instead of adding up on the issue path
+        const int sv = c % kStages, pv = (c / kStages) & 1;
+        const int sk = (c + 1) % kStages, pk = ((c + 1) / kStages) & 1;
+        c += more ? 2 : 1;
+        uint32_t w_bar = 0, w_par = 0;
+        if (lane == 0) { w_bar = BAR(kBarP + t * 2 + buf); w_par = ph; }
+        if (lane == 1) { w_bar = BAR(kBarFull + sv); w_par = pv; }
+        if (lane == 2 && more) { w_bar = BAR(kBarFull + sk); w_par = pk; }
+        TRACE(2 + t, 4 * k + 0);
+        {
+          uint32_t spins = 0;
+          while (true) {
+            const bool ok = (w_bar == 0) || mbar_try_wait(w_bar, w_par);
+            if (__all_sync(0xffffffffu, ok)) break;
+            if (++spins > (1u << 26)) __trap();
+          }
         }
-        mbar_wait(BAR(kBarP + 2 + buf), ph);
         tc_fence_after();
-        issue_pv(1, buf, sV, k > 0, sv);
-        if (more) issue_qk(1, buf, sK, sk);
+        TRACE(2 + t, 4 * k + 1);
+        issue_pv(buf, sKV + sv * kTileBytes, k > 0, sv);
+        TRACE(2 + t, 4 * k + 2);
+        if (more) issue_qk(buf, sKV + sk * kTileBytes, sk);
+        TRACE(2 + t, 4 * k + 3);
       }
       if (leader) mma_commit(BAR(kBarDone));
       __syncwarp();
@@ -268,12 +290,15 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
 
     for (int k = 0; k < n; ++k) {
       const int buf = k & 1, ph = (k >> 1) & 1;
+      if (w4 == 0) TRACE(t, 4 * k + 0);
       mbar_wait(BAR(kBarS + t * 2 + buf), ph);
       tc_fence_after();
+      if (w4 == 0) TRACE(t, 4 * k + 1);
       uint32_t s[64];
       tmem_ld32(t_s + buf * 64, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
       tmem_ld32(t_s + buf * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&s[32]));
       tmem_wait_ld();
+      if (w4 == 0) TRACE(t, 4 * k + 2);
       // masks: only chunks that touch the diagonal or the end of the sequence
       {
         const int k0 = s_list[k];
@@ -335,6 +360,7 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(BAR(kBarP + t * 2 + buf));
+      if (w4 == 0) TRACE(t, 4 * k + 3);
     }
 
     // epilogue: O / l -> bf16 -> global
@@ -387,6 +413,12 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
 }
 
 }  // namespace
+
+#ifdef SW_TRACE
+extern "C" __attribute__((visibility("default"))) int sw_debug_read_trace(long long* host, size_t bytes) {
+  return (int)cudaMemcpyFromSymbol(host, g_trace, bytes);
+}
+#endif
 
 namespace sw {
 

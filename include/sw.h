@@ -183,6 +183,21 @@ SW_API int32_t sw_select_topk_row(int32_t batch, int32_t block, int32_t max_bloc
                            const int32_t* seqlens, const int32_t* tau, int32_t tau_max,
                            uint32_t flags, int32_t* idx, int32_t* count, sw_stream_t stream);
 
+/* Decode selection, fused -- Alg. 2 Steps 2-6 in ONE launch: exactly the sequence
+ *   sw_sketch_append(k_new -> kbar, ks); sw_sketch_append(q -> q~_t); sw_block_scores_row;
+ *   sw_walk_update_row (with SW_ROWNORM: r_out / max|r_out|, P9); sw_select_topk_row
+ * with the same arguments and the same results up to fp32 summation order (the selected indices are
+ * bit-exact given the same r_out).  One thread-block cluster per sequence; the cached W is read once.
+ * q: [batch, h_q, d], k_new: [batch, h_kv, d] (bf16 or fp32, same dtype).  kbar [batch, max_blocks, d]
+ * and ks [batch, max_blocks, r] are updated in place for block b_curr.  r_prev (NULL = e_{b_q}),
+ * r_out: dev fp32 [batch, max_blocks].  Needs !SW_POW_MATRIX. */
+SW_API int32_t sw_decode_select(int32_t batch, int32_t block, int32_t max_blocks, const sw_tensor* q,
+                         const sw_tensor* k_new, const int32_t* seqlens, const int8_t* signs,
+                         const int32_t* cols, int32_t r, float scale, int32_t s, uint32_t flags,
+                         float* kbar, float* ks, const float* W_cache, int64_t stride_seq,
+                         const float* r_prev, float* r_out, const int32_t* tau, int32_t tau_max,
+                         int32_t* idx, int32_t* count, sw_stream_t stream);
+
 /* ---------------------------------------------------------------------------------------
  * (5) Block-sparse attention, prefill -- Alg. 1 Step 8; "zero outside selected
  *     blocks, renormalized within".

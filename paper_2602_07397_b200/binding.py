@@ -27,7 +27,7 @@ SW_OP_SKETCH, SW_OP_BLOCK_SCORES, SW_OP_WALK_UPDATE, SW_OP_SELECT_TOPK, SW_OP_AT
 
 EXPORTS = [
     "sw_sketch", "sw_sketch_append", "sw_block_scores", "sw_block_scores_row", "sw_walk_update",
-    "sw_walk_update_row", "sw_select_topk", "sw_select_topk_row", "sw_sparse_attn_prefill",
+    "sw_walk_update_row", "sw_select_topk", "sw_select_topk_row", "sw_decode_select", "sw_sparse_attn_prefill",
     "sw_sparse_attn_decode", "sw_workspace_bytes", "sw_decode_workspace_bytes", "sw_decode_num_splits",
     "sw_set_prefill_kernel", "sw_get_prefill_kernel_used", "sw_last_error", "sw_version",
 ]
@@ -67,6 +67,8 @@ def _load() -> C.CDLL:
         "sw_walk_update_row": (i32, [i32, i32, i32, vp, vp, i64, vp, vp, u32, vp, vp]),
         "sw_select_topk": (i32, [LP, vp, vp, i32, u32, vp, vp, vp]),
         "sw_select_topk_row": (i32, [i32, i32, i32, vp, vp, vp, i32, u32, vp, vp, vp]),
+        "sw_decode_select": (i32, [i32, i32, i32, TP, TP, vp, vp, vp, i32, f32, i32, u32, vp, vp, vp, i64, vp, vp,
+                                   vp, i32, vp, vp, vp]),
         "sw_sparse_attn_prefill": (i32, [LP, TP, TP, TP, vp, vp, i32, f32, u32, vp, vp, vp, sz, vp]),
         "sw_sparse_attn_decode": (i32, [i32, i32, TP, TP, TP, i64, vp, vp, vp, i32, f32, vp, vp, vp, sz, vp]),
         "sw_workspace_bytes": (sz, [i32, LP, i32, i32, i32, i32, i32]),
@@ -217,6 +219,15 @@ def sw_select_topk(L: Layout, R, tau, tau_max, flags, idx, count, stream=None) -
 def sw_select_topk_row(batch, block, max_blocks, r, seqlens, tau, tau_max, flags, idx, count, stream=None) -> None:
     _check(_lib.sw_select_topk_row(batch, block, max_blocks, _ptr(r), _ptr(seqlens), _ptr(tau), tau_max, flags,
                                    _ptr(idx), _ptr(count), _stream(stream)))
+
+
+def sw_decode_select(batch, block, max_blocks, q, k_new, seqlens, signs, cols, r, scale, s, flags, kbar, ks,
+                     W_cache, stride_seq, r_prev, r_out, tau, tau_max, idx, count, stream=None) -> None:
+    qt, kt = _tensor(q), _tensor(k_new)
+    _check(_lib.sw_decode_select(batch, block, max_blocks, C.byref(qt), C.byref(kt), _ptr(seqlens), _ptr(signs),
+                                 _ptr(cols), r, scale, s, flags, _ptr(kbar), _ptr(ks), _ptr(W_cache), stride_seq,
+                                 _ptr(r_prev), _ptr(r_out), _ptr(tau), tau_max, _ptr(idx), _ptr(count),
+                                 _stream(stream)))
 
 
 def sw_workspace_bytes(op, L: Optional[Layout], h_q=0, h_kv=0, d=0, tau_max=0, dtype=SW_BF16) -> int:

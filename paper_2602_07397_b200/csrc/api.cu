@@ -200,6 +200,31 @@ SW_API int32_t sw_select_topk_row(int32_t batch, int32_t block, int32_t max_bloc
                            (cudaStream_t)stream);
 }
 
+SW_API int32_t sw_decode_select(int32_t batch, int32_t block, int32_t max_blocks, const sw_tensor* q,
+                         const sw_tensor* k_new, const int32_t* seqlens, const int8_t* signs,
+                         const int32_t* cols, int32_t r, float scale, int32_t s, uint32_t flags, float* kbar,
+                         float* ks, const float* W_cache, int64_t stride_seq, const float* r_prev,
+                         float* r_out, const int32_t* tau, int32_t tau_max, int32_t* idx, int32_t* count,
+                         sw_stream_t stream) {
+  SW_REQUIRE(batch >= 0 && max_blocks >= 1, SW_ERR_INVALID_ARG, "batch %d / max_blocks %d", batch, max_blocks);
+  SW_REQUIRE(block == 64 || block == 128, SW_ERR_UNSUPPORTED, "block size %d not in {64,128}", block);
+  SW_TRY(validate_tensor(q, "q"));
+  SW_TRY(validate_tensor(k_new, "k_new"));
+  SW_REQUIRE(q->dtype == k_new->dtype && q->d == k_new->d, SW_ERR_UNSUPPORTED, "q / k_new dtype or head_dim differ");
+  SW_TRY(validate_sketch_params(q, cols, r));
+  SW_REQUIRE(seqlens && kbar && ks && W_cache && r_out && tau && idx && count, SW_ERR_INVALID_ARG, "NULL argument");
+  SW_REQUIRE(r_out != r_prev, SW_ERR_INVALID_ARG, "r_out must not alias r_prev");
+  SW_REQUIRE(s >= 1 && tau_max >= 1, SW_ERR_INVALID_ARG, "s = %d / tau_max = %d", s, tau_max);
+  SW_REQUIRE(!(flags & SW_POW_MATRIX), SW_ERR_UNSUPPORTED, "row mode needs the element-wise power (P4)");
+  SW_TRY(check_arch());
+  DecodeSelectArgs a;
+  a.batch = batch; a.block = block; a.max_blocks = max_blocks; a.q = *q; a.k = *k_new; a.seqlens = seqlens;
+  a.signs = signs; a.cols = cols; a.r = r; a.scale = scale; a.s = s; a.flags = flags; a.kbar = kbar; a.ks = ks;
+  a.W_cache = W_cache; a.stride_seq = stride_seq; a.r_prev = r_prev; a.r_out = r_out; a.tau = tau;
+  a.tau_max = tau_max; a.idx = idx; a.count = count;
+  return launch_decode_select(a, (cudaStream_t)stream);
+}
+
 static size_t cast_bytes(int64_t tokens, int heads, int d) {
   return ((size_t)tokens * heads * d * 2 + 255) & ~(size_t)255;
 }

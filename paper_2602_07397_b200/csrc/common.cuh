@@ -52,6 +52,27 @@ int32_t launch_select_row(int batch, int block, int max_blocks, const float* r, 
                           const int32_t* tau, int tau_max, uint32_t flags, int32_t* idx, int32_t* count,
                           cudaStream_t st);
 
+struct DecodeSelectArgs {
+  int batch, block, max_blocks;
+  sw_tensor q, k;                            // [batch, heads, d]; stride_tok = stride between sequences
+  const int32_t* seqlens;
+  const int8_t* signs;
+  const int32_t* cols;
+  int r;
+  float scale;
+  int s;
+  uint32_t flags;
+  float *kbar, *ks;
+  const float* W_cache;
+  int64_t stride_seq;
+  const float* r_prev;
+  float* r_out;
+  const int32_t* tau;
+  int tau_max;
+  int32_t *idx, *count;
+};
+int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st);
+
 struct AttnPrefillArgs {
   const sw_layout* L;
   const __nv_bfloat16 *q, *k, *v;           // bf16 operands (possibly the cast copies in ws)

@@ -1,0 +1,160 @@
+// Block-wide exact top-k of one score row (Alg. 1 Step 7 PAPER.md:788-791, Alg. 2 Step 6
+// PAPER.md:832-833; readings P7, P8): forced blocks + radix select of the rest on an
+// order-preserving uint32 image of the fp32 scores, ties to the lower index, output ascending.
+// Integer work only, hence bit-exact.  Shared by select.cu and decode_select.cu.
+//
+// One CTA of kThreads = 256 threads per row:
+//   * 4 radix passes of 8 bits; per-warp private histograms with match.any aggregation (the top
+//     byte of rescaled scores falls into a handful of bins), a 256-thread suffix scan picks the bin;
+//   * one ordered compaction: every thread owns a contiguous index range, a block scan of the
+//     (certain, equal-to-threshold) counts gives each range its output offset.
+#pragma once
+
+#include <stdint.h>
+
+namespace swsel {
+
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+
+struct Scratch {
+  uint32_t hist[kWarps][256];
+  uint32_t warp_tot[kWarps];
+  unsigned long long warp_scan[kWarps];
+  uint32_t bcast[2];
+};
+
+// fp32 -> uint32 whose unsigned order equals the float order; NaN ranks as -inf (P8)
+__device__ __forceinline__ uint32_t order_key(float v) {
+  if (v != v) v = -INFINITY;
+  if (v == 0.f) v = 0.f;               // -0 and +0 compare equal
+  uint32_t u = __float_as_uint(v);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+
+struct RowJob {
+  int n_cand;            // candidates are [0, n_cand)
+  int f0, f1;            // forced indices (-1 = none), already inside [0, n_cand), f0 != f1
+  int need;              // how many non-forced candidates to pick
+  int budget;            // total selected
+};
+
+__device__ __forceinline__ RowJob make_job(int n_cand, int diag, bool force_last, bool force_first, int tau) {
+  RowJob J;
+  J.n_cand = n_cand;
+  J.budget = min(tau, n_cand);
+  J.f0 = -1; J.f1 = -1;
+  int nf = 0;
+  if (force_last && diag >= 0 && diag < n_cand && nf < J.budget) { J.f0 = diag; ++nf; }
+  if (force_first && n_cand > 0 && 0 != J.f0 && nf < J.budget) { J.f1 = 0; ++nf; }
+  J.need = J.budget - nf;
+  return J;
+}
+
+__device__ __forceinline__ bool is_forced(const RowJob& J, int j) { return j == J.f0 || j == J.f1; }
+
+// After the 4 passes `thr` is the key of the need-th largest non-forced candidate and `n_gt` the
+// number of non-forced candidates with a strictly larger key.  All threads return the same values.
+template <typename Load>
+__device__ void radix_threshold(Load load, const RowJob& J, Scratch& S, uint32_t& thr, int& n_gt_out) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  uint32_t prefix = 0;
+  int remaining = J.need;      // rank (1-based, from the top) still to locate inside the prefix bucket
+  int n_gt = 0;
+  for (int pass = 0; pass < 4; ++pass) {
+    const int shift = 24 - 8 * pass;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) S.hist[w][tid] = 0;
+    __syncthreads();
+    const uint32_t mask_hi = (pass == 0) ? 0u : (0xffffffffu << (shift + 8));
+    for (int j0 = 0; j0 < J.n_cand; j0 += kThreads) {
+      const int j = j0 + tid;
+      uint32_t bin = 256u + lane;                       // distinct per lane: never aggregated
+      if (j < J.n_cand && !is_forced(J, j)) {
+        const uint32_t k = order_key(load(j));
+        if ((k & mask_hi) == prefix) bin = (k >> shift) & 0xffu;
+      }
+      const uint32_t peers = __match_any_sync(0xffffffffu, bin);
+      if (bin < 256u && lane == __ffs(peers) - 1) atomicAdd(&S.hist[warp][bin], (uint32_t)__popc(peers));
+    }
+    __syncthreads();
+    // thread b owns bin b: count, then an inclusive suffix sum over bins b..255
+    uint32_t cnt = 0;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) cnt += S.hist[w][tid];
+    uint32_t suf = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t v = __shfl_down_sync(0xffffffffu, suf, o);
+      if (lane + o < 32) suf += v;
+    }
+    if (lane == 0) S.warp_tot[warp] = suf;
+    __syncthreads();
+    for (int w = warp + 1; w < kWarps; ++w) suf += S.warp_tot[w];
+    const uint32_t above = suf - cnt;                   // candidates in strictly higher bins
+    if ((int)above < remaining && (int)suf >= remaining) { S.bcast[0] = (uint32_t)tid; S.bcast[1] = above; }
+    __syncthreads();
+    prefix |= S.bcast[0] << shift;
+    n_gt += (int)S.bcast[1];
+    remaining -= (int)S.bcast[1];
+  }
+  thr = prefix;
+  n_gt_out = n_gt;
+}
+
+// load(j): score of candidate j (global or shared memory).  out: tau_max ints (ascending, -1 padded).
+template <typename Load>
+__device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out, int tau_max,
+                           int32_t* __restrict__ count_out, Scratch& S) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  uint32_t thr = 0;
+  int n_gt = 0;
+  const int n_free = J.n_cand - (J.f0 >= 0) - (J.f1 >= 0);
+  const bool take_all = J.need >= n_free;
+  if (!take_all && J.need > 0) radix_threshold(load, J, S, thr, n_gt);
+  const int eq_quota = J.need - n_gt;       // equal-key candidates to take, lowest index first
+
+  // ordered compaction: thread t owns indices [t*per, (t+1)*per)
+  const int per = (J.n_cand + kThreads - 1) / kThreads;
+  const int lo = min(tid * per, J.n_cand), hi = min(lo + per, J.n_cand);
+  auto classify = [&](int j, bool& certain, bool& eq) {
+    certain = false; eq = false;
+    if (is_forced(J, j)) { certain = true; return; }
+    if (take_all) { certain = true; return; }
+    if (J.need > 0) {
+      const uint32_t k = order_key(load(j));
+      certain = k > thr;
+      eq = k == thr;
+    }
+  };
+  uint32_t n_c = 0, n_e = 0;
+  for (int j = lo; j < hi; ++j) {
+    bool c, e;
+    classify(j, c, e);
+    n_c += c; n_e += e;
+  }
+  unsigned long long v = ((unsigned long long)n_e << 32) | n_c, incl = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned long long u = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += u;
+  }
+  if (lane == 31) S.warp_scan[warp] = incl;
+  __syncthreads();
+  unsigned long long base = 0;
+  for (int w = 0; w < warp; ++w) base += S.warp_scan[w];
+  const unsigned long long excl = base + incl - v;
+  int c_before = (int)(excl & 0xffffffffu), e_before = (int)(excl >> 32);
+  for (int j = lo; j < hi; ++j) {
+    bool c, e;
+    classify(j, c, e);
+    const int pos = c_before + min(e_before, eq_quota);
+    if ((c || (e && e_before < eq_quota)) && pos < tau_max) out[pos] = j;
+    c_before += c; e_before += e;
+  }
+  for (int p = J.budget + tid; p < tau_max; p += kThreads) out[p] = -1;
+  if (tid == 0) *count_out = J.budget;
+  __syncthreads();                            // scratch may be reused by the caller
+}
+
+}  // namespace swsel

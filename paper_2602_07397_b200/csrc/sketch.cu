@@ -4,8 +4,11 @@
 // HBM-bound: every element of x is read exactly once with 128-bit loads; H_d is never
 // materialised.
 #include "common.cuh"
+#include "sketch_common.cuh"
 
 namespace {
+
+using namespace swsk;
 
 constexpr int kThreads = 256;
 constexpr int kUnroll = 8;
@@ -37,55 +40,6 @@ template <> struct Chunk<float> {
     for (int i = 0; i < 4; ++i) { acc[i] += fa[i]; acc[4 + i] += fb[i]; }
   }
 };
-
-// In-warp FWHT of a d-vector held as EPL = d/32 consecutive elements per lane
-// (element x = lane*EPL + e), natural (Sylvester) order: y[x] = sum_z v[z] (-1)^popcount(x&z).
-template <int EPL>
-__device__ __forceinline__ void fwht_warp(float (&v)[EPL], int lane) {
-#pragma unroll
-  for (int h = 1; h < EPL; h <<= 1) {
-#pragma unroll
-    for (int e = 0; e < EPL; ++e) {
-      if ((e & h) == 0) {
-        float a = v[e], b = v[e | h];
-        v[e] = a + b;
-        v[e | h] = a - b;
-      }
-    }
-  }
-#pragma unroll
-  for (int m = 1; m < 32; m <<= 1) {
-#pragma unroll
-    for (int e = 0; e < EPL; ++e) {
-      float other = __shfl_xor_sync(0xffffffffu, v[e], m);
-      v[e] = (lane & m) ? (other - v[e]) : (v[e] + other);
-    }
-  }
-}
-
-// Shared tail: warp 0 turns the d-vector in s_vec into the r-vector of the sketch.
-template <int D>
-__device__ __forceinline__ void sketch_tail(float* s_vec, const int8_t* __restrict__ signs,
-                                            const int32_t* __restrict__ cols, int r, float scale,
-                                            float* __restrict__ out_row) {
-  constexpr int EPL = D / 32;
-  const int lane = threadIdx.x & 31;
-  if (threadIdx.x < 32) {
-    float v[EPL];
-#pragma unroll
-    for (int e = 0; e < EPL; ++e) {
-      int x = lane * EPL + e;
-      float sg = signs ? (float)signs[x] : 1.f;
-      v[e] = s_vec[x] * sg;
-    }
-    fwht_warp<EPL>(v, lane);
-    __syncwarp();
-#pragma unroll
-    for (int e = 0; e < EPL; ++e) s_vec[lane * EPL + e] = v[e];
-    __syncwarp();
-    for (int c = lane; c < r; c += 32) out_row[c] = s_vec[__ldg(cols + c)] * scale;
-  }
-}
 
 template <typename T, int D>
 __global__ void __launch_bounds__(kThreads)

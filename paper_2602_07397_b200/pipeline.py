@@ -112,10 +112,19 @@ class DecodePipeline:
     def reset(self) -> None:
         self.cur = -1
 
-    def select(self, q, k_new, seqlens, kbar, ks, W_cache, stream=None) -> None:
+    def select(self, q, k_new, seqlens, kbar, ks, W_cache, stream=None, fused: bool = True) -> None:
         """q [batch,h_q,d], k_new [batch,h_kv,d]; kbar [batch,max_blocks,d], ks [batch,max_blocks,r]
-        (updated in place for block b_curr); W_cache [batch,max_blocks,max_blocks]."""
+        (updated in place for block b_curr); W_cache [batch,max_blocks,max_blocks].
+        ``fused`` = one sw_decode_select launch (default); otherwise the five row-mode calls."""
         b, B, mb = self.batch, self.B, self.max_blocks
+        if fused:
+            nxt = 0 if self.cur < 0 else 1 - self.cur
+            r_prev = None if self.cur < 0 else self.rvec[self.cur]
+            sw.sw_decode_select(b, B, mb, q, k_new, seqlens, self.signs, self.cols, self.r, self.sketch_scale,
+                                self.s, self.flags, kbar, ks, W_cache, W_cache.stride(0), r_prev, self.rvec[nxt],
+                                self.tau, self.tau_max, self.idx, self.count, stream)
+            self.cur = nxt
+            return
         sw.sw_sketch_append(b, B, mb, k_new, seqlens, self.signs, self.cols, self.r, self.sketch_scale,
                             kbar, ks, None, stream)
         sw.sw_sketch_append(b, B, mb, q, seqlens, self.signs, self.cols, self.r, self.sketch_scale,

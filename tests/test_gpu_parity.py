@@ -357,17 +357,19 @@ def test_sparse_attn_decode(sw, ts, h_q, h_kv, d, B, tau):
 
 
 # ------------------------------------------------------------------------------ decode selection path
-@pytest.mark.parametrize("t", [64 * 5 + 1, 64 * 5 + 32, 64 * 6])
-def test_decode_selection_matches_literal_alg2(sw, t):
-    """Row-vector GPU path (sketch_append, block_scores_row, walk_update_row, select_topk_row) against the
-    oracle's literal full-matrix Alg. 2, three layers, caches built by the GPU prefill path."""
+@pytest.mark.parametrize("fused", [True, False])
+@pytest.mark.parametrize("t,tau", [(64 * 5 + 1, 4), (64 * 5 + 32, 4), (64 * 6, 4), (64 * 70 + 9, 12),
+                                   (64 * 300 + 1, 40), (64 * 301, 40)])
+def test_decode_selection_matches_literal_alg2(sw, t, tau, fused):
+    """GPU decode selection -- the fused sw_decode_select launch, or the five row-vector calls (sketch_append x2,
+    block_scores_row, walk_update_row, select_topk_row) -- against the oracle's literal full-matrix Alg. 2,
+    three layers, caches built by the GPU prefill path.  The larger t span several column tiles per cluster CTA."""
     cfg = gen.CONFIGS[2]
     B, r, s, d, h_q, h_kv = cfg.B, cfg.r, cfg.s, cfg.d, 8, 2
     signs, cols, H = H_of(d, r, seed=3)
     flags = O.DEFAULT_FLAGS
     n_pre = t - 1
     b_pre, mb = O.num_blocks(n_pre, B), O.num_blocks(t, B)
-    tau = 4
     dp = sw.DecodePipeline(1, mb, h_q, h_kv, d, B, r, s, [tau], signs, cols, flags)
     R_full = None
     for layer in range(3):
@@ -381,7 +383,7 @@ def test_decode_selection_matches_literal_alg2(sw, t):
         Wc = torch.zeros(1, mb, mb, device="cuda")
         Wc[0, :b_pre, :b_pre] = pp.W.view(b_pre, b_pre)
         seqlens = dev(np.asarray([t], np.int32))
-        dp.select(Q[t - 1:t].cuda(), K[t - 1:t].cuda(), seqlens, kbar, ks, Wc)
+        dp.select(Q[t - 1:t].cuda(), K[t - 1:t].cuda(), seqlens, kbar, ks, Wc, fused=fused)
         torch.cuda.synchronize()
         # oracle, literal
         Qn, Kn = gen.to_numpy_f64(Q), gen.to_numpy_f64(K)

@@ -147,8 +147,11 @@ SW_API int32_t sw_block_scores_row(int32_t batch, int32_t block, int32_t max_blo
  *   SW_ROWNORM: each row of R_out is divided by its max-abs (P9)
  *   SW_CAUSAL: both operands are lower triangular; the strictly upper part of R_out is 0.
  * R_prev, W, R_out: dev fp32 packed (cu_sq).  R_out must not alias R_prev or W.
- * ws: dev scratch of sw_workspace_bytes(SW_OP_WALK_UPDATE, ...) bytes (only used, and only
- * needed, with SW_POW_MATRIX and s > 1; may be NULL otherwise).
+ * ws: dev scratch of sw_workspace_bytes(SW_OP_WALK_UPDATE, ...) bytes = one ping-pong matrix
+ * (batch * max_blocks^2 floats; required with SW_POW_MATRIX and s > 1, else SW_ERR_WORKSPACE) followed
+ * by the hi/lo operand images of the tensor-core kernel (4 b^2 floats; only when batch = 1, b >= 256
+ * and b % 4 == 0).  ws may be NULL or shorter otherwise: the fp32 SIMT kernel then runs (see
+ * sw_set_walk_kernel).  Both kernels keep ~fp32 accuracy (the tcgen05 one by 3xTF32 splitting).
  * ------------------------------------------------------------------------------------- */
 SW_API int32_t sw_walk_update(const sw_layout* L, const float* R_prev, const float* W, int32_t s,
                        uint32_t flags, float* R_out, void* ws, size_t ws_bytes, sw_stream_t stream);
@@ -230,7 +233,7 @@ SW_API int32_t sw_sparse_attn_decode(int32_t batch, int32_t block, const sw_tens
                               void* ws, size_t ws_bytes, sw_stream_t stream);
 
 /* Bytes of device scratch ``op`` needs for this problem (pure host functions; 0 = none).
- * SW_OP_WALK_UPDATE: only used with SW_POW_MATRIX and s > 1.  SW_OP_ATTN_PREFILL: only for
+ * SW_OP_WALK_UPDATE: see sw_walk_update.  SW_OP_ATTN_PREFILL: only for
  * dtype = SW_F32 (the bf16 cast copies, P17).  SW_OP_ATTN_DECODE: the split-KV partials
  * (batch = L->batch; or call sw_decode_workspace_bytes without a layout). */
 SW_API size_t sw_workspace_bytes(int32_t op, const sw_layout* L, int32_t h_q, int32_t h_kv, int32_t d,
@@ -253,6 +256,19 @@ SW_API int32_t sw_decode_num_splits(int32_t batch, int32_t h_kv, int32_t d, int3
 enum sw_prefill_kernel { SW_PREFILL_AUTO = 0, SW_PREFILL_GENERIC = 1, SW_PREFILL_TCGEN05 = 2 };
 SW_API int32_t sw_set_prefill_kernel(int32_t which);
 SW_API int32_t sw_get_prefill_kernel_used(void);
+
+/* Kernel choice of sw_walk_update (process-wide; for tests and benchmarks -- both are CUDA kernels of
+ * this library).
+ *   SW_WALK_AUTO (default): the tcgen05 3xTF32 GEMM when batch = 1, b >= 512, b % 4 == 0 and the
+ *                    workspace holds its operand images, else the fp32 SIMT GEMM.
+ *   SW_WALK_SIMT: always the SIMT kernel.
+ *   SW_WALK_TCGEN05: the tcgen05 kernel (b >= 256); SW_ERR_UNSUPPORTED / SW_ERR_WORKSPACE when the
+ *                    problem or the workspace does not fit it.
+ * Returns the previous setting, or SW_ERR_INVALID_ARG.  sw_get_walk_kernel_used(): the kernel the last
+ * sw_walk_update of this thread launched (SW_WALK_SIMT / SW_WALK_TCGEN05; 0 = none yet). */
+enum sw_walk_kernel { SW_WALK_AUTO = 0, SW_WALK_SIMT = 1, SW_WALK_TCGEN05 = 2 };
+SW_API int32_t sw_set_walk_kernel(int32_t which);
+SW_API int32_t sw_get_walk_kernel_used(void);
 
 SW_API const char* sw_last_error(void);
 SW_API int32_t sw_version(void);

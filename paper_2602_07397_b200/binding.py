@@ -23,13 +23,15 @@ SW_BF16, SW_F32 = 0, 1
 SW_CAUSAL, SW_SCORE_SOFTMAX, SW_POW_MATRIX, SW_FORCE_FIRST, SW_FORCE_LAST, SW_ROWNORM = 1, 2, 4, 8, 16, 32
 SW_DEFAULT_FLAGS = SW_CAUSAL | SW_SCORE_SOFTMAX | SW_FORCE_FIRST | SW_FORCE_LAST | SW_ROWNORM
 SW_PREFILL_AUTO, SW_PREFILL_GENERIC, SW_PREFILL_TCGEN05 = 0, 1, 2
+SW_WALK_AUTO, SW_WALK_SIMT, SW_WALK_TCGEN05 = 0, 1, 2
 SW_OP_SKETCH, SW_OP_BLOCK_SCORES, SW_OP_WALK_UPDATE, SW_OP_SELECT_TOPK, SW_OP_ATTN_PREFILL, SW_OP_ATTN_DECODE = range(6)
 
 EXPORTS = [
     "sw_sketch", "sw_sketch_append", "sw_block_scores", "sw_block_scores_row", "sw_walk_update",
     "sw_walk_update_row", "sw_select_topk", "sw_select_topk_row", "sw_decode_select", "sw_sparse_attn_prefill",
     "sw_sparse_attn_decode", "sw_workspace_bytes", "sw_decode_workspace_bytes", "sw_decode_num_splits",
-    "sw_set_prefill_kernel", "sw_get_prefill_kernel_used", "sw_last_error", "sw_version",
+    "sw_set_prefill_kernel", "sw_get_prefill_kernel_used", "sw_set_walk_kernel", "sw_get_walk_kernel_used",
+    "sw_last_error", "sw_version",
 ]
 
 
@@ -76,6 +78,8 @@ def _load() -> C.CDLL:
         "sw_decode_num_splits": (i32, [i32, i32, i32, i32]),
         "sw_set_prefill_kernel": (i32, [i32]),
         "sw_get_prefill_kernel_used": (i32, []),
+        "sw_set_walk_kernel": (i32, [i32]),
+        "sw_get_walk_kernel_used": (i32, []),
         "sw_last_error": (C.c_char_p, []),
         "sw_version": (i32, []),
     }
@@ -169,6 +173,17 @@ def sw_set_prefill_kernel(which: int) -> int:
 
 def sw_get_prefill_kernel_used() -> int:
     return _lib.sw_get_prefill_kernel_used()
+
+
+def sw_set_walk_kernel(which: int) -> int:
+    prev = _lib.sw_set_walk_kernel(which)
+    if prev < 0:
+        raise SwError(prev, _lib.sw_last_error().decode())
+    return prev
+
+
+def sw_get_walk_kernel_used() -> int:
+    return _lib.sw_get_walk_kernel_used()
 
 
 def sw_last_error() -> str:

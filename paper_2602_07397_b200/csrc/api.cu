@@ -159,7 +159,7 @@ SW_API int32_t sw_walk_update(const sw_layout* L, const float* R_prev, const flo
   SW_REQUIRE(R_out != R_prev && R_out != W, SW_ERR_INVALID_ARG, "R_out must not alias its inputs");
   SW_REQUIRE(s >= 1, SW_ERR_INVALID_ARG, "s = %d must be >= 1", s);
   if ((flags & SW_POW_MATRIX) && s > 1) {
-    const size_t need = sw_workspace_bytes(SW_OP_WALK_UPDATE, L, 0, 0, 0, 0, SW_F32);
+    const size_t need = (size_t)L->batch * L->max_blocks * L->max_blocks * sizeof(float);
     SW_REQUIRE(ws != nullptr && ws_bytes >= need, SW_ERR_WORKSPACE,
                "sw_walk_update: workspace %zu < %zu bytes", ws_bytes, need);
   }
@@ -233,7 +233,7 @@ SW_API size_t sw_workspace_bytes(int32_t op, const sw_layout* L, int32_t h_q, in
                           int32_t tau_max, int32_t dtype) {
   switch (op) {
     case SW_OP_WALK_UPDATE:
-      return L ? (size_t)L->batch * L->max_blocks * L->max_blocks * sizeof(float) : 0;
+      return L ? (size_t)L->batch * L->max_blocks * L->max_blocks * sizeof(float) + walk_tc_ws_bytes(*L) : 0;
     case SW_OP_ATTN_PREFILL:
       if (!L || dtype != SW_F32) return 0;
       return cast_bytes(L->total_tokens, h_q, d) + 2 * cast_bytes(L->total_tokens, h_kv, d);
@@ -321,6 +321,13 @@ SW_API int32_t sw_set_prefill_kernel(int32_t which) {
   return prev;
 }
 SW_API int32_t sw_get_prefill_kernel_used(void) { return g_prefill_used; }
+
+SW_API int32_t sw_set_walk_kernel(int32_t which) {
+  SW_REQUIRE(which >= SW_WALK_AUTO && which <= SW_WALK_TCGEN05, SW_ERR_INVALID_ARG,
+             "sw_set_walk_kernel: unknown value %d", which);
+  return set_walk_kernel(which);
+}
+SW_API int32_t sw_get_walk_kernel_used(void) { return walk_kernel_used(); }
 
 SW_API int32_t sw_sparse_attn_decode(int32_t batch, int32_t block, const sw_tensor* q, const sw_tensor* kcache,
                               const sw_tensor* vcache, int64_t stride_batch, const int32_t* seqlens,

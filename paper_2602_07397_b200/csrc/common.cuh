@@ -43,6 +43,12 @@ int32_t launch_block_scores_row(int batch, int block, int max_blocks, const floa
                                 cudaStream_t st);
 int32_t launch_walk(const sw_layout& L, const float* R_prev, const float* W, int s, uint32_t flags,
                     float* R_out, void* ws, size_t ws_bytes, cudaStream_t st);
+bool walk_tc_supported(const sw_layout& L);
+size_t walk_tc_ws_bytes(const sw_layout& L);
+int32_t launch_walk_tc(int b, const float* A, const float* Bm, float* dst, float* ws4, bool split_R, bool split_W,
+                       int causal, cudaStream_t st);
+int32_t set_walk_kernel(int32_t which);
+int32_t walk_kernel_used();
 int32_t launch_walk_row(int batch, int block, int max_blocks, const float* r_prev, const float* W_cache,
                         int64_t stride_seq, const float* w_row, const int32_t* seqlens, uint32_t flags,
                         float* r_out, cudaStream_t st);

@@ -134,6 +134,15 @@ __device__ __forceinline__ uint64_t desc_mnmajor_sw128(uint32_t smem_addr, uint3
   return kDescSw128 | kDescVersion | ((uint64_t)(sbo >> 4) << 32) | ((uint64_t)(lbo >> 4) << 16) |
          (uint64_t)((smem_addr & 0x3FFFF) >> 4);
 }
+// MN-major operand of 32-bit (tf32) elements: the tensor core only transposes 32-bit data in the
+// "128-byte swizzle with 32-byte atomicity" mode (swizzle code 1; TMA SWIZZLE_128B_ATOM_32B): rows of
+// 128 B (32 elements along MN), 4 K-rows per 512-byte atom, 32-byte chunks XORed with (row % 4).
+// lbo = byte distance between 32-element MN chunks, sbo = byte distance between 4-row K groups.
+// (Measured on B200: the plain 128-byte swizzle code makes a kind::tf32 MN-major MMA write zeros.)
+__device__ __forceinline__ uint64_t desc_mnmajor_sw128_atom32(uint32_t smem_addr, uint32_t lbo, uint32_t sbo) {
+  return ((uint64_t)1 << 61) | kDescVersion | ((uint64_t)(sbo >> 4) << 32) | ((uint64_t)(lbo >> 4) << 16) |
+         (uint64_t)((smem_addr & 0x3FFFF) >> 4);
+}
 // Instruction descriptor, kind::f16, bf16 x bf16 -> fp32: [4,6) D fmt (1 = f32), [7,10) A fmt (1 = bf16),
 // [10,13) B fmt, [15] A major (0 = K), [16] B major (0 = K, 1 = MN), [17,23) N >> 3, [24,29) M >> 4.
 __host__ __device__ constexpr uint32_t idesc_bf16(int M, int N, int a_mn_major, int b_mn_major) {

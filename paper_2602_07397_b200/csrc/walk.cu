@@ -195,19 +195,43 @@ vec_rescale_kernel(float* __restrict__ r, int max_blocks) {
 
 namespace sw {
 
+static int32_t g_walk_kernel = SW_WALK_AUTO;
+static thread_local int32_t g_walk_used = 0;
+constexpr int kWalkTcMinBlocks = 512;      // SW_WALK_AUTO: tensor-core path from this b on
+
+int32_t set_walk_kernel(int32_t which) { const int32_t prev = g_walk_kernel; g_walk_kernel = which; return prev; }
+int32_t walk_kernel_used() { return g_walk_used; }
+
 int32_t launch_walk(const sw_layout& L, const float* R_prev, const float* W, int s, uint32_t flags,
                     float* R_out, void* ws, size_t ws_bytes, cudaStream_t st) {
   if (L.total_blocks == 0) return SW_OK;
   const int causal = (flags & SW_CAUSAL) ? 1 : 0;
   const int rownorm = (flags & SW_ROWNORM) ? 1 : 0;
   const int nprod = (flags & SW_POW_MATRIX) ? s : 1;
+  // workspace = [ping-pong matrix (batch * max_blocks^2 floats) | hi/lo images of the tcgen05 path]
+  const size_t pp_bytes = (size_t)L.batch * L.max_blocks * L.max_blocks * sizeof(float);
+  const size_t tc_bytes = walk_tc_ws_bytes(L);
+  bool use_tc = false;
+  if (g_walk_kernel != SW_WALK_SIMT && tc_bytes > 0 && ws != nullptr && ws_bytes >= pp_bytes + tc_bytes)
+    use_tc = (g_walk_kernel == SW_WALK_TCGEN05) || L.total_blocks >= kWalkTcMinBlocks;
+  if (g_walk_kernel == SW_WALK_TCGEN05 && !use_tc)
+    return fail(tc_bytes == 0 ? SW_ERR_UNSUPPORTED : SW_ERR_WORKSPACE,
+                "sw_walk_update: SW_WALK_TCGEN05 needs batch = 1, b >= 256, b %% 4 == 0 and %zu bytes of workspace",
+                pp_bytes + tc_bytes);
+  float* ws4 = use_tc ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(ws) + pp_bytes) : nullptr;
+  g_walk_used = use_tc ? SW_WALK_TCGEN05 : SW_WALK_SIMT;
   dim3 grid(cdiv(L.max_blocks, TN), cdiv(L.max_blocks, TM), L.batch);
   const float* cur = R_prev;
+  bool w_split = false;
   for (int k = 1; k <= nprod; ++k) {
     // the last product must land in R_out; alternate with the workspace before that
     float* dst = ((nprod - k) % 2 == 0) ? R_out : reinterpret_cast<float*>(ws);
     if (cur == nullptr) {                   // identity * W = W
       row_rescale_kernel<<<L.total_blocks, 128, 0, st>>>(W, dst, L.cu_blocks, L.cu_sq, L.batch, 0);
+    } else if (use_tc) {
+      const int32_t rc = launch_walk_tc(L.total_blocks, cur, W, dst, ws4, true, !w_split, causal, st);
+      if (rc != SW_OK) return rc;
+      w_split = true;
     } else {
       walk_gemm_kernel<<<grid, kThreads, 0, st>>>(cur, W, dst, L.cu_blocks, L.cu_sq, causal);
     }

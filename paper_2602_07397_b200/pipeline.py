@@ -45,7 +45,8 @@ class PrefillPipeline:
         self.cur = -1                                   # index of the live R buffer (-1: none yet)
         self.idx = torch.empty(L.total_blocks, self.tau_max, dtype=torch.int32, device=device)
         self.count = torch.empty(L.total_blocks, dtype=torch.int32, device=device)
-        nb = sw.sw_workspace_bytes(sw.SW_OP_WALK_UPDATE, L) if (flags & sw.SW_POW_MATRIX and s > 1) else 0
+        # ping-pong matrix of the matrix-power reading + operand images of the tcgen05 walk GEMM
+        nb = sw.sw_workspace_bytes(sw.SW_OP_WALK_UPDATE, L)
         self.walk_ws = torch.empty(nb, dtype=torch.uint8, device=device) if nb else None
         nb = sw.sw_workspace_bytes(sw.SW_OP_ATTN_PREFILL, L, h_q, h_kv, d, self.tau_max,
                                    sw.SW_F32 if dtype == torch.float32 else sw.SW_BF16)

@@ -149,6 +149,67 @@ def test_walk_update(sw, blocks, flags):
             off += b * b
 
 
+# tcgen05 3xTF32 walk GEMM (walk_tc.cu): same product, both kernels, fp32-class accuracy.
+@pytest.mark.parametrize("b", [256, 300, 512, 1000, 1156])
+@pytest.mark.parametrize("flags", [O.DEFAULT_FLAGS, O.DEFAULT_FLAGS & ~O.ROWNORM, O.DEFAULT_FLAGS & ~O.CAUSAL,
+                                   O.DEFAULT_FLAGS | O.POW_MATRIX, O.CAUSAL | O.ROWNORM])
+def test_walk_update_tcgen05(sw, b, flags):
+    rng = np.random.RandomState(40 + b)
+    B, s = 64, 2
+    L = sw.make_layout([b * B], B)
+    if flags & O.SCORE_SOFTMAX:
+        A = O.masked_softmax(rng.randn(b, b) * 2, flags)
+        R = O.masked_softmax(rng.randn(b, b) * 2, flags)
+    else:                                   # raw signed scores reading (P5)
+        A = np.tril(rng.randn(b, b)); R = np.tril(rng.randn(b, b))
+    mat = bool(flags & O.POW_MATRIX)
+    Wsrc = (A if mat else O.power(A, s, flags)).astype(np.float32)
+    R32 = R.astype(np.float32)
+    Wd, Rp = dev(Wsrc.ravel()), dev(R32.ravel())
+    ws = torch.empty(sw.sw_workspace_bytes(sw.SW_OP_WALK_UPDATE, L), dtype=torch.uint8, device="cuda")
+    if mat:
+        ref = O.walk_update(R32.astype(np.float64), Wsrc.astype(np.float64), s, flags)
+    else:
+        ref = R32.astype(np.float64) @ Wsrc.astype(np.float64)
+        if flags & O.ROWNORM:
+            ref = O.row_rescale(ref)
+    outs = {}
+    for kern in (sw.SW_WALK_SIMT, sw.SW_WALK_TCGEN05):
+        prev = sw.sw_set_walk_kernel(kern)
+        try:
+            out = torch.full((b * b,), float("nan"), device="cuda")
+            sw.sw_walk_update(L, Rp, Wd, s, flags, out, ws)
+            torch.cuda.synchronize()
+            assert sw.sw_get_walk_kernel_used() == kern
+        finally:
+            sw.sw_set_walk_kernel(prev)
+        outs[kern] = out.cpu().numpy().reshape(b, b)
+        assert rowwise_close(outs[kern], ref)
+        if flags & O.CAUSAL:
+            assert not np.triu(outs[kern], 1).any()
+    # the split keeps fp32-class accuracy: a single TF32 product would be off by ~5e-4 of the row max
+    scale = np.abs(ref).max(axis=-1, keepdims=True)
+    err_tc = (np.abs(outs[sw.SW_WALK_TCGEN05] - ref) / scale).max()
+    assert err_tc <= 1e-5, err_tc
+
+
+def test_walk_tcgen05_needs_workspace_and_shape(sw):
+    B = 64
+    prev = sw.sw_set_walk_kernel(sw.SW_WALK_TCGEN05)
+    try:
+        for blocks, ws_ok in (((512,), False), ((100,), True), ((256, 256), True)):
+            L = sw.make_layout([b * B for b in blocks], B)
+            x = torch.zeros(L.total_sq, device="cuda")
+            out = torch.zeros(L.total_sq, device="cuda")
+            ws = torch.empty(sw.sw_workspace_bytes(sw.SW_OP_WALK_UPDATE, L) if ws_ok else 16, dtype=torch.uint8,
+                             device="cuda")
+            with pytest.raises(sw.SwError) as e:
+                sw.sw_walk_update(L, x, x, 1, O.DEFAULT_FLAGS, out, ws)
+            assert e.value.code == (sw.SW_ERR_UNSUPPORTED if ws_ok else sw.SW_ERR_WORKSPACE)
+    finally:
+        sw.sw_set_walk_kernel(prev)
+
+
 def test_walk_s1_identity_is_block_scores(sw):
     # north_star: s = 1, R^0 = I  =>  R == A (one-hop)
     rng = np.random.RandomState(8)

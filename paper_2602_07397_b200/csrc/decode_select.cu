@@ -12,9 +12,33 @@
 // (select.cuh) runs.  Three cluster barriers in total.
 #include <cooperative_groups.h>
 
+#include <algorithm>
+
 #include "common.cuh"
+
+// Phase stamps for tuning (compiled in only with -DSW_PHASE_PROF; the product build has none).
+#ifdef SW_PHASE_PROF
+__device__ unsigned long long g_sw_prof[4096 * 16];
+extern "C" __attribute__((visibility("default"))) void* sw_debug_prof_ptr() {
+  void* p = nullptr;
+  cudaGetSymbolAddress(&p, g_sw_prof);
+  return p;
+}
+#define SW_STAMP(k)                                                                 \
+  do {                                                                              \
+    if (threadIdx.x == 0) {                                                         \
+      unsigned long long t_;                                                        \
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                        \
+      g_sw_prof[(blockIdx.x & 4095) * 16 + (k)] = t_;                               \
+    }                                                                               \
+  } while (0)
+#else
+#define SW_STAMP(k) do { } while (0)
+#endif
+
 #include "select.cuh"
 #include "sketch_common.cuh"
+#include "sm100.cuh"
 
 namespace cg = cooperative_groups;
 
@@ -25,6 +49,16 @@ constexpr int kTile = 64;            // columns per tile
 constexpr int kRowGroups = 16;       // row lanes of the vector-matrix product
 constexpr int kUnroll = 8;           // independent 16-byte loads in flight per thread
 constexpr int kMaxCluster = 16;
+// W stream: cp.async ring of kStages chunks of 64 rows x 64 columns fp32 (16 KB).  Measured on B200
+// (one CTA per SM streaming HBM): cp.async 16 KB x 8 stages 6.8 TB/s, 8 KB x 8 5.5 TB/s; a TMA ring
+// (cp.async.bulk[.tensor] + mbarrier) pays ~0.27 us per box whatever its size, so it needs >= 32 KB
+// boxes, and the 128-bit register loads used before held only 32 KB per SM in flight (1.7 TB/s).
+// 5 stages keep the CTA under ~105 KB of shared memory so that two CTAs fit on an SM: one GPC of the
+// B200 has fewer than 16 free SMs, and with one CTA per SM only 7 clusters of 16 were co-resident.
+constexpr int kChunkRows = 64;
+constexpr int kStages = 5;
+constexpr int kChunkBytes = kChunkRows * kTile * 4;
+constexpr int kPieces = kChunkBytes / 16 / kThreads;     // 16-byte cp.async pieces per thread per chunk
 
 struct Params {
   const void* q;  int64_t q_stride_seq, q_stride_head;  int h_q;
@@ -38,6 +72,7 @@ struct Params {
   const int32_t* tau;  int tau_max;
   int32_t* idx;  int32_t* count;
   int B, max_blocks, slots;
+  int use_async;                     // W streamed by cp.async (needs 16-byte aligned rows), else plain loads
 };
 
 __device__ __forceinline__ float block_max(float v, float* s_red) {
@@ -70,13 +105,17 @@ decode_select_kernel(const Params p) {
   const int seq = blockIdx.x / C;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
-  extern __shared__ __align__(16) uint8_t smem_raw[];
-  const int mb4 = (p.max_blocks + 3) & ~3;                             // keeps the float4 rows aligned
-  float* s_rprev = reinterpret_cast<float*>(smem_raw);                 // [max_blocks]
-  float* s_rfull = s_rprev + mb4;                                      // [max_blocks] (used on rank 0)
-  float* s_w = s_rfull + mb4;                                          // [slots][64]: S -> w -> r
+  extern __shared__ __align__(128) uint8_t smem_raw[];
+  const int mbp = ((p.max_blocks + kTile - 1) / kTile) * kTile + kChunkRows;   // zero-padded r_prev
+  float* s_rprev = reinterpret_cast<float*>(smem_raw);                 // [mbp]
+  float* s_w = s_rprev + mbp;                                          // [slots][64]: S -> w -> r
   float* s_part = s_w + p.slots * kTile;                               // [kRowGroups][64]
-  __shared__ float s_vec[D], s_qt[128], s_kt[128];
+  uint8_t* s_ring = reinterpret_cast<uint8_t*>(
+      (reinterpret_cast<uintptr_t>(s_part + kRowGroups * kTile) + 127) & ~(uintptr_t)127);   // [kStages][16 KB]
+  float* s_rfull = reinterpret_cast<float*>(s_ring);                   // [max_blocks] on rank 0, after the walk
+  __shared__ __align__(16) float s_vec[D], s_veck[D], s_qt[128], s_kt[128], s_sign[D];
+  __shared__ float s_hq[kThreads / D][D], s_hk[kThreads / D][D];
+  __shared__ int32_t s_cols[128];
   __shared__ float s_red[kThreads / 32];
   __shared__ float s_stat[2], s_amax[1];
   __shared__ swsel::Scratch scratch;
@@ -94,51 +133,149 @@ decode_select_kernel(const Params p) {
   const int bq_tile = bq / kTile, bq_pass = bq_tile / C;
   const bool owns_bq = tile_of(bq_pass) == bq_tile;
 
-  // ---- Steps 2-3: head means, running key-block mean, sketches ----------------------------------
-  if (tid < D) {
-    const T* qp = reinterpret_cast<const T*>(p.q) + (int64_t)seq * p.q_stride_seq + tid;
-    float sq = 0.f;
-    for (int h = 0; h < p.h_q; ++h) sq += (float)qp[(int64_t)h * p.q_stride_head];
-    s_vec[tid] = sq / (float)p.h_q;                                     // PAPER.md:815
+  // ---- operand loads of Steps 2-3, issued before anything waits: head values of q and k (heads dealt
+  // to kGroups thread groups), the old running mean, the SRHT signs and columns
+  constexpr int kGroups = kThreads / D, kHeadRegs = 16;
+  const int hx = tid % D, hx_g = tid / D;
+  const T* qp = reinterpret_cast<const T*>(p.q) + (int64_t)seq * p.q_stride_seq + hx;
+  const T* kp = reinterpret_cast<const T*>(p.k) + (int64_t)seq * p.k_stride_seq + hx;
+  float qreg[kHeadRegs], kreg[kHeadRegs];
+#pragma unroll
+  for (int u = 0; u < kHeadRegs; ++u) {
+    const int h = hx_g + u * kGroups;
+    qreg[u] = (h < p.h_q) ? (float)qp[(int64_t)h * p.q_stride_head] : 0.f;
+    kreg[u] = (owns_bq && h < p.h_kv) ? (float)kp[(int64_t)h * p.k_stride_head] : 0.f;
   }
-  __syncthreads();
-  swsk::sketch_tail<D>(s_vec, p.signs, p.cols, p.r, p.scale, s_qt);     // q~_t
-  __syncthreads();
-  if (owns_bq) {
-    if (tid < D) {
-      const T* kp = reinterpret_cast<const T*>(p.k) + (int64_t)seq * p.k_stride_seq + tid;
-      float sk = 0.f;
-      for (int h = 0; h < p.h_kv; ++h) sk += (float)kp[(int64_t)h * p.k_stride_head];
-      const float avg = sk / (float)p.h_kv;
-      float* mp = p.kbar + ((int64_t)seq * mb + bq) * D + tid;
-      const float m = (cnt_in_block == 0) ? avg : ((float)cnt_in_block * (*mp) + avg) / (float)(cnt_in_block + 1);
-      *mp = m;
-      s_vec[tid] = m;
+  float kbar_old = 0.f;
+  if (owns_bq && cnt_in_block != 0 && tid >= 128 && tid < 128 + D)
+    kbar_old = p.kbar[((int64_t)seq * mb + bq) * D + (tid - 128)];
+  if (tid < D) s_sign[tid] = p.signs ? (float)p.signs[tid] : 1.f;
+  if (tid < p.r && tid < 128) s_cols[tid] = p.cols[tid];
+
+  // ---- W stream (Step 5 operand): rows [m_lo, b_q) of this CTA's column tiles, 64-row TMA boxes.
+  // Nothing in it depends on this step's q/k, so the first kStages - 1 chunks are requested up front
+  // and land while Steps 2-4 run.
+  const bool walk = p.r_prev != nullptr;
+  const bool async = walk && p.use_async;
+  auto chunks_of = [&](int pass) {
+    const int tile = tile_of(pass);
+    const int m_lo = causal ? tile * kTile : 0;
+    return (tile < n_tiles && bq > m_lo) ? (bq - m_lo + kChunkRows - 1) / kChunkRows : 0;
+  };
+  const float* Wseq = p.W + (int64_t)seq * p.w_stride_seq;
+  int pr_pass = 0, pr_chunk = 0, pr_issued = 0;       // producer cursor (same in every thread)
+  auto issue_next = [&]() {                           // all threads: request the next chunk (or an empty group)
+    while (pr_pass < p.slots && pr_chunk >= chunks_of(pr_pass)) { ++pr_pass; pr_chunk = 0; }
+    if (pr_pass < p.slots) {
+      const int tile = tile_of(pr_pass);
+      const int m0 = (causal ? tile * kTile : 0) + pr_chunk * kChunkRows;
+      const uint32_t dst = sm100::smem_u32(s_ring + (size_t)(pr_issued % kStages) * kChunkBytes);
+#pragma unroll
+      for (int u = 0; u < kPieces; ++u) {
+        const int pc = u * kThreads + tid, rr = pc >> 4, c4 = tile * kTile + (pc & 15) * 4;
+        if (m0 + rr < bq && c4 < mb)                  // rows >= b_q / columns >= max_blocks are never read
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + pc * 16),
+                       "l"(Wseq + (int64_t)(m0 + rr) * mb + c4) : "memory");
+      }
+      ++pr_issued; ++pr_chunk;
     }
-    __syncthreads();
-    swsk::sketch_tail<D>(s_vec, p.signs, p.cols, p.r, p.scale, s_kt, p.ks + ((int64_t)seq * mb + bq) * p.r);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  if (async)
+    for (int i = 0; i < kStages - 1; ++i) issue_next();
+
+  SW_STAMP(0);
+  // ---- Steps 2-3: head means, running key-block mean, sketches ----------------------------------
+  // (the q / k / signs / cols loads were issued before the W prologue: one memory latency for all)
+  {
+    float sq = 0.f, sk = 0.f;
+#pragma unroll
+    for (int u = 0; u < kHeadRegs; ++u) { sq += qreg[u]; sk += kreg[u]; }
+    for (int h = hx_g + kHeadRegs * kGroups; h < p.h_q; h += kGroups) sq += (float)qp[(int64_t)h * p.q_stride_head];
+    if (owns_bq)
+      for (int h = hx_g + kHeadRegs * kGroups; h < p.h_kv; h += kGroups) sk += (float)kp[(int64_t)h * p.k_stride_head];
+    s_hq[hx_g][hx] = sq;
+    s_hk[hx_g][hx] = sk;
   }
+  __syncthreads();
+  if (tid < D) {
+    float sq = 0.f;
+#pragma unroll
+    for (int g = 0; g < kGroups; ++g) sq += s_hq[g][tid];
+    s_vec[tid] = sq / (float)p.h_q;                                     // PAPER.md:815
+  } else if (owns_bq && tid >= 128 && tid < 128 + D) {
+    const int x = tid - 128;
+    float sk = 0.f;
+#pragma unroll
+    for (int g = 0; g < kGroups; ++g) sk += s_hk[g][x];
+    const float avg = sk / (float)p.h_kv;
+    const float m = (cnt_in_block == 0) ? avg : ((float)cnt_in_block * kbar_old + avg) / (float)(cnt_in_block + 1);
+    p.kbar[((int64_t)seq * mb + bq) * D + x] = m;
+    s_veck[x] = m;
+  }
+  __syncthreads();
+  swsk::sketch_tail<D>(s_vec, s_sign, s_cols, p.r, p.scale, s_qt);      // q~_t
+  if (owns_bq)
+    swsk::sketch_tail<D>(s_veck, s_sign, s_cols, p.r, p.scale, s_kt, p.ks + ((int64_t)seq * mb + bq) * p.r, 4);
   __syncthreads();
 
+  SW_STAMP(1);
   // ---- Steps 3-4: the new row of scores for this CTA's columns ------------------------------------
   const float* ksb = p.ks + (int64_t)seq * mb * p.r;
   float lmax = -INFINITY;
-  for (int pass = 0; pass < p.slots; ++pass) {
-    const int tile = tile_of(pass);
-    for (int cj = warp; cj < kTile; cj += kThreads / 32) {
-      const int j = tile * kTile + cj;
-      float sc = -INFINITY;
-      if (tile < n_tiles && j < hi) {
-        const float* kp = (j == bq) ? s_kt : ksb + (int64_t)j * p.r;
-        float acc = 0.f;
-        for (int c = lane; c < p.r; c += 32) acc = fmaf(s_qt[c], kp[c], acc);
-        sc = swd::warp_sum(acc) * p.inv_sqrt_r;
+  const int q4 = p.r >> 2;                            // float4s per sketch row
+  if ((p.r & 3) == 0 && q4 <= 32 && (reinterpret_cast<uintptr_t>(ksb) & 15u) == 0) {
+    // q4 adjacent lanes share one column: all of a tile's sketch rows are requested before the first
+    // use (one memory latency per pass), partial dots meet in a fixed xor butterfly
+    const int per_pass = kTile * q4, total = p.slots * per_pass;
+    const int part = tid & (q4 - 1);
+    const float4 qv = *reinterpret_cast<const float4*>(s_qt + part * 4);
+    constexpr int kU = 8;
+    for (int i0 = 0; i0 < total; i0 += kU * kThreads) {
+      float4 kv[kU];
+      bool ok[kU];
+#pragma unroll
+      for (int u = 0; u < kU; ++u) {
+        const int i = i0 + u * kThreads + tid;
+        const int pass = i / per_pass, tile = tile_of(pass);
+        const int j = tile * kTile + (i - pass * per_pass) / q4;
+        ok[u] = i < total && tile < n_tiles && j < hi;
+        kv[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (ok[u]) {
+          const float* kp2 = (j == bq) ? s_kt : ksb + (int64_t)j * p.r;
+          kv[u] = *reinterpret_cast<const float4*>(kp2 + part * 4);
+        }
       }
-      if (lane == 0) s_w[pass * kTile + cj] = sc;
-      lmax = fmaxf(lmax, sc);
+#pragma unroll
+      for (int u = 0; u < kU; ++u) {
+        const int i = i0 + u * kThreads + tid;
+        if (i0 + u * kThreads >= total) break;                          // warp-uniform
+        float acc = fmaf(qv.w, kv[u].w, fmaf(qv.z, kv[u].z, fmaf(qv.y, kv[u].y, qv.x * kv[u].x)));
+        for (int o = q4 >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        const float sc = ok[u] ? acc * p.inv_sqrt_r : -INFINITY;
+        if (part == 0 && i < total) s_w[i / q4] = sc;                   // = s_w[pass * kTile + column]
+        lmax = fmaxf(lmax, sc);
+      }
+    }
+  } else {
+    for (int pass = 0; pass < p.slots; ++pass) {
+      const int tile = tile_of(pass);
+      for (int cj = warp; cj < kTile; cj += kThreads / 32) {
+        const int j = tile * kTile + cj;
+        float sc = -INFINITY;
+        if (tile < n_tiles && j < hi) {
+          const float* kp = (j == bq) ? s_kt : ksb + (int64_t)j * p.r;
+          float acc = 0.f;
+          for (int c = lane; c < p.r; c += 32) acc = fmaf(s_qt[c], kp[c], acc);
+          sc = swd::warp_sum(acc) * p.inv_sqrt_r;
+        }
+        if (lane == 0) s_w[pass * kTile + cj] = sc;
+        lmax = fmaxf(lmax, sc);
+      }
     }
   }
   __syncthreads();
+  SW_STAMP(2);
   if (soft) {
     const float m_i = block_max(lmax, s_red);
     float e = 0.f;
@@ -170,19 +307,45 @@ decode_select_kernel(const Params p) {
   }
   __syncthreads();
 
+  SW_STAMP(3);
   // ---- Step 5: r_out[j] = sum_{m < b_q} r_prev[m] W[m][j] + r_prev[b_q] w[j] --------------------------
   float lamax = 0.f;
   if (p.r_prev != nullptr) {
     const float* rp = p.r_prev + (int64_t)seq * mb;
-    for (int i = tid; i <= bq; i += kThreads) s_rprev[i] = __ldg(rp + i);
+    for (int i = tid; i < mbp; i += kThreads) s_rprev[i] = (i <= bq) ? __ldg(rp + i) : 0.f;
     __syncthreads();
     const float* Wm = p.W + (int64_t)seq * p.w_stride_seq;
     const int cq = tid & 15, rg = tid >> 4;
     const bool vec_ok = (mb & 3) == 0 && ((reinterpret_cast<uintptr_t>(Wm) & 15u) == 0);
+    int cons = 0;                                     // chunks consumed so far (cp.async path)
     for (int pass = 0; pass < p.slots; ++pass) {
       const int tile = tile_of(pass);
       const int col0 = tile * kTile;
       float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (async) {
+        const int m_lo = causal ? col0 : 0;
+        const int nch = chunks_of(pass);
+        for (int ch = 0; ch < nch; ++ch, ++cons) {
+          asm volatile("cp.async.wait_group %0;" ::"n"(kStages - 2) : "memory");   // chunk `cons` has landed
+          __syncthreads();                            // ... for every thread; chunk cons-1 is fully consumed
+          issue_next();                               // refill the stage chunk cons-1 occupied
+          const int m0 = m_lo + ch * kChunkRows;
+          const int rows = min(kChunkRows, bq - m0);  // rows >= b_q are not part of the product
+          const float* box = reinterpret_cast<const float*>(s_ring + (size_t)(cons % kStages) * kChunkBytes);
+#pragma unroll
+          for (int u = 0; u < kChunkRows / kRowGroups; ++u) {
+            const int rr = rg + u * kRowGroups;
+            if (rr < rows) {
+              const float4 v = *reinterpret_cast<const float4*>(box + rr * kTile + cq * 4);
+              const float a = s_rprev[m0 + rr];
+              acc.x = fmaf(a, v.x, acc.x);
+              acc.y = fmaf(a, v.y, acc.y);
+              acc.z = fmaf(a, v.z, acc.z);
+              acc.w = fmaf(a, v.w, acc.w);
+            }
+          }
+        }
+      } else
       if (tile < n_tiles) {
         const int m_lo = causal ? col0 : 0;           // W[m][j] = 0 for m < j
         const int c4 = col0 + cq * 4;
@@ -234,11 +397,13 @@ decode_select_kernel(const Params p) {
       }
       __syncthreads();
     }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
   } else {
     // r^{-1} = e_{b_q}: the product is row b_q of W', i.e. the new row itself
     for (int i = tid; i < p.slots * kTile; i += kThreads) lamax = fmaxf(lamax, fabsf(s_w[i]));
   }
 
+  SW_STAMP(4);
   // ---- P9 rescale, write r_out, gather the row on rank 0 ---------------------------------------------
   const float amax_i = block_max(lamax, s_red);
   if (tid == 0) s_amax[0] = amax_i;
@@ -261,6 +426,7 @@ decode_select_kernel(const Params p) {
   }
   for (int j = n_tiles * kTile + rk * kThreads + tid; j < mb; j += C * kThreads) ro[j] = 0.f;
   cluster.sync();
+  SW_STAMP(5);
 
   // ---- Step 6 on rank 0: S = TopK(r[0..b_q), tau - |forced|) U {b_q} (U {0}) ----------------------------
   if (rk == 0) {
@@ -270,6 +436,7 @@ decode_select_kernel(const Params p) {
     swsel::select_row([row](int j) { return row[j]; }, J, p.idx + (int64_t)seq * p.tau_max, p.tau_max,
                       p.count + seq, scratch);
   }
+  SW_STAMP(6);
 }
 
 }  // namespace
@@ -302,11 +469,17 @@ int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st) {
   else if (a.q.dtype == SW_F32 && d == 64) kern = decode_select_kernel<float, 64>;
   else return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: dtype %d / d %d", a.q.dtype, d);
 
+  // cp.async stream of the cached W needs 16-byte aligned row pieces; otherwise the plain-load path runs
+  p.use_async = a.r_prev != nullptr && a.W_cache != nullptr && aligned16(a.W_cache) && (a.max_blocks & 3) == 0 &&
+                (a.stride_seq & 3) == 0;
+
   int C = pick_cluster(a.batch, a.max_blocks);
   for (;; C >>= 1) {
     p.slots = cdiv(cdiv(a.max_blocks, kTile), C);
-    const size_t smem = sizeof(float) * ((size_t)2 * ((a.max_blocks + 3) & ~3) + (size_t)p.slots * kTile + kRowGroups * kTile);
-    if (smem > 200 * 1024) return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: max_blocks %d too large", a.max_blocks);
+    const size_t mbp = (size_t)cdiv(a.max_blocks, kTile) * kTile + kChunkRows;
+    const size_t ring = std::max(p.use_async ? (size_t)kStages * kChunkBytes : 0, sizeof(float) * (size_t)((a.max_blocks + 3) & ~3));
+    const size_t smem = sizeof(float) * (mbp + (size_t)p.slots * kTile + kRowGroups * kTile) + 128 + ring;
+    if (smem > 220 * 1024) return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: max_blocks %d too large", a.max_blocks);
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (C > 8) cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
     cudaLaunchConfig_t cfg = {};

@@ -4,13 +4,17 @@
 // Integer work only, hence bit-exact.  Shared by select.cu and decode_select.cu.
 //
 // One CTA of kThreads = 256 threads per row:
-//   * 4 radix passes of 8 bits; per-warp private histograms with match.any aggregation (the top
-//     byte of rescaled scores falls into a handful of bins), a 256-thread suffix scan picks the bin;
+//   * 4 radix passes of 8 bits on one shared histogram (match.any aggregation on the top byte, which
+//     falls into a handful of bins for rescaled scores), a 256-thread suffix scan picks the bin;
 //   * one ordered compaction: every thread owns a contiguous index range, a block scan of the
 //     (certain, equal-to-threshold) counts gives each range its output offset.
 #pragma once
 
 #include <stdint.h>
+
+#ifndef SW_STAMP
+#define SW_STAMP(k) do { } while (0)
+#endif
 
 namespace swsel {
 
@@ -18,7 +22,7 @@ constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 
 struct Scratch {
-  uint32_t hist[kWarps][256];
+  uint32_t hist[256];
   uint32_t warp_tot[kWarps];
   unsigned long long warp_scan[kWarps];
   uint32_t bcast[2];
@@ -63,25 +67,28 @@ __device__ void radix_threshold(Load load, const RowJob& J, Scratch& S, uint32_t
   int n_gt = 0;
   for (int pass = 0; pass < 4; ++pass) {
     const int shift = 24 - 8 * pass;
-#pragma unroll
-    for (int w = 0; w < kWarps; ++w) S.hist[w][tid] = 0;
+    S.hist[tid] = 0;
     __syncthreads();
     const uint32_t mask_hi = (pass == 0) ? 0u : (0xffffffffu << (shift + 8));
     for (int j0 = 0; j0 < J.n_cand; j0 += kThreads) {
       const int j = j0 + tid;
-      uint32_t bin = 256u + lane;                       // distinct per lane: never aggregated
+      uint32_t bin = 256u;                              // not a candidate of this pass
       if (j < J.n_cand && !is_forced(J, j)) {
         const uint32_t k = order_key(load(j));
         if ((k & mask_hi) == prefix) bin = (k >> shift) & 0xffu;
       }
-      const uint32_t peers = __match_any_sync(0xffffffffu, bin);
-      if (bin < 256u && lane == __ffs(peers) - 1) atomicAdd(&S.hist[warp][bin], (uint32_t)__popc(peers));
+      if (pass == 0) {
+        // the top byte (sign + 7 exponent bits) of rescaled scores falls into a handful of bins:
+        // aggregate equal bins in the warp (match.any costs one round per distinct value)
+        const uint32_t peers = __match_any_sync(0xffffffffu, bin);
+        if (bin < 256u && lane == __ffs(peers) - 1) atomicAdd(&S.hist[bin], (uint32_t)__popc(peers));
+      } else if (bin < 256u) {
+        atomicAdd(&S.hist[bin], 1u);              // lower bytes spread over the bins
+      }
     }
     __syncthreads();
     // thread b owns bin b: count, then an inclusive suffix sum over bins b..255
-    uint32_t cnt = 0;
-#pragma unroll
-    for (int w = 0; w < kWarps; ++w) cnt += S.hist[w][tid];
+    const uint32_t cnt = S.hist[tid];
     uint32_t suf = cnt;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -111,7 +118,9 @@ __device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out
   int n_gt = 0;
   const int n_free = J.n_cand - (J.f0 >= 0) - (J.f1 >= 0);
   const bool take_all = J.need >= n_free;
+  SW_STAMP(7);
   if (!take_all && J.need > 0) radix_threshold(load, J, S, thr, n_gt);
+  SW_STAMP(8);
   const int eq_quota = J.need - n_gt;       // equal-key candidates to take, lowest index first
 
   // ordered compaction: thread t owns indices [t*per, (t+1)*per)
@@ -141,6 +150,7 @@ __device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out
   }
   if (lane == 31) S.warp_scan[warp] = incl;
   __syncthreads();
+  SW_STAMP(9);
   unsigned long long base = 0;
   for (int w = 0; w < warp; ++w) base += S.warp_scan[w];
   const unsigned long long excl = base + incl - v;
@@ -152,6 +162,7 @@ __device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out
     if ((c || (e && e_before < eq_quota)) && pos < tau_max) out[pos] = j;
     c_before += c; e_before += e;
   }
+  SW_STAMP(10);
   for (int p = J.budget + tid; p < tau_max; p += kThreads) out[p] = -1;
   if (tid == 0) *count_out = J.budget;
   __syncthreads();                            // scratch may be reused by the caller

@@ -32,14 +32,14 @@ __device__ __forceinline__ void fwht_warp(float (&v)[EPL], int lane) {
   }
 }
 
-// Shared tail: warp 0 turns the d-vector in s_vec into the r-vector of the sketch.
-template <int D>
-__device__ __forceinline__ void sketch_tail(float* s_vec, const int8_t* __restrict__ signs,
-                                            const int32_t* __restrict__ cols, int r, float scale,
-                                            float* out_row, float* out_row2 = nullptr) {
+// Shared tail: one warp (warp_id) turns the d-vector in s_vec into the r-vector of the sketch.
+// signs / cols may live in global or shared memory (SG: int8_t or float elements; null = +1).
+template <int D, typename SG>
+__device__ __forceinline__ void sketch_tail(float* s_vec, const SG* signs, const int32_t* cols, int r, float scale,
+                                            float* out_row, float* out_row2 = nullptr, int warp_id = 0) {
   constexpr int EPL = D / 32;
   const int lane = threadIdx.x & 31;
-  if (threadIdx.x < 32) {
+  if ((threadIdx.x >> 5) == warp_id) {
     float v[EPL];
 #pragma unroll
     for (int e = 0; e < EPL; ++e) {
@@ -53,7 +53,7 @@ __device__ __forceinline__ void sketch_tail(float* s_vec, const int8_t* __restri
     for (int e = 0; e < EPL; ++e) s_vec[lane * EPL + e] = v[e];
     __syncwarp();
     for (int c = lane; c < r; c += 32) {
-      const float y = s_vec[__ldg(cols + c)] * scale;
+      const float y = s_vec[cols[c]] * scale;
       out_row[c] = y;
       if (out_row2) out_row2[c] = y;
     }

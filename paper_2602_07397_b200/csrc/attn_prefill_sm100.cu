@@ -73,6 +73,40 @@ __device__ __forceinline__ float ex2(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
   return r;
 }
+// 2^x on the FMA pipe for a pair of values (x <= ~16): round-to-nearest split x = n + f with the
+// 1.5*2^23 magic add, degree-3 minimax polynomial of 2^f on [-0.5, 0.5] (max relative error 7.5e-5,
+// well under the bf16 rounding of P), n added into the exponent field.  Takes MUFU work off the
+// softmax warps: ex2.approx runs at 16/clk/SM, which at 64 exps per row and key chunk costs exactly
+// as many cycles as the chunk's two MMAs.
+#ifndef SW_EARLY_Q
+#define SW_EARLY_Q 1
+#endif
+#ifndef SW_TMA_EPI
+#define SW_TMA_EPI 1
+#endif
+#ifndef SW_POLY_PAIRS
+#define SW_POLY_PAIRS 2
+#endif
+constexpr int kPolyPairs = SW_POLY_PAIRS;     // of every 8 column pairs
+__host__ __device__ constexpr bool use_poly(int pair) {          // evenly spread: pairs where the running
+  return ((pair % 8 + 1) * kPolyPairs) / 8 != ((pair % 8) * kPolyPairs) / 8;   // count k*P/8 steps up
+}
+__device__ __forceinline__ float2 ex2_poly2(float2 x) {
+  x.x = fmaxf(x.x, -125.f);
+  x.y = fmaxf(x.y, -125.f);
+  const float2 magic = make_float2(12582912.f, 12582912.f), nmagic = make_float2(-12582912.f, -12582912.f);
+  const float2 t = __fadd2_rn(x, magic);                        // low mantissa bits of t = n = rint(x)
+  const float2 nf = __fadd2_rn(t, nmagic);
+  const float2 f = __fadd2_rn(x, make_float2(-nf.x, -nf.y));
+  float2 pl = __ffma2_rn(f, make_float2(0.055171459913253784f, 0.055171459913253784f),
+                         make_float2(0.2426108568906784f, 0.2426108568906784f));
+  pl = __ffma2_rn(pl, f, make_float2(0.6932609677314758f, 0.6932609677314758f));
+  pl = __ffma2_rn(pl, f, make_float2(0.9999281167984009f, 0.9999281167984009f));
+  float2 r;
+  r.x = __uint_as_float(__float_as_uint(pl.x) + (__float_as_uint(t.x) << 23));
+  r.y = __uint_as_float(__float_as_uint(pl.y) + (__float_as_uint(t.y) << 23));
+  return r;
+}
 template <int N> __device__ __forceinline__ void reg_alloc() {
   asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N));
 }
@@ -87,7 +121,8 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
 
 __global__ void __launch_bounds__(kThreads, 1)
 attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
-                          const __grid_constant__ CUtensorMap map_v, const Params p) {
+                          const __grid_constant__ CUtensorMap map_v, const __grid_constant__ CUtensorMap map_o,
+                          const Params p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* base = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const uint32_t sQ = smem_u32(base);
@@ -114,39 +149,51 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   if (q_valid <= 0) return;
   const int q_last = q_tok0 + q_valid - 1;
 
+  if (warp == 4) TRACE(4, 0);
   // ---- one-time setup ------------------------------------------------------------------------
   if (warp == 0 && lane == 0) {
-    prefetch_tmap(&map_q); prefetch_tmap(&map_k); prefetch_tmap(&map_v);
+    prefetch_tmap(&map_q); prefetch_tmap(&map_k); prefetch_tmap(&map_v); prefetch_tmap(&map_o);
     mbar_init(BAR(kBarQ), 1);
     for (int s = 0; s < kStages; ++s) { mbar_init(BAR(kBarFull + s), 1); mbar_init(BAR(kBarEmpty + s), 2); }
     for (int i = 0; i < 4; ++i) { mbar_init(BAR(kBarS + i), 1); mbar_init(BAR(kBarP + i), 4); }
     mbar_init(BAR(kBarO), 1); mbar_init(BAR(kBarO + 1), 1);
     mbar_init(BAR(kBarDone), 2);
     fence_barrier_init();
+    // the Q tile does not depend on the chunk list: request it before the set-up barrier
+    if (SW_EARLY_Q) mbar_arrive_expect_tx(BAR(kBarQ), kQBytes);
+    if (SW_EARLY_Q) tma_load_3d(sQ, &map_q, BAR(kBarQ), 0, kvh * 4, q_tok0);
+    if (SW_EARLY_Q) tma_load_3d(sQ + kQBytes / 2, &map_q, BAR(kBarQ), 64, kvh * 4, q_tok0);
   } else if (warp == 2) {
     tmem_alloc<512>(smem_u32((const void*)s_tmem));
   } else if (warp == 3) {
-    // 64-key chunks (token offset of their first key) of the selected blocks that hold a visible key
+    // 64-key chunks (token offset of their first key) of the selected blocks that hold a visible key;
+    // the index loads of 128 list entries are issued together (one memory latency per 128 entries)
     const int cnt = __ldg(p.count + gb);
     const int32_t* list = p.idx + (int64_t)gb * p.tau_max;
     const int total = cnt * TPB;
     int n = 0;
-    for (int base_i = 0; base_i < total; base_i += 32) {
-      const int i = base_i + lane;
-      int k0 = -1;
-      if (i < total) {
-        const int j = __ldg(list + i / TPB);
-        if (j >= 0) {
-          k0 = seq_lo + j * p.B + (i % TPB) * 64;
+    for (int base_i = 0; base_i < total; base_i += 128) {
+      int jv[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int i = base_i + u * 32 + lane;
+        jv[u] = (i < total) ? __ldg(list + i / TPB) : -1;
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int i = base_i + u * 32 + lane;
+        int k0 = -1;
+        if (jv[u] >= 0) {
+          k0 = seq_lo + jv[u] * p.B + (i % TPB) * 64;
           if (k0 >= seq_hi || (p.causal && k0 > q_last)) k0 = -1;
         }
+        const unsigned m = __ballot_sync(0xffffffffu, k0 >= 0);
+        if (k0 >= 0) {
+          const int pos = n + __popc(m & ((1u << lane) - 1));
+          if (pos < kMaxChunks) s_list[pos] = k0;
+        }
+        n += __popc(m);
       }
-      const unsigned m = __ballot_sync(0xffffffffu, k0 >= 0);
-      if (k0 >= 0) {
-        const int pos = n + __popc(m & ((1u << lane) - 1));
-        if (pos < kMaxChunks) s_list[pos] = k0;
-      }
-      n += __popc(m);
     }
     if (lane == 0) *s_nchunks = min(n, kMaxChunks);
   }
@@ -157,6 +204,7 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   // operands in uniform registers instead of broadcasting them per instruction
   const uint32_t tm = __shfl_sync(0xffffffffu, *s_tmem, 0);
   const int n = __shfl_sync(0xffffffffu, *s_nchunks, 0);
+  if (warp == 4) TRACE(4, 1);
 
   if (warp < 4) {
   reg_dealloc<64>();
@@ -166,7 +214,7 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     // (the whole warp runs the loop; one elected lane issues the copies)
     if (n > 0) {
       const bool leader = elect_one();
-      if (leader) {
+      if (!SW_EARLY_Q && leader) {
         mbar_arrive_expect_tx(BAR(kBarQ), kQBytes);
         tma_load_3d(sQ, &map_q, BAR(kBarQ), 0, kvh * 4, q_tok0);
         tma_load_3d(sQ + kQBytes / 2, &map_q, BAR(kBarQ), 64, kvh * 4, q_tok0);
@@ -191,6 +239,8 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
         push(&map_v, k);
         if (k + 2 < n) push(&map_k, k + 2);
       }
+    } else {
+      if (SW_EARLY_Q) mbar_wait(BAR(kBarQ), 0);   // nothing to attend to: let the early Q load land before exit
     }
   } else if (warp == 1 || warp == 3) {
     // ===================== MMA issuers: warp 1 -> tile 0, warp 3 -> tile 1 =====================
@@ -343,12 +393,14 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
       const float2 nm2 = make_float2(-m_use, -m_use);
       float2 sum0 = make_float2(0.f, 0.f), sum1 = make_float2(0.f, 0.f);
       uint32_t pk[32];
+      // of every 8 column pairs, kPolyPairs go through the FMA-pipe polynomial (ex2_poly2) instead of
+      // MUFU ex2, spread over the loop so that both pipes stay busy
 #pragma unroll
       for (int i = 0; i < 32; i += 2) {
         const float2 x0 = __ffma2_rn(make_float2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), c2, nm2);
         const float2 x1 = __ffma2_rn(make_float2(__uint_as_float(s[2 * i + 2]), __uint_as_float(s[2 * i + 3])), c2, nm2);
-        const float2 e0 = make_float2(ex2(x0.x), ex2(x0.y));
-        const float2 e1 = make_float2(ex2(x1.x), ex2(x1.y));
+        const float2 e0 = use_poly(i) ? ex2_poly2(x0) : make_float2(ex2(x0.x), ex2(x0.y));
+        const float2 e1 = use_poly(i + 1) ? ex2_poly2(x1) : make_float2(ex2(x1.x), ex2(x1.y));
         sum0 = __fadd2_rn(sum0, e0);
         sum1 = __fadd2_rn(sum1, e1);
         pk[i] = pack_bf16(e0.x, e0.y);
@@ -364,16 +416,50 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     }
 
     // epilogue: O / l -> bf16 -> global
+    if (warp == 4) TRACE(4, 2);
     if (n > 0) {
       mbar_wait(BAR(kBarDone), 0);
       tc_fence_after();
     }
+    if (warp == 4) TRACE(4, 3);
     const int n_iter = n;
     const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
     const bool valid = q_pos <= q_last;
     const int64_t o_off = ((int64_t)q_pos * p.h_q + head) * 128;
     __nv_bfloat16* op = reinterpret_cast<__nv_bfloat16*>(p.out) + o_off;
     float* opf = reinterpret_cast<float*>(p.out) + o_off;
+    // A full 32-token tile goes out as bf16 through shared memory (the Q buffer is free once every
+    // MMA has completed) and one TMA store per d-half: row-per-thread global stores took ~6000 cycles
+    // per CTA.  Ragged tiles and fp32 output keep the direct stores.
+    const bool tile_full = q_tok0 + t * 32 + 31 <= q_last;
+    if (SW_TMA_EPI && n_iter > 0 && tile_full && !p.out_f32) {
+      const int R = t * 128 + row;                         // row of the 256-row tile = 4 * token + head
+      uint8_t* sO = base + (size_t)R * 128;
+#pragma unroll
+      for (int ch = 0; ch < 4; ++ch) {
+        uint32_t o[32];
+        tmem_ld32(t_o + ch * 32, o);
+        tmem_wait_ld();
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          uint4 w;
+          w.x = pack_bf16(__uint_as_float(o[8 * v + 0]) * inv, __uint_as_float(o[8 * v + 1]) * inv);
+          w.y = pack_bf16(__uint_as_float(o[8 * v + 2]) * inv, __uint_as_float(o[8 * v + 3]) * inv);
+          w.z = pack_bf16(__uint_as_float(o[8 * v + 4]) * inv, __uint_as_float(o[8 * v + 5]) * inv);
+          w.w = pack_bf16(__uint_as_float(o[8 * v + 6]) * inv, __uint_as_float(o[8 * v + 7]) * inv);
+          const int c16 = (ch & 1) * 4 + v;                // 16-byte chunk inside the 128-byte row of this d-half
+          *reinterpret_cast<uint4*>(sO + (ch >> 1) * (kQBytes / 2) + ((c16 ^ (R & 7)) << 4)) = w;   // SWIZZLE_128B
+        }
+      }
+      fence_proxy_async();
+      asm volatile("bar.sync %0, 128;" ::"r"(1 + t) : "memory");
+      if (row == 0) {
+        tma_store_3d(&map_o, sQ + t * 16384, 0, kvh * 4, q_tok0 + t * 32);
+        tma_store_3d(&map_o, sQ + kQBytes / 2 + t * 16384, 64, kvh * 4, q_tok0 + t * 32);
+        tma_store_commit();
+        tma_store_wait_read<0>();
+      }
+    } else {
 #pragma unroll
     for (int ch = 0; ch < 4; ++ch) {
       uint32_t o[32];
@@ -402,13 +488,16 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
         }
       }
     }
+    }
     if (p.lse && valid)
       p.lse[(int64_t)q_pos * p.h_q + head] =
           l_run > 0.f ? (m_run + log2f(l_run)) * 0.6931471805599453f : -INFINITY;
   }
 
+  if (warp == 4) TRACE(4, 4);
   tc_fence_before();
   __syncthreads();
+  if (warp == 4) TRACE(4, 5);
   if (warp == 2) tmem_dealloc<512>(tm);
 }
 
@@ -433,11 +522,18 @@ bool attn_prefill_sm100_supported(const AttnPrefillArgs& a) {
 int32_t launch_attn_prefill_sm100(const AttnPrefillArgs& a, cudaStream_t st) {
   const sw_layout& L = *a.L;
   if (L.total_blocks == 0 || L.total_tokens == 0) return SW_OK;
-  CUtensorMap mq, mk, mv;
+  CUtensorMap mq, mk, mv, mo;
   const bool ok = sm100host::make_map_thd(&mq, a.q, L.total_tokens, a.h_q, 128, a.q_stride_tok, a.q_stride_head, 4, 64) &&
                   sm100host::make_map_thd(&mk, a.k, L.total_tokens, a.h_kv, 128, a.k_stride_tok, a.k_stride_head, 1, 64) &&
                   sm100host::make_map_thd(&mv, a.v, L.total_tokens, a.h_kv, 128, a.v_stride_tok, a.v_stride_head, 1, 64);
   if (!ok) return fail(SW_ERR_CUDA, "sw_sparse_attn_prefill: cuTensorMapEncodeTiled failed");
+  // output map (bf16 output only): store box = 64 d x 4 heads x 32 tokens = one MMA tile's d-half
+  if (a.out_dtype == SW_BF16) {
+    if (!sm100host::make_map_thd(&mo, a.out, L.total_tokens, a.h_q, 128, (int64_t)a.h_q * 128, 128, 4, 32))
+      return fail(SW_ERR_CUDA, "sw_sparse_attn_prefill: cuTensorMapEncodeTiled failed (output)");
+  } else {
+    mo = mq;                                   // unused by the fp32 epilogue
+  }
   static bool attr_set = false;
   if (!attr_set) {
     if (cudaFuncSetAttribute(attn_prefill_sm100_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes) !=
@@ -452,7 +548,7 @@ int32_t launch_attn_prefill_sm100(const AttnPrefillArgs& a, cudaStream_t st) {
   p.h_q = a.h_q; p.causal = (a.flags & SW_CAUSAL) ? 1 : 0;
   p.scale_log2 = a.softmax_scale * 1.4426950408889634f;
   dim3 grid(p.total_slots, a.h_kv);
-  attn_prefill_sm100_kernel<<<grid, kThreads, kSmemBytes, st>>>(mq, mk, mv, p);
+  attn_prefill_sm100_kernel<<<grid, kThreads, kSmemBytes, st>>>(mq, mk, mv, mo, p);
   return check_launch("sw_sparse_attn_prefill(sm100)");
 }
 

@@ -9,6 +9,7 @@ import time
 import numpy as np
 import torch
 
+from paper_2602_07397_b200.replicas import max_over_ranks, rank_seed, whole_job_throughput
 from synth import gen
 
 CFG_IDX = 1
@@ -48,7 +49,7 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
     Qs, Ks, Vs = [], [], []
     for layer in range(layers):
         g = torch.Generator(device=dev)  # noqa: F841  (generator lives inside gen.planted_qkv)
-        q, k, v = gen.planted_qkv(1000 * (CFG_IDX + 1) + layer + 100003 * rank, n, cfg.h_q, cfg.h_kv, cfg.d, cfg.B,
+        q, k, v = gen.planted_qkv(rank_seed(1000 * (CFG_IDX + 1) + layer, rank), n, cfg.h_q, cfg.h_kv, cfg.d, cfg.B,
                                   torch.bfloat16, plans[0].queries[layer], plans[0].targets[layer], device=str(dev))
         Qs.append(q); Ks.append(k); Vs.append(v)
     outs = [torch.empty(n, cfg.h_q, cfg.d, dtype=torch.bfloat16, device=dev) for _ in range(2)]
@@ -92,19 +93,17 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
     if rank == 0:
         sampler.start()
     barrier()
+    launches0 = pkg.sw_launch_count()
     e0.record(stream)
     for k in range(args.steps):
         step(events[k])
     e1.record(stream)
     barrier()
+    launches = pkg.sw_launch_count() - launches0
     clocks = sampler.stop() if rank == 0 else None
-    ms_total = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms_total], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(e0.elapsed_time(e1), dist, dev)
     ms_step = ms_total / args.steps
-    value = world * n * layers / (ms_step * 1e-3)
+    value = whole_job_throughput(n * layers, world, ms_step * 1e-3)
 
     # per-kernel device times (CUDA events on the launching stream, inside the timed region)
     per = {k: [] for k in KERNELS}
@@ -144,7 +143,7 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
                      "flops_per_launch": attn_flops, "ms_per_launch": attn_ms,
                      "whole_layer_frac": (attn_flops / peak / 1e12) / (layer_ms * 1e-3)},
         "clocks": clocks,
-        "gpu_launches": args.steps * layers * 7,   # 2 sketch + scores + (walk gemm | copy) + rownorm + select + attn
+        "gpu_launches": launches,                  # counted by libsw (sw_launch_count) over the timed region
     }
     res = {"line": line, "n": n, "pipe": pipe, "Qs": Qs, "Ks": Ks, "Vs": Vs, "outs": outs}
 
@@ -196,13 +195,10 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
             e2e_step()
         barrier()
         dt = (time.perf_counter() - t0) / e2e_steps
-        if dist is not None:
-            t = torch.tensor([dt], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dt, dist, dev)
         h2d = layers * (Qs[0].numel() + Ks[0].numel() + Vs[0].numel()) * 2
         d2h = layers * outs[0].numel() * 2
-        line["e2e"] = {"value": world * n * layers / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
+        line["e2e"] = {"value": whole_job_throughput(n * layers, world, dt), "unit": UNIT, "h2d_bytes_per_step": h2d,
                        "d2h_bytes_per_step": d2h, "ms_per_step": dt * 1e3, "steps": e2e_steps,
                        "note": "pinned host Q/K/V -> device, every layer's output -> host; copies overlap compute"}
     return res
@@ -269,20 +265,41 @@ def decode_bench(pkg, args, peaks, n_layer_bufs: int = 4, steps: int = 20):
     evs = [[[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(n_model_layers)]
            for _ in range(steps)]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = pkg.sw_launch_count()
     e0.record(stream)
     for k in range(steps):
         decode_step(evs[k])
     e1.record(stream)
     torch.cuda.synchronize()
-    us_layer = e0.elapsed_time(e1) * 1e3 / (steps * n_model_layers)
+    launches = pkg.sw_launch_count() - launches0
+    us_layer_eager = e0.elapsed_time(e1) * 1e3 / (steps * n_model_layers)
+    # the decode step is launch-bound at these kernel sizes (2 launches of 35 / 140 us per layer through
+    # ctypes): capture the 32-layer step once in a CUDA graph and replay it -- the library only launches
+    # on the stream it is given, never synchronises or allocates, so its calls capture as they are
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        decode_step()
+    for _ in range(3):
+        graph.replay()
+    torch.cuda.synchronize()
+    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    g0.record(stream)
+    for k in range(steps):
+        graph.replay()
+    g1.record(stream)
+    torch.cuda.synchronize()
+    us_layer = g0.elapsed_time(g1) * 1e3 / (steps * n_model_layers)
     sel_us = statistics.mean(e[0].elapsed_time(e[1]) * 1e3 for st in evs for e in st)
     att_us = statistics.mean(e[1].elapsed_time(e[2]) * 1e3 for st in evs for e in st)
     kv_bytes = batch * tau * B * cfg.h_kv * d * 2 * 2
     gbs = kv_bytes / (att_us * 1e-6) / 1e9
     return {"workload": cfg.name, "metric": "decode_us_per_step_per_layer_at_20pct_density",
-            "us_per_layer": us_layer, "selection_us": sel_us, "attention_us": att_us,
+            "us_per_layer": us_layer, "us_per_layer_eager": us_layer_eager,
+            "launch": "one CUDA graph per 32-layer decode step (us_per_layer); eager ctypes launches (us_per_layer_eager, selection_us, attention_us)",
+            "selection_us": sel_us, "attention_us": att_us,
             "selection_overhead_share": sel_us / (sel_us + att_us), "batch": batch, "kv_len": t, "tau": tau,
             "splits": pkg.sw_decode_num_splits(batch, cfg.h_kv, d, tau), "layer_buffers_cycled": n_layer_bufs,
+            "steps": steps, "gpu_launches": launches,
             "roofline": {"kernel": "sw_sparse_attn_decode", "bound": "hbm", "achieved": gbs,
                          "peak": peaks.get("hbm_gbs"), "unit": "GB/s", "frac": gbs / peaks.get("hbm_gbs"),
                          "bytes_per_launch": kv_bytes, "traffic": _ncu_traffic("sw_sparse_attn_decode")}}

@@ -272,6 +272,9 @@ SW_API int32_t sw_get_walk_kernel_used(void);
 
 SW_API const char* sw_last_error(void);
 SW_API int32_t sw_version(void);
+/* Number of CUDA kernels this library has launched in the calling process so far (all streams, all calls).
+ * Host-only counter for benchmarks that report how many of the library's kernels a timed region ran. */
+SW_API uint64_t sw_launch_count(void);
 
 #ifdef __cplusplus
 }

@@ -31,7 +31,7 @@ EXPORTS = [
     "sw_walk_update_row", "sw_select_topk", "sw_select_topk_row", "sw_decode_select", "sw_sparse_attn_prefill",
     "sw_sparse_attn_decode", "sw_workspace_bytes", "sw_decode_workspace_bytes", "sw_decode_num_splits",
     "sw_set_prefill_kernel", "sw_get_prefill_kernel_used", "sw_set_walk_kernel", "sw_get_walk_kernel_used",
-    "sw_last_error", "sw_version",
+    "sw_last_error", "sw_version", "sw_launch_count",
 ]
 
 
@@ -82,6 +82,7 @@ def _load() -> C.CDLL:
         "sw_get_walk_kernel_used": (i32, []),
         "sw_last_error": (C.c_char_p, []),
         "sw_version": (i32, []),
+        "sw_launch_count": (C.c_uint64, []),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -162,6 +163,11 @@ def make_layout(seqlens: Sequence[int], block: int, device="cuda") -> Layout:
 # ---- the calls (same names as the C ABI) ------------------------------------------------------
 def sw_version() -> int:
     return _lib.sw_version()
+
+
+def sw_launch_count() -> int:
+    """Kernels launched by libsw in this process so far."""
+    return int(_lib.sw_launch_count())
 
 
 def sw_set_prefill_kernel(which: int) -> int:

@@ -1,5 +1,7 @@
 // C ABI of libsw (include/sw.h): host-side validation and dispatch.  Nothing here computes.
 #include <stdarg.h>
+
+#include <atomic>
 #include <string.h>
 
 #include "common.cuh"
@@ -46,6 +48,10 @@ int32_t check_arch() {
 }
 
 int num_sms() { return g_sms > 0 ? g_sms : 148; }
+
+static std::atomic<uint64_t> g_launches{0};
+void count_launch(int n) { g_launches.fetch_add((uint64_t)n, std::memory_order_relaxed); }
+uint64_t launches() { return g_launches.load(std::memory_order_relaxed); }
 
 int32_t check_launch(const char* what) {
   cudaError_t e = cudaGetLastError();
@@ -103,6 +109,7 @@ extern "C" {
 
 SW_API const char* sw_last_error(void) { return g_err; }
 SW_API int32_t sw_version(void) { return SW_VERSION; }
+SW_API uint64_t sw_launch_count(void) { return sw::launches(); }
 
 SW_API int32_t sw_sketch(const sw_layout* L, const sw_tensor* x, const int8_t* signs, const int32_t* cols,
                   int32_t r, float scale, float* sketch, float* mean, sw_stream_t stream) {

@@ -306,6 +306,7 @@ static int32_t launch_decode_t(int batch, int block, const sw_tensor& q, const s
       (const __nv_bfloat16*)vc.ptr, stride_batch, kc.stride_tok, kc.stride_head, vc.stride_tok,
       vc.stride_head, q.heads, kc.heads, seqlens, block, idx, count, tau_max,
       softmax_scale * 1.4426950408889634f, nsplit, Opart, ML);
+  count_launch(2);
   attn_decode_merge_kernel<D><<<batch * q.heads, D, 0, st>>>(Opart, ML, nsplit, (__nv_bfloat16*)out, lse);
   return check_launch("sw_sparse_attn_decode");
 }

@@ -291,6 +291,7 @@ int32_t launch_cast_f32_to_bf16(const float* src, __nv_bfloat16* dst, int64_t to
                                 int64_t stride_tok, int64_t stride_head, cudaStream_t st) {
   const int64_t n8 = tokens * heads * (d / 8);
   if (n8 == 0) return SW_OK;
+  count_launch();
   cast_f32_bf16_kernel<<<(unsigned)((n8 + 255) / 256), 256, 0, st>>>(src, dst, n8, heads, d, stride_tok,
                                                                      stride_head);
   return check_launch("cast_f32_to_bf16");
@@ -310,6 +311,7 @@ static int32_t launch_generic_t(const AttnPrefillArgs& a, cudaStream_t st) {
   }
   dim3 grid(total_slots, a.h_q);
   const float scale_log2 = a.softmax_scale * 1.4426950408889634f;
+  count_launch();
   kern<<<grid, kThreads, smem, st>>>(a.q, a.k, a.v, a.q_stride_tok, a.q_stride_head, a.k_stride_tok,
                                      a.k_stride_head, a.v_stride_tok, a.v_stride_head, a.h_q, a.h_kv,
                                      L.cu_seqlens, L.cu_blocks, L.batch, L.block, total_slots, a.idx,

@@ -84,13 +84,13 @@ __device__ __forceinline__ float ex2(float x) {
 #ifndef SW_TMA_EPI
 #define SW_TMA_EPI 1
 #endif
-#ifndef SW_POLY_PAIRS
-#define SW_POLY_PAIRS 2
+#ifndef SW_POLY_MASK
+#define SW_POLY_MASK 0x88
 #endif
-constexpr int kPolyPairs = SW_POLY_PAIRS;     // of every 8 column pairs
-__host__ __device__ constexpr bool use_poly(int pair) {          // evenly spread: pairs where the running
-  return ((pair % 8 + 1) * kPolyPairs) / 8 != ((pair % 8) * kPolyPairs) / 8;   // count k*P/8 steps up
-}
+// bit q set = column pair q (mod 8) of a row takes the polynomial; which pairs matters as much as how
+// many (the compiler's interleaving of the MUFU and FMA streams changes): measured on cfg 2, 0x88
+// (pairs 3 and 7) 2.69 ms, 0x80 2.98 ms, 0xA4 2.76 ms, none 2.93 ms
+__host__ __device__ constexpr bool use_poly(int pair) { return (SW_POLY_MASK >> (pair % 8)) & 1; }
 __device__ __forceinline__ float2 ex2_poly2(float2 x) {
   x.x = fmaxf(x.x, -125.f);
   x.y = fmaxf(x.y, -125.f);
@@ -393,8 +393,7 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
       const float2 nm2 = make_float2(-m_use, -m_use);
       float2 sum0 = make_float2(0.f, 0.f), sum1 = make_float2(0.f, 0.f);
       uint32_t pk[32];
-      // of every 8 column pairs, kPolyPairs go through the FMA-pipe polynomial (ex2_poly2) instead of
-      // MUFU ex2, spread over the loop so that both pipes stay busy
+      // the column pairs of SW_POLY_MASK go through the FMA-pipe polynomial (ex2_poly2) instead of MUFU ex2
 #pragma unroll
       for (int i = 0; i < 32; i += 2) {
         const float2 x0 = __ffma2_rn(make_float2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), c2, nm2);
@@ -548,6 +547,7 @@ int32_t launch_attn_prefill_sm100(const AttnPrefillArgs& a, cudaStream_t st) {
   p.h_q = a.h_q; p.causal = (a.flags & SW_CAUSAL) ? 1 : 0;
   p.scale_log2 = a.softmax_scale * 1.4426950408889634f;
   dim3 grid(p.total_slots, a.h_kv);
+  count_launch();
   attn_prefill_sm100_kernel<<<grid, kThreads, kSmemBytes, st>>>(mq, mk, mv, mo, p);
   return check_launch("sw_sparse_attn_prefill(sm100)");
 }

@@ -17,6 +17,8 @@ int32_t fail(int32_t code, const char* fmt, ...);
 int32_t check_arch();                      // SW_OK or SW_ERR_ARCH (cached per device)
 int32_t check_launch(const char* what);    // cudaGetLastError -> SW_ERR_CUDA
 int num_sms();
+void count_launch(int n = 1);
+uint64_t launches();           // kernels launched by this library (sw_launch_count)
 
 #define SW_REQUIRE(cond, code, ...)            \
   do {                                         \

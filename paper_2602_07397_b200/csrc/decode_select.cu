@@ -492,7 +492,7 @@ int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st) {
     attr[0].val.clusterDim.x = C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
     cudaError_t e = cudaLaunchKernelEx(&cfg, kern, p);
-    if (e == cudaSuccess) break;
+    if (e == cudaSuccess) { count_launch(); break; }
     cudaGetLastError();
     if (C == 1) return fail(SW_ERR_CUDA, "sw_decode_select: %s", cudaGetErrorString(e));
   }

@@ -243,6 +243,7 @@ int32_t launch_block_scores(const sw_layout& L, const float* qs, const float* ks
     attr_set = true;
   }
   dim3 grid(cdiv(L.max_blocks, kCols), cdiv(L.max_blocks, kRows), L.batch);
+  count_launch(2);
   score_tile_kernel<<<grid, kThreads, smem, st>>>(qs, ks, r, flags, L.cu_blocks, L.cu_sq, W, 1.0f / sqrtf((float)r));
   score_rows_kernel<<<cdiv(L.total_blocks, kThreads / 32), kThreads, 0, st>>>(s, flags, L.cu_blocks, L.cu_sq, L.batch,
                                                                              W, A);
@@ -253,6 +254,7 @@ int32_t launch_block_scores_row(int batch, int block, int max_blocks, const floa
                                 const int32_t* seqlens, int r, int s, uint32_t flags, float* w_row,
                                 cudaStream_t st) {
   if (batch == 0) return SW_OK;
+  count_launch();
   block_scores_row_kernel<<<batch, 256, 0, st>>>(q_tok, ks, seqlens, block, max_blocks, r, s, flags,
                                                  w_row, 1.0f / sqrtf((float)r));
   return check_launch("sw_block_scores_row");

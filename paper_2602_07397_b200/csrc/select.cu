@@ -51,6 +51,7 @@ namespace sw {
 int32_t launch_select(const sw_layout& L, const float* R, const int32_t* tau, int tau_max,
                       uint32_t flags, int32_t* idx, int32_t* count, cudaStream_t st) {
   if (L.total_blocks == 0) return SW_OK;
+  count_launch();
   select_topk_kernel<<<L.total_blocks, kThreads, 0, st>>>(R, L.cu_blocks, L.cu_sq, L.batch, tau, tau_max,
                                                           flags, idx, count);
   return check_launch("sw_select_topk");
@@ -60,6 +61,7 @@ int32_t launch_select_row(int batch, int block, int max_blocks, const float* r, 
                           const int32_t* tau, int tau_max, uint32_t flags, int32_t* idx, int32_t* count,
                           cudaStream_t st) {
   if (batch == 0) return SW_OK;
+  count_launch();
   select_topk_row_kernel<<<batch, kThreads, 0, st>>>(r, seqlens, block, max_blocks, tau, tau_max, flags,
                                                      idx, count);
   return check_launch("sw_select_topk_row");

@@ -145,6 +145,7 @@ int32_t launch_sketch(const sw_layout& L, const sw_tensor& x, const int8_t* sign
   sketch_kernel<T, D><<<grid, block, 0, st>>>((const T*)x.ptr, x.stride_tok, x.stride_head, x.heads, \
                                               L.cu_seqlens, L.cu_blocks, L.batch, L.block, signs,    \
                                               cols, r, scale, sketch, mean)
+  count_launch();
   if (x.dtype == SW_BF16 && x.d == 128) SW_LAUNCH(__nv_bfloat16, 128);
   else if (x.dtype == SW_BF16 && x.d == 64) SW_LAUNCH(__nv_bfloat16, 64);
   else if (x.dtype == SW_F32 && x.d == 128) SW_LAUNCH(float, 128);
@@ -162,6 +163,7 @@ int32_t launch_sketch_append(int batch, int block, int max_blocks, const sw_tens
   sketch_append_kernel<T, D><<<batch, 128, 0, st>>>((const T*)x.ptr, x.stride_tok, x.stride_head, \
                                                     x.heads, seqlens, block, max_blocks, signs,   \
                                                     cols, r, scale, mean, sketch, tok_sketch)
+  count_launch();
   if (x.dtype == SW_BF16 && x.d == 128) SW_LAUNCH(__nv_bfloat16, 128);
   else if (x.dtype == SW_BF16 && x.d == 64) SW_LAUNCH(__nv_bfloat16, 64);
   else if (x.dtype == SW_F32 && x.d == 128) SW_LAUNCH(float, 128);

@@ -227,16 +227,19 @@ int32_t launch_walk(const sw_layout& L, const float* R_prev, const float* W, int
     // the last product must land in R_out; alternate with the workspace before that
     float* dst = ((nprod - k) % 2 == 0) ? R_out : reinterpret_cast<float*>(ws);
     if (cur == nullptr) {                   // identity * W = W
+      count_launch();
       row_rescale_kernel<<<L.total_blocks, 128, 0, st>>>(W, dst, L.cu_blocks, L.cu_sq, L.batch, 0);
     } else if (use_tc) {
       const int32_t rc = launch_walk_tc(L.total_blocks, cur, W, dst, ws4, true, !w_split, causal, st);
       if (rc != SW_OK) return rc;
       w_split = true;
     } else {
+      count_launch();
       walk_gemm_kernel<<<grid, kThreads, 0, st>>>(cur, W, dst, L.cu_blocks, L.cu_sq, causal);
     }
     cur = dst;
   }
+  if (rownorm) count_launch();
   if (rownorm)
     row_rescale_kernel<<<L.total_blocks, 128, 0, st>>>(R_out, R_out, L.cu_blocks, L.cu_sq, L.batch, 1);
   return check_launch("sw_walk_update");
@@ -247,6 +250,7 @@ int32_t launch_walk_row(int batch, int block, int max_blocks, const float* r_pre
                         float* r_out, cudaStream_t st) {
   if (batch == 0) return SW_OK;
   dim3 grid(cdiv(max_blocks, 32), batch);
+  count_launch((flags & SW_ROWNORM) ? 2 : 1);
   walk_row_kernel<<<grid, 256, 0, st>>>(r_prev, W_cache, stride_seq, w_row, seqlens, block, max_blocks,
                                         (flags & SW_CAUSAL) ? 1 : 0, r_out);
   if (flags & SW_ROWNORM) vec_rescale_kernel<<<batch, 256, 0, st>>>(r_out, max_blocks);

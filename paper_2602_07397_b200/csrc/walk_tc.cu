@@ -263,6 +263,7 @@ int32_t launch_walk_tc(int b, const float* A, const float* Bm, float* dst, float
   float *Rhi = ws4, *Rlo = ws4 + bb, *Whi = ws4 + 2 * bb, *Wlo = ws4 + 3 * bb;
   if (split_R || split_W) {
     dim3 grid(b, 2);
+    count_launch();
     split_tf32_kernel<<<grid, 256, 0, st>>>(split_R ? A : nullptr, split_W ? Bm : nullptr, Rhi, Rlo, Whi, Wlo, b,
                                             causal);
   }
@@ -279,6 +280,7 @@ int32_t launch_walk_tc(int b, const float* A, const float* Bm, float* dst, float
   Params p;
   p.out = dst; p.b = b; p.nt = cdiv(b, BM); p.causal = causal;
   p.n_work = causal ? p.nt * (p.nt + 1) / 2 : p.nt * p.nt;
+  count_launch();
   walk_tc_kernel<<<p.nt * p.nt, kThreads, kSmemBytes, st>>>(mrh, mrl, mwh, mwl, p);
   return check_launch("sw_walk_update(tcgen05)");
 }

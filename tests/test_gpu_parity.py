@@ -420,7 +420,9 @@ def test_sparse_attn_decode(sw, ts, h_q, h_kv, d, B, tau):
 # ------------------------------------------------------------------------------ decode selection path
 @pytest.mark.parametrize("fused", [True, False])
 @pytest.mark.parametrize("t,tau", [(64 * 5 + 1, 4), (64 * 5 + 32, 4), (64 * 6, 4), (64 * 70 + 9, 12),
-                                   (64 * 300 + 1, 40), (64 * 301, 40)])
+                                   (64 * 300 + 1, 40), (64 * 301, 40),
+                                   # max_blocks % 4 == 0: the cp.async ring of the fused kernel (else plain loads)
+                                   (64 * 7 + 3, 4), (64 * 71 + 9, 12), (64 * 299 + 5, 40), (64 * 300, 40)])
 def test_decode_selection_matches_literal_alg2(sw, t, tau, fused):
     """GPU decode selection -- the fused sw_decode_select launch, or the five row-vector calls (sketch_append x2,
     block_scores_row, walk_update_row, select_topk_row) -- against the oracle's literal full-matrix Alg. 2,

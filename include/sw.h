@@ -160,9 +160,12 @@ SW_API int32_t sw_walk_update(const sw_layout* L, const float* R_prev, const flo
  * consumed by Step 6, and row b_q of R_prev*W depends only on row b_q of R_prev, so
  *   r_out = r_prev * W',   W' = W_cache with row b_q replaced by w_row,  r_prev = NULL -> e_{b_q}.
  * W_cache: dev fp32, sequence s at W_cache + s*stride_seq, row-major [max_blocks, max_blocks]
- * (rows < b_q are read).  w_row, r_prev, r_out: dev fp32 [batch, max_blocks]. */
+ * (rows < b_q are read).  w_row, r_prev, r_out: dev fp32 [batch, max_blocks].
+ * Cache update of Alg. 2 Step 4 ("update cached A^"): w_row is also stored as row b_q
+ * of W_cache (zeros right of the diagonal), so that when the token completes block b_q the cache holds
+ * that block's row for the following steps -- the row the literal algorithm leaves behind (P11). */
 SW_API int32_t sw_walk_update_row(int32_t batch, int32_t block, int32_t max_blocks, const float* r_prev,
-                           const float* W_cache, int64_t stride_seq, const float* w_row,
+                           float* W_cache, int64_t stride_seq, const float* w_row,
                            const int32_t* seqlens, uint32_t flags, float* r_out, sw_stream_t stream);
 
 /* ---------------------------------------------------------------------------------------
@@ -192,12 +195,14 @@ SW_API int32_t sw_select_topk_row(int32_t batch, int32_t block, int32_t max_bloc
  * with the same arguments and the same results up to fp32 summation order (the selected indices are
  * bit-exact given the same r_out).  One thread-block cluster per sequence; the cached W is read once.
  * q: [batch, h_q, d], k_new: [batch, h_kv, d] (bf16 or fp32, same dtype).  kbar [batch, max_blocks, d]
- * and ks [batch, max_blocks, r] are updated in place for block b_curr.  r_prev (NULL = e_{b_q}),
+ * and ks [batch, max_blocks, r] are updated in place for block b_curr, and the new row of W is stored
+ * as row b_q of W_cache (as sw_walk_update_row does), so consecutive decode steps -- across block
+ * boundaries too -- need no other cache maintenance than appending K/V.  r_prev (NULL = e_{b_q}),
  * r_out: dev fp32 [batch, max_blocks].  Needs !SW_POW_MATRIX. */
 SW_API int32_t sw_decode_select(int32_t batch, int32_t block, int32_t max_blocks, const sw_tensor* q,
                          const sw_tensor* k_new, const int32_t* seqlens, const int8_t* signs,
                          const int32_t* cols, int32_t r, float scale, int32_t s, uint32_t flags,
-                         float* kbar, float* ks, const float* W_cache, int64_t stride_seq,
+                         float* kbar, float* ks, float* W_cache, int64_t stride_seq,
                          const float* r_prev, float* r_out, const int32_t* tau, int32_t tau_max,
                          int32_t* idx, int32_t* count, sw_stream_t stream);
 

@@ -175,7 +175,7 @@ SW_API int32_t sw_walk_update(const sw_layout* L, const float* R_prev, const flo
 }
 
 SW_API int32_t sw_walk_update_row(int32_t batch, int32_t block, int32_t max_blocks, const float* r_prev,
-                           const float* W_cache, int64_t stride_seq, const float* w_row,
+                           float* W_cache, int64_t stride_seq, const float* w_row,
                            const int32_t* seqlens, uint32_t flags, float* r_out, sw_stream_t stream) {
   SW_REQUIRE(batch >= 0 && max_blocks >= 1, SW_ERR_INVALID_ARG, "batch %d / max_blocks %d", batch, max_blocks);
   SW_REQUIRE(block == 64 || block == 128, SW_ERR_UNSUPPORTED, "block size %d not in {64,128}", block);
@@ -210,7 +210,7 @@ SW_API int32_t sw_select_topk_row(int32_t batch, int32_t block, int32_t max_bloc
 SW_API int32_t sw_decode_select(int32_t batch, int32_t block, int32_t max_blocks, const sw_tensor* q,
                          const sw_tensor* k_new, const int32_t* seqlens, const int8_t* signs,
                          const int32_t* cols, int32_t r, float scale, int32_t s, uint32_t flags, float* kbar,
-                         float* ks, const float* W_cache, int64_t stride_seq, const float* r_prev,
+                         float* ks, float* W_cache, int64_t stride_seq, const float* r_prev,
                          float* r_out, const int32_t* tau, int32_t tau_max, int32_t* idx, int32_t* count,
                          sw_stream_t stream) {
   SW_REQUIRE(batch >= 0 && max_blocks >= 1, SW_ERR_INVALID_ARG, "batch %d / max_blocks %d", batch, max_blocks);

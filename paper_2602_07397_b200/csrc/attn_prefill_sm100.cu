@@ -27,11 +27,17 @@ namespace {
 
 using namespace sm100;
 
-constexpr int kThreads = 384;
-constexpr int kStages = 8;                    // ring of 64-key K or V tiles
+#ifndef SW_TILES
+#define SW_TILES 2
+#endif
+constexpr int kTiles = SW_TILES;              // 128-row MMA tiles per CTA: 2 (one CTA per SM) or 1 (two CTAs per SM)
+constexpr int kQTok = 32 * kTiles;            // query tokens per CTA
+constexpr int kThreads = 128 + 128 * kTiles;
+constexpr int kStages = 4 * kTiles;           // ring of 64-key K or V tiles
+constexpr int kTmemCols = 256 * kTiles;
 constexpr int kTileBytes = 64 * 128 * 2;      // 16 KB: [d-half][64 keys][128 B]
-constexpr int kQBytes = 256 * 128 * 2;        // 64 KB: [d-half][256 rows][128 B]
-constexpr int kMaxChunks = 4096;              // 64-key chunks per query row the list buffer holds
+constexpr int kQBytes = kTiles * 128 * 128 * 2;   // 32 KB per tile: [d-half][128 kTiles rows][128 B]
+constexpr int kMaxChunks = 2048 * kTiles;     // 64-key chunks per query row the list buffer holds
 constexpr int kSmemBytes = kQBytes + kStages * kTileBytes + kMaxChunks * 4 + 1024 /*align*/ + 512 /*barriers*/;
 constexpr float kRescaleThreshold = 8.0f;     // log2 units
 
@@ -119,7 +125,7 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   return r;
 }
 
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(kThreads, 3 - kTiles)
 attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
                           const __grid_constant__ CUtensorMap map_v, const __grid_constant__ CUtensorMap map_o,
                           const Params p) {
@@ -139,13 +145,14 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   // ---- work unit ---------------------------------------------------------------------------
   const int TPB = p.B >> 6;
   const int slot_id = p.total_slots - 1 - (int)blockIdx.x;     // longest rows first
-  const int gb = slot_id / TPB, sub = slot_id - gb * TPB;
+  const int QPB = p.B / kQTok;                                 // query tiles (CTAs) per block
+  const int gb = slot_id / QPB, sub = slot_id - gb * QPB;
   const int kvh = blockIdx.y;
   const int seq = swd::find_seq(p.cu_blocks, p.batch, gb);
   const int bi = gb - __ldg(p.cu_blocks + seq);
   const int seq_lo = __ldg(p.cu_seqlens + seq), seq_hi = __ldg(p.cu_seqlens + seq + 1);
-  const int q_tok0 = seq_lo + bi * p.B + sub * 64;
-  const int q_valid = min(64, seq_hi - q_tok0);
+  const int q_tok0 = seq_lo + bi * p.B + sub * kQTok;
+  const int q_valid = min(kQTok, seq_hi - q_tok0);
   if (q_valid <= 0) return;
   const int q_last = q_tok0 + q_valid - 1;
 
@@ -154,17 +161,17 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&map_q); prefetch_tmap(&map_k); prefetch_tmap(&map_v); prefetch_tmap(&map_o);
     mbar_init(BAR(kBarQ), 1);
-    for (int s = 0; s < kStages; ++s) { mbar_init(BAR(kBarFull + s), 1); mbar_init(BAR(kBarEmpty + s), 2); }
+    for (int s = 0; s < kStages; ++s) { mbar_init(BAR(kBarFull + s), 1); mbar_init(BAR(kBarEmpty + s), kTiles); }
     for (int i = 0; i < 4; ++i) { mbar_init(BAR(kBarS + i), 1); mbar_init(BAR(kBarP + i), 4); }
     mbar_init(BAR(kBarO), 1); mbar_init(BAR(kBarO + 1), 1);
-    mbar_init(BAR(kBarDone), 2);
+    mbar_init(BAR(kBarDone), kTiles);
     fence_barrier_init();
     // the Q tile does not depend on the chunk list: request it before the set-up barrier
     if (SW_EARLY_Q) mbar_arrive_expect_tx(BAR(kBarQ), kQBytes);
     if (SW_EARLY_Q) tma_load_3d(sQ, &map_q, BAR(kBarQ), 0, kvh * 4, q_tok0);
     if (SW_EARLY_Q) tma_load_3d(sQ + kQBytes / 2, &map_q, BAR(kBarQ), 64, kvh * 4, q_tok0);
   } else if (warp == 2) {
-    tmem_alloc<512>(smem_u32((const void*)s_tmem));
+    tmem_alloc<kTmemCols>(smem_u32((const void*)s_tmem));
   } else if (warp == 3) {
     // 64-key chunks (token offset of their first key) of the selected blocks that hold a visible key;
     // the index loads of 128 list entries are issued together (one memory latency per 128 entries)
@@ -242,7 +249,7 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     } else {
       if (SW_EARLY_Q) mbar_wait(BAR(kBarQ), 0);   // nothing to attend to: let the early Q load land before exit
     }
-  } else if (warp == 1 || warp == 3) {
+  } else if (warp == 1 || (warp == 3 && kTiles == 2)) {
     // ===================== MMA issuers: warp 1 -> tile 0, warp 3 -> tile 1 =====================
     // One issuing warp per tile: the barrier waits of one tile overlap the tensor work of the other
     // (tcgen05.mma issue blocks while the pipe's short queue is full, so a single issuing warp exposes
@@ -252,7 +259,7 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
       const bool leader = elect_one();
       const uint32_t id_qk = idesc_bf16(128, 64, 0, 0);
       const uint32_t id_pv = idesc_bf16(128, 128, 0, 1);
-      const uint32_t t_sp = tm + t * 128, t_acc = tm + 256 + t * 128;
+      const uint32_t t_sp = tm + t * 128, t_acc = tm + kTiles * 128 + t * 128;
       const uint32_t sQt = sQ + t * 16384;
       int c = 0;
       auto next_tile = [&](int& stage) -> uint32_t {       // waits for the next tile of the ring
@@ -325,7 +332,7 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     }
   }
   } else {
-    reg_alloc<200>();
+    reg_alloc<kTiles == 2 ? 200 : 192>();
     // ===================== softmax + epilogue: one thread per query row =====================
     const int t = (warp - 4) >> 2;                       // MMA tile
     const int w4 = warp & 3;                             // TMEM lane quadrant of this warp
@@ -333,7 +340,7 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     const int q_pos = q_tok0 + t * 32 + (row >> 2);      // global token index of this row
     const int head = kvh * 4 + (row & 3);
     const uint32_t t_s = tm + ((uint32_t)(w4 * 32) << 16) + t * 128;
-    const uint32_t t_o = tm + ((uint32_t)(w4 * 32) << 16) + 256 + t * 128;
+    const uint32_t t_o = tm + ((uint32_t)(w4 * 32) << 16) + kTiles * 128 + t * 128;
     float m_run = -INFINITY, l_run = 0.f;
     const float c = p.scale_log2;
     const float2 c2 = make_float2(c, c);
@@ -497,7 +504,7 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   tc_fence_before();
   __syncthreads();
   if (warp == 4) TRACE(4, 5);
-  if (warp == 2) tmem_dealloc<512>(tm);
+  if (warp == 2) tmem_dealloc<kTmemCols>(tm);
 }
 
 }  // namespace
@@ -522,7 +529,7 @@ int32_t launch_attn_prefill_sm100(const AttnPrefillArgs& a, cudaStream_t st) {
   const sw_layout& L = *a.L;
   if (L.total_blocks == 0 || L.total_tokens == 0) return SW_OK;
   CUtensorMap mq, mk, mv, mo;
-  const bool ok = sm100host::make_map_thd(&mq, a.q, L.total_tokens, a.h_q, 128, a.q_stride_tok, a.q_stride_head, 4, 64) &&
+  const bool ok = sm100host::make_map_thd(&mq, a.q, L.total_tokens, a.h_q, 128, a.q_stride_tok, a.q_stride_head, 4, kQTok) &&
                   sm100host::make_map_thd(&mk, a.k, L.total_tokens, a.h_kv, 128, a.k_stride_tok, a.k_stride_head, 1, 64) &&
                   sm100host::make_map_thd(&mv, a.v, L.total_tokens, a.h_kv, 128, a.v_stride_tok, a.v_stride_head, 1, 64);
   if (!ok) return fail(SW_ERR_CUDA, "sw_sparse_attn_prefill: cuTensorMapEncodeTiled failed");
@@ -543,7 +550,7 @@ int32_t launch_attn_prefill_sm100(const AttnPrefillArgs& a, cudaStream_t st) {
   Params p;
   p.cu_seqlens = L.cu_seqlens; p.cu_blocks = L.cu_blocks; p.idx = a.idx; p.count = a.count;
   p.out = a.out; p.lse = a.lse; p.out_f32 = (a.out_dtype == SW_F32) ? 1 : 0;
-  p.batch = L.batch; p.B = L.block; p.total_slots = L.total_blocks * (L.block / 64); p.tau_max = a.tau_max;
+  p.batch = L.batch; p.B = L.block; p.total_slots = L.total_blocks * (L.block / kQTok); p.tau_max = a.tau_max;
   p.h_q = a.h_q; p.causal = (a.flags & SW_CAUSAL) ? 1 : 0;
   p.scale_log2 = a.softmax_scale * 1.4426950408889634f;
   dim3 grid(p.total_slots, a.h_kv);

@@ -51,7 +51,7 @@ int32_t launch_walk_tc(int b, const float* A, const float* Bm, float* dst, float
                        int causal, cudaStream_t st);
 int32_t set_walk_kernel(int32_t which);
 int32_t walk_kernel_used();
-int32_t launch_walk_row(int batch, int block, int max_blocks, const float* r_prev, const float* W_cache,
+int32_t launch_walk_row(int batch, int block, int max_blocks, const float* r_prev, float* W_cache,
                         int64_t stride_seq, const float* w_row, const int32_t* seqlens, uint32_t flags,
                         float* r_out, cudaStream_t st);
 int32_t launch_select(const sw_layout& L, const float* R, const int32_t* tau, int tau_max,
@@ -71,7 +71,7 @@ struct DecodeSelectArgs {
   int s;
   uint32_t flags;
   float *kbar, *ks;
-  const float* W_cache;
+  float* W_cache;
   int64_t stride_seq;
   const float* r_prev;
   float* r_out;

@@ -67,7 +67,7 @@ struct Params {
   const int8_t* signs;  const int32_t* cols;  int r;  float scale;  float inv_sqrt_r;
   int s;  uint32_t flags;
   float* kbar;  float* ks;
-  const float* W;  int64_t w_stride_seq;
+  float* W;  int64_t w_stride_seq;
   const float* r_prev;  float* r_out;
   const int32_t* tau;  int tau_max;
   int32_t* idx;  int32_t* count;
@@ -306,6 +306,16 @@ decode_select_kernel(const Params p) {
     }
   }
   __syncthreads();
+  // Alg. 2 Step 4 cache update: the new row becomes row b_q of the cached W, zeros right
+  // of the diagonal.  Row b_q is never read while b_q is the current block (the walk reads rows < b_q).
+  {
+    float* wrow = p.W + (int64_t)seq * p.w_stride_seq + (int64_t)bq * mb;
+    for (int i = tid; i < p.slots * kTile; i += kThreads) {
+      const int pass = i / kTile;
+      const int j = tile_of(pass) * kTile + (i - pass * kTile);
+      if (j < mb) wrow[j] = s_w[i];                    // masked columns hold 0 already
+    }
+  }
 
   SW_STAMP(3);
   // ---- Step 5: r_out[j] = sum_{m < b_q} r_prev[m] W[m][j] + r_prev[b_q] w[j] --------------------------

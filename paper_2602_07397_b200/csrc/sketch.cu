@@ -17,14 +17,13 @@ template <typename T> struct Chunk;          // 8 consecutive elements of one ro
 template <> struct Chunk<__nv_bfloat16> {
   uint4 v;
   __device__ __forceinline__ void load(const __nv_bfloat16* p) { v = swd::ld_nc_v4(p); }
+  // bf16 -> fp32 is a 16-bit shift; the two halves of a word are added with one packed FADD2
   __device__ __forceinline__ void add_to(float* acc) const {
-    const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&v);
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+    float2* a2 = reinterpret_cast<float2*>(acc);
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      float2 f = __bfloat1622float2(h[i]);
-      acc[2 * i] += f.x;
-      acc[2 * i + 1] += f.y;
-    }
+    for (int i = 0; i < 4; ++i)
+      a2[i] = __fadd2_rn(a2[i], make_float2(__uint_as_float(w[i] << 16), __uint_as_float(w[i] & 0xffff0000u)));
   }
 };
 template <> struct Chunk<float> {
@@ -62,11 +61,27 @@ sketch_kernel(const T* __restrict__ x, int64_t stride_tok, int64_t stride_head, 
   const int chunk = tid % D8;                    // constant per thread: kThreads % D8 == 0
   const int rows_per_pass = kThreads / D8;       // (token, head) rows covered per pass
   const int total_rows = ntok * heads;
-  float acc[8];
+  __align__(8) float acc[8];
 #pragma unroll
   for (int i = 0; i < 8; ++i) acc[i] = 0.f;
 
   int row = tid / D8;
+  if (stride_head == D && stride_tok == (int64_t)heads * D) {
+    // packed layout: the block is one contiguous run of ntok * heads rows of D elements (no index division)
+    const T* xb = x + (int64_t)tok0 * stride_tok + chunk * 8;
+    for (; row + (kUnroll - 1) * rows_per_pass < total_rows; row += kUnroll * rows_per_pass) {
+      Chunk<T> c[kUnroll];
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) c[u].load(xb + (int64_t)(row + u * rows_per_pass) * D);
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) c[u].add_to(acc);
+    }
+    for (; row < total_rows; row += rows_per_pass) {
+      Chunk<T> c;
+      c.load(xb + (int64_t)row * D);
+      c.add_to(acc);
+    }
+  } else {
   // main loop: kUnroll independent 128-bit loads in flight per thread
   for (; row + (kUnroll - 1) * rows_per_pass < total_rows; row += kUnroll * rows_per_pass) {
     Chunk<T> c[kUnroll];
@@ -84,6 +99,7 @@ sketch_kernel(const T* __restrict__ x, int64_t stride_tok, int64_t stride_head, 
     Chunk<T> c;
     c.load(x + (int64_t)(tok0 + tok) * stride_tok + (int64_t)hd * stride_head + chunk * 8);
     c.add_to(acc);
+  }
   }
 #pragma unroll
   for (int i = 0; i < 8; ++i) s_part[tid][i] = acc[i];

@@ -139,7 +139,7 @@ row_rescale_kernel(const float* __restrict__ src, float* __restrict__ dst,
 // Decode: r_out = r_prev * W'  with W' = W_cache except row b_q = w_row (see sw.h).
 // CTA = 32 columns x 8 row lanes; deterministic reduction order.
 __global__ void __launch_bounds__(256)
-walk_row_kernel(const float* __restrict__ r_prev, const float* __restrict__ Wc, int64_t stride_seq,
+walk_row_kernel(const float* __restrict__ r_prev, float* Wc, int64_t stride_seq,
                 const float* __restrict__ w_row, const int32_t* __restrict__ seqlens, int B,
                 int max_blocks, int causal, float* __restrict__ r_out) {
   __shared__ float s_part[8][33];
@@ -150,7 +150,7 @@ walk_row_kernel(const float* __restrict__ r_prev, const float* __restrict__ Wc, 
   const int lane = threadIdx.x & 31, rl = threadIdx.x >> 5;
   const int j = blockIdx.x * 32 + lane;
   const int j_hi = causal ? bq + 1 : nb;
-  const float* W = Wc + (int64_t)seq * stride_seq;
+  float* W = Wc + (int64_t)seq * stride_seq;
   const float* wr = w_row + (int64_t)seq * max_blocks;
   float* out = r_out + (int64_t)seq * max_blocks;
   if (blockIdx.x * 32 >= max_blocks) return;
@@ -172,6 +172,9 @@ walk_row_kernel(const float* __restrict__ r_prev, const float* __restrict__ Wc, 
 #pragma unroll
     for (int k = 0; k < 8; ++k) v += s_part[k][lane];
     out[j] = (j < j_hi) ? v : 0.f;
+    // Alg. 2 Step 4 cache update: the new row becomes row b_q of the cached W (rows < b_q were the only
+    // ones read above, by any CTA)
+    W[(int64_t)bq * max_blocks + j] = (j < j_hi) ? wr[j] : 0.f;
   }
 }
 
@@ -245,7 +248,7 @@ int32_t launch_walk(const sw_layout& L, const float* R_prev, const float* W, int
   return check_launch("sw_walk_update");
 }
 
-int32_t launch_walk_row(int batch, int block, int max_blocks, const float* r_prev, const float* W_cache,
+int32_t launch_walk_row(int batch, int block, int max_blocks, const float* r_prev, float* W_cache,
                         int64_t stride_seq, const float* w_row, const int32_t* seqlens, uint32_t flags,
                         float* r_out, cudaStream_t st) {
   if (batch == 0) return SW_OK;

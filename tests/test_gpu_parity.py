@@ -465,6 +465,63 @@ def test_decode_selection_matches_literal_alg2(sw, t, tau, fused):
         assert bq in got
 
 
+@pytest.mark.parametrize("fused", [True, False])
+def test_decode_many_steps_across_a_block_boundary(sw, fused):
+    """Twelve consecutive decode steps, two layers, caches carried on the GPU with no maintenance other
+    than the calls themselves: the running key-block mean / sketch and the cached-W row of the current
+    block (Alg. 2 Step 4) are updated in place, a block completes at t = 256 and a new one starts at 257.
+    Every step is compared with the oracle's literal Alg. 2 carrying its own caches."""
+    cfg = gen.CONFIGS[2]
+    B, r, s, d, h_q, h_kv, tau, layers = cfg.B, cfg.r, cfg.s, cfg.d, 8, 2, 3, 2
+    signs, cols, H = H_of(d, r, seed=3)
+    flags = O.DEFAULT_FLAGS
+    t0, steps = 64 * 3 + 58, 12
+    n_pre, t_end = t0 - 1, t0 + steps - 1
+    b_pre, mb = O.num_blocks(n_pre, B), O.num_blocks(t_end, B)
+    assert mb == b_pre + 1
+    dp = sw.DecodePipeline(1, mb, h_q, h_kv, d, B, r, s, [tau], signs, cols, flags)
+    torch.manual_seed(11)
+    Q = [(torch.randn(t_end, h_q, d) + 0.5).bfloat16() for _ in range(layers)]
+    K = [(torch.randn(t_end, h_kv, d) + 0.5).bfloat16() for _ in range(layers)]
+    gpu, ora = [], []
+    for l in range(layers):
+        pp = sw.PrefillPipeline([n_pre], h_q, h_kv, d, B, r, s, 0.5, signs, cols, flags)
+        pp.select(Q[l][:n_pre].cuda(), K[l][:n_pre].cuda())
+        kbar = torch.zeros(1, mb, d, device="cuda"); ks = torch.zeros(1, mb, r, device="cuda")
+        kbar[0, :b_pre] = pp.kbar; ks[0, :b_pre] = pp.ks
+        Wc = torch.full((1, mb, mb), float("nan"), device="cuda")      # rows the calls must fill themselves
+        Wc[0, :b_pre, :b_pre] = pp.W.view(b_pre, b_pre)
+        Wc[0, :b_pre, b_pre:] = 0.0
+        gpu.append((kbar, ks, Wc))
+        pre = O.prefill_selection(gen.to_numpy_f64(Q[l][:n_pre]), gen.to_numpy_f64(K[l][:n_pre]), None, B=B, H_d=H,
+                                  s=s, tau=tau, flags=flags)
+        ora.append(O.DecodeCache(pre.qbar, pre.kbar, pre.S))
+    for t in range(t0, t_end + 1):
+        dp.reset()
+        R_full = None
+        seqlens = dev(np.asarray([t], np.int32))
+        bq = (t - 1) // B
+        for l in range(layers):
+            kbar, ks, Wc = gpu[l]
+            dp.select(Q[l][t - 1:t].cuda(), K[l][t - 1:t].cuda(), seqlens, kbar, ks, Wc, fused=fused)
+            torch.cuda.synchronize()
+            sel, R_full, ora[l] = O.decode_layer_literal(gen.to_numpy_f64(Q[l][t - 1]), gen.to_numpy_f64(K[l][t - 1]),
+                                                         ora[l], t, R_full, B=B, H_d=H, s=s, tau=tau, flags=flags)
+            assert rowwise_close(kbar[0, :bq + 1].cpu().numpy(), ora[l].kbar[:bq + 1])
+            assert rowwise_close(dp.rvec[dp.cur][0, :bq + 1].cpu().numpy()[None], R_full[bq][None, :bq + 1], rel=2e-3)
+            # the cached row of the current block is the new row of W (what a later step will read)
+            W_ref = O.power(O.masked_softmax(ora[l].S, flags), s, flags)
+            assert rowwise_close(Wc[0, bq, :bq + 1].cpu().numpy()[None], W_ref[bq][None, :bq + 1])
+            assert (Wc[0, bq, bq + 1:] == 0).all()
+            got = dp.idx[0, :dp.count[0].item()].cpu().numpy()
+            if not np.array_equal(got, sel):                 # only near-ties may differ
+                diff = set(got.tolist()) ^ set(sel.tolist())
+                ref_r = R_full[bq]
+                assert all(np.abs(ref_r[j] - np.sort(ref_r[1:bq])[::-1][tau - 3]) <= 1e-3 * np.abs(ref_r).max()
+                           for j in diff)
+            assert bq in got and len(got) == min(tau, bq + 1)
+
+
 # ------------------------------------------------------------------------------ end to end
 def check_overlap(idx_gpu, cnt_gpu, sel, R_ref):
     b = R_ref.shape[0]

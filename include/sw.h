@@ -237,6 +237,18 @@ SW_API int32_t sw_sparse_attn_decode(int32_t batch, int32_t block, const sw_tens
                               int32_t tau_max, float softmax_scale, void* out, float* lse,
                               void* ws, size_t ws_bytes, sw_stream_t stream);
 
+/* Paged KV cache: the same computation with K and V in one pool of pages of ``block`` tokens.
+ * kpool/vpool: [num_pages * block, h_kv, d] bf16 (page p = tokens [p*block, (p+1)*block)); logical block j of
+ * sequence s lives in page block_table[s * table_stride + j] (dev int32; entries of the selected blocks
+ * must be valid pages, others are never read).  Selected blocks are gathered page by page, so nothing is
+ * copied.  Everything else as sw_sparse_attn_decode. */
+SW_API int32_t sw_sparse_attn_decode_paged(int32_t batch, int32_t block, const sw_tensor* q,
+                                    const sw_tensor* kpool, const sw_tensor* vpool, int64_t num_pages,
+                                    const int32_t* block_table, int32_t table_stride,
+                                    const int32_t* seqlens, const int32_t* idx, const int32_t* count,
+                                    int32_t tau_max, float softmax_scale, void* out, float* lse,
+                                    void* ws, size_t ws_bytes, sw_stream_t stream);
+
 /* Bytes of device scratch ``op`` needs for this problem (pure host functions; 0 = none).
  * SW_OP_WALK_UPDATE: see sw_walk_update.  SW_OP_ATTN_PREFILL: only for
  * dtype = SW_F32 (the bf16 cast copies, P17).  SW_OP_ATTN_DECODE: the split-KV partials

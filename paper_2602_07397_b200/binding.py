@@ -29,7 +29,7 @@ SW_OP_SKETCH, SW_OP_BLOCK_SCORES, SW_OP_WALK_UPDATE, SW_OP_SELECT_TOPK, SW_OP_AT
 EXPORTS = [
     "sw_sketch", "sw_sketch_append", "sw_block_scores", "sw_block_scores_row", "sw_walk_update",
     "sw_walk_update_row", "sw_select_topk", "sw_select_topk_row", "sw_decode_select", "sw_sparse_attn_prefill",
-    "sw_sparse_attn_decode", "sw_workspace_bytes", "sw_decode_workspace_bytes", "sw_decode_num_splits",
+    "sw_sparse_attn_decode", "sw_sparse_attn_decode_paged", "sw_workspace_bytes", "sw_decode_workspace_bytes", "sw_decode_num_splits",
     "sw_set_prefill_kernel", "sw_get_prefill_kernel_used", "sw_set_walk_kernel", "sw_get_walk_kernel_used",
     "sw_last_error", "sw_version", "sw_launch_count",
 ]
@@ -73,6 +73,8 @@ def _load() -> C.CDLL:
                                    vp, i32, vp, vp, vp]),
         "sw_sparse_attn_prefill": (i32, [LP, TP, TP, TP, vp, vp, i32, f32, u32, vp, vp, vp, sz, vp]),
         "sw_sparse_attn_decode": (i32, [i32, i32, TP, TP, TP, i64, vp, vp, vp, i32, f32, vp, vp, vp, sz, vp]),
+        "sw_sparse_attn_decode_paged": (i32, [i32, i32, TP, TP, TP, i64, vp, i32, vp, vp, vp, i32, f32, vp, vp, vp, sz,
+                                              vp]),
         "sw_workspace_bytes": (sz, [i32, LP, i32, i32, i32, i32, i32]),
         "sw_decode_workspace_bytes": (sz, [i32, i32, i32, i32, i32]),
         "sw_decode_num_splits": (i32, [i32, i32, i32, i32]),
@@ -288,3 +290,21 @@ def sw_sparse_attn_decode(batch, block, q, kcache, vcache, seqlens, idx, count, 
                                       _ptr(seqlens), _ptr(idx), _ptr(count), tau_max, softmax_scale, _ptr(out),
                                       _ptr(lse), _ptr(ws), 0 if ws is None else ws.numel() * ws.element_size(),
                                       _stream(stream)))
+
+
+def sw_sparse_attn_decode_paged(batch, block, q, kpool, vpool, block_table, seqlens, idx, count, tau_max,
+                                softmax_scale, out, lse=None, ws=None, stream=None) -> None:
+    """q [batch, h_q, d]; kpool/vpool [num_pages, block, h_kv, d] (or [num_pages*block, h_kv, d]) with contiguous
+    pages; block_table [batch, max_blocks] int32: page of every logical block."""
+    if kpool.dim() == 4:
+        if kpool.shape[1] != block or not kpool.is_contiguous() or not vpool.is_contiguous():
+            raise SwError(SW_ERR_INVALID_ARG, "pools must be contiguous [num_pages, block, h_kv, d]")
+        kpool = kpool.view(-1, kpool.shape[2], kpool.shape[3]); vpool = vpool.view(-1, vpool.shape[2], vpool.shape[3])
+    if block_table.dim() != 2 or block_table.stride(1) != 1 or block_table.dtype != torch.int32:
+        raise SwError(SW_ERR_INVALID_ARG, "block_table must be int32 [batch, max_blocks] with unit stride")
+    qt, kt, vt = _tensor(q), _tensor(kpool), _tensor(vpool)
+    _check(_lib.sw_sparse_attn_decode_paged(batch, block, C.byref(qt), C.byref(kt), C.byref(vt),
+                                            kpool.shape[0] // block, _ptr(block_table), block_table.stride(0),
+                                            _ptr(seqlens), _ptr(idx), _ptr(count), tau_max, softmax_scale, _ptr(out),
+                                            _ptr(lse), _ptr(ws), 0 if ws is None else ws.numel() * ws.element_size(),
+                                            _stream(stream)))

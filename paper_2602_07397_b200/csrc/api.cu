@@ -355,7 +355,30 @@ SW_API int32_t sw_sparse_attn_decode(int32_t batch, int32_t block, const sw_tens
   SW_REQUIRE(tau_max >= 1 && stride_batch % 8 == 0, SW_ERR_INVALID_ARG, "tau_max / stride_batch");
   SW_TRY(check_arch());
   return launch_attn_decode(batch, block, *q, *kcache, *vcache, stride_batch, seqlens, idx, count, tau_max,
-                            softmax_scale, out, lse, ws, ws_bytes, (cudaStream_t)stream);
+                            softmax_scale, out, lse, ws, ws_bytes, nullptr, 0, (cudaStream_t)stream);
+}
+
+SW_API int32_t sw_sparse_attn_decode_paged(int32_t batch, int32_t block, const sw_tensor* q, const sw_tensor* kpool,
+                                    const sw_tensor* vpool, int64_t num_pages, const int32_t* block_table,
+                                    int32_t table_stride, const int32_t* seqlens, const int32_t* idx,
+                                    const int32_t* count, int32_t tau_max, float softmax_scale, void* out,
+                                    float* lse, void* ws, size_t ws_bytes, sw_stream_t stream) {
+  SW_REQUIRE(batch >= 0 && num_pages >= 0, SW_ERR_INVALID_ARG, "batch = %d / num_pages = %lld", batch, (long long)num_pages);
+  SW_REQUIRE(block == 64 || block == 128, SW_ERR_UNSUPPORTED, "block size %d not in {64,128}", block);
+  SW_TRY(validate_tensor(q, "q"));
+  SW_TRY(validate_tensor(kpool, "kpool"));
+  SW_TRY(validate_tensor(vpool, "vpool"));
+  SW_REQUIRE(q->dtype == SW_BF16 && kpool->dtype == SW_BF16 && vpool->dtype == SW_BF16, SW_ERR_UNSUPPORTED,
+             "decode attention takes bf16 q and caches");
+  SW_REQUIRE(q->d == kpool->d && q->d == vpool->d, SW_ERR_UNSUPPORTED, "head_dim mismatch");
+  SW_REQUIRE(kpool->heads == vpool->heads && q->heads % kpool->heads == 0 && q->heads / kpool->heads <= 16,
+             SW_ERR_UNSUPPORTED, "GQA group h_q/h_kv = %d/%d must be an integer <= 16", q->heads, kpool->heads);
+  SW_REQUIRE(block_table && seqlens && idx && count && out, SW_ERR_INVALID_ARG, "NULL argument");
+  SW_REQUIRE(tau_max >= 1 && table_stride >= 1, SW_ERR_INVALID_ARG, "tau_max = %d / table_stride = %d", tau_max,
+             table_stride);
+  SW_TRY(check_arch());
+  return launch_attn_decode(batch, block, *q, *kpool, *vpool, 0, seqlens, idx, count, tau_max, softmax_scale, out,
+                            lse, ws, ws_bytes, block_table, table_stride, (cudaStream_t)stream);
 }
 
 }  // extern "C"

@@ -55,6 +55,7 @@ attn_decode_kernel(const __nv_bfloat16* __restrict__ Q, int64_t q_sb, int64_t q_
                    int64_t kv_sb, int64_t k_st, int64_t k_sh, int64_t v_st, int64_t v_sh, int h_q, int h_kv,
                    const int32_t* __restrict__ seqlens, int B, const int32_t* __restrict__ idx,
                    const int32_t* __restrict__ count, int tau_max, float scale_log2, int nsplit,
+                   const int32_t* __restrict__ table, int table_stride,
                    float* __restrict__ Opart, float* __restrict__ ML) {
   extern __shared__ __align__(128) uint8_t smem_raw[];
   constexpr int TILE_BYTES = KT * D * 2;
@@ -70,13 +71,18 @@ attn_decode_kernel(const __nv_bfloat16* __restrict__ Q, int64_t q_sb, int64_t q_
   const int per = (cnt + nsplit - 1) / nsplit;            // selected blocks per split
   const int blk_lo = split * per, blk_hi = min(cnt, blk_lo + per);
   const int nslots = max(0, blk_hi - blk_lo) * TPB;
-  const __nv_bfloat16* Kb = Kc + (int64_t)seq * kv_sb + (int64_t)kvh * k_sh;
-  const __nv_bfloat16* Vb = Vc + (int64_t)seq * kv_sb + (int64_t)kvh * v_sh;
+  // contiguous cache: sequence s at + s * kv_sb; paged cache (table != NULL): one pool of pages of B
+  // tokens, logical block j of sequence s lives in page table[s * table_stride + j]
+  const __nv_bfloat16* Kb = Kc + (table ? 0 : (int64_t)seq * kv_sb) + (int64_t)kvh * k_sh;
+  const __nv_bfloat16* Vb = Vc + (table ? 0 : (int64_t)seq * kv_sb) + (int64_t)kvh * v_sh;
+  const int32_t* pages = table ? table + (int64_t)seq * table_stride : nullptr;
 
+  // k_tok0: token offset of the tile in memory; k_valid: keys of it that exist (logical position < t)
   auto slot_info = [&](int slot, int& k_tok0, int& k_valid) {
     const int j = __ldg(list + blk_lo + slot / TPB);
-    k_tok0 = j * B + (slot % TPB) * KT;
-    k_valid = max(0, min(KT, t - k_tok0));
+    const int off = (slot % TPB) * KT;
+    k_valid = max(0, min(KT, t - (j * B + off)));
+    k_tok0 = (pages ? __ldg(pages + j) : j) * B + off;
   };
   auto issue = [&](int slot, int stage) {
     int k_tok0, k_valid;
@@ -289,7 +295,8 @@ template <int D>
 static int32_t launch_decode_t(int batch, int block, const sw_tensor& q, const sw_tensor& kc,
                                const sw_tensor& vc, int64_t stride_batch, const int32_t* seqlens,
                                const int32_t* idx, const int32_t* count, int tau_max, float softmax_scale,
-                               void* out, float* lse, void* ws, int nsplit, cudaStream_t st) {
+                               void* out, float* lse, void* ws, int nsplit, const int32_t* table,
+                               int table_stride, cudaStream_t st) {
   const size_t ring = (size_t)kStages * 2 * KT * D * 2;
   const size_t merge = (size_t)(4 * 16 * D + 4 * 16 * 2) * sizeof(float);
   const size_t smem = ring > merge ? ring : merge;
@@ -305,7 +312,7 @@ static int32_t launch_decode_t(int batch, int block, const sw_tensor& q, const s
       (const __nv_bfloat16*)q.ptr, q.stride_tok, q.stride_head, (const __nv_bfloat16*)kc.ptr,
       (const __nv_bfloat16*)vc.ptr, stride_batch, kc.stride_tok, kc.stride_head, vc.stride_tok,
       vc.stride_head, q.heads, kc.heads, seqlens, block, idx, count, tau_max,
-      softmax_scale * 1.4426950408889634f, nsplit, Opart, ML);
+      softmax_scale * 1.4426950408889634f, nsplit, table, table_stride, Opart, ML);
   count_launch(2);
   attn_decode_merge_kernel<D><<<batch * q.heads, D, 0, st>>>(Opart, ML, nsplit, (__nv_bfloat16*)out, lse);
   return check_launch("sw_sparse_attn_decode");
@@ -314,7 +321,8 @@ static int32_t launch_decode_t(int batch, int block, const sw_tensor& q, const s
 int32_t launch_attn_decode(int batch, int block, const sw_tensor& q, const sw_tensor& kc,
                            const sw_tensor& vc, int64_t stride_batch, const int32_t* seqlens,
                            const int32_t* idx, const int32_t* count, int tau_max, float softmax_scale,
-                           void* out, float* lse, void* ws, size_t ws_bytes, cudaStream_t st) {
+                           void* out, float* lse, void* ws, size_t ws_bytes, const int32_t* table,
+                           int table_stride, cudaStream_t st) {
   if (batch == 0) return SW_OK;
   const int nsplit = decode_num_splits(batch, kc.heads, tau_max, q.d);
   if (ws == nullptr || ws_bytes < decode_ws_bytes(batch, q.heads, q.d, nsplit))
@@ -322,10 +330,10 @@ int32_t launch_attn_decode(int batch, int block, const sw_tensor& q, const sw_te
                 decode_ws_bytes(batch, q.heads, q.d, nsplit));
   if (q.d == 128)
     return launch_decode_t<128>(batch, block, q, kc, vc, stride_batch, seqlens, idx, count, tau_max,
-                                softmax_scale, out, lse, ws, nsplit, st);
+                                softmax_scale, out, lse, ws, nsplit, table, table_stride, st);
   if (q.d == 64)
     return launch_decode_t<64>(batch, block, q, kc, vc, stride_batch, seqlens, idx, count, tau_max,
-                               softmax_scale, out, lse, ws, nsplit, st);
+                               softmax_scale, out, lse, ws, nsplit, table, table_stride, st);
   return fail(SW_ERR_UNSUPPORTED, "sw_sparse_attn_decode: head_dim %d", q.d);
 }
 

@@ -105,7 +105,8 @@ size_t decode_ws_bytes(int batch, int h_q, int d, int nsplit);
 int32_t launch_attn_decode(int batch, int block, const sw_tensor& q, const sw_tensor& kc,
                            const sw_tensor& vc, int64_t stride_batch, const int32_t* seqlens,
                            const int32_t* idx, const int32_t* count, int tau_max, float softmax_scale,
-                           void* out, float* lse, void* ws, size_t ws_bytes, cudaStream_t st);
+                           void* out, float* lse, void* ws, size_t ws_bytes, const int32_t* table,
+                           int table_stride, cudaStream_t st);
 
 }  // namespace sw
 

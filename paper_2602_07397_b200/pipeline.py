@@ -145,3 +145,11 @@ class DecodePipeline:
         sw.sw_sparse_attn_decode(self.batch, self.B, q, kcache, vcache, seqlens, self.idx, self.count,
                                  self.tau_max, self.softmax_scale, out, lse, self.attn_ws, stream)
         return out
+
+    def attend_paged(self, q, kpool, vpool, block_table, seqlens, out=None, lse=None, stream=None) -> torch.Tensor:
+        """Step 7 on a paged KV cache: pools [num_pages, B, h_kv, d], block_table [batch, max_blocks] int32."""
+        if out is None:
+            out = torch.empty(self.batch, self.h_q, self.d, dtype=torch.bfloat16, device=q.device)
+        sw.sw_sparse_attn_decode_paged(self.batch, self.B, q, kpool, vpool, block_table, seqlens, self.idx, self.count,
+                                       self.tau_max, self.softmax_scale, out, lse, self.attn_ws, stream)
+        return out

@@ -417,6 +417,56 @@ def test_sparse_attn_decode(sw, ts, h_q, h_kv, d, B, tau):
         assert err.max() <= ATT_MAX and err.mean() <= ATT_MEAN, (err.max(), err.mean())
 
 
+@pytest.mark.parametrize("ts,h_q,h_kv,d,B,tau", [
+    ((64 * 9 + 1, 64 * 9 + 32, 64 * 10), 32, 8, 128, 64, 5),
+    ((1000, 513), 16, 2, 128, 128, 4),
+])
+def test_sparse_attn_decode_paged(sw, ts, h_q, h_kv, d, B, tau):
+    """Paged KV cache: the logical blocks of every sequence are scattered over one pool of pages in a random
+    order (sequences interleaved, unused pages filled with NaN); the result must equal the oracle's on the
+    logically contiguous cache, and the contiguous call's bit for bit."""
+    rng = np.random.RandomState(4)
+    torch.manual_seed(4)
+    batch, tmax = len(ts), max(ts)
+    mb = O.num_blocks(tmax, B)
+    q = torch.randn(batch, h_q, d).bfloat16()
+    kc = torch.randn(batch, tmax, h_kv, d).bfloat16(); vc = torch.randn(batch, tmax, h_kv, d).bfloat16()
+    idx = np.full((batch, tau), -1, np.int32); cnt = np.zeros(batch, np.int32)
+    for s_, t in enumerate(ts):
+        bq = (t - 1) // B
+        sel = O.select_topk_row(rng.rand(bq + 1), bq, tau, O.DEFAULT_FLAGS)
+        idx[s_, :len(sel)] = sel; cnt[s_] = len(sel)
+    n_pages = batch * mb + 7
+    perm = rng.permutation(n_pages)
+    table = np.full((batch, mb), -1, np.int32)
+    kpool = torch.full((n_pages, B, h_kv, d), float("nan"), dtype=torch.bfloat16)
+    vpool = torch.full((n_pages, B, h_kv, d), float("nan"), dtype=torch.bfloat16)
+    nxt = 0
+    for s_, t in enumerate(ts):
+        for j in range(O.num_blocks(t, B)):
+            pg = int(perm[nxt]); nxt += 1
+            table[s_, j] = pg
+            m = min(B, t - j * B)
+            kpool[pg, :m] = kc[s_, j * B:j * B + m]; vpool[pg, :m] = vc[s_, j * B:j * B + m]
+    scale = 1 / math.sqrt(d)
+    ws = torch.empty(sw.sw_decode_workspace_bytes(batch, h_q, h_kv, d, tau), dtype=torch.uint8, device="cuda")
+    seql = dev(np.asarray(ts, np.int32))
+    out_p = torch.full((batch, h_q, d), float("nan"), dtype=torch.bfloat16, device="cuda")
+    out_c = torch.full((batch, h_q, d), float("nan"), dtype=torch.bfloat16, device="cuda")
+    sw.sw_sparse_attn_decode_paged(batch, B, q.cuda(), kpool.cuda(), vpool.cuda(), dev(table), seql, dev(idx), dev(cnt),
+                                   tau, scale, out_p, None, ws)
+    sw.sw_sparse_attn_decode(batch, B, q.cuda(), kc.cuda(), vc.cuda(), seql, dev(idx), dev(cnt), tau, scale, out_c,
+                             None, ws)
+    assert torch.equal(out_p, out_c)
+    got = out_p.float().cpu().numpy()
+    assert np.isfinite(got).all()
+    for s_, t in enumerate(ts):
+        ref = O.decode_attention(gen.to_numpy_f64(q[s_]), gen.to_numpy_f64(kc[s_, :t]), gen.to_numpy_f64(vc[s_, :t]),
+                                 idx[s_, :cnt[s_]], B, scale)
+        err = np.abs(got[s_] - ref)
+        assert err.max() <= ATT_MAX and err.mean() <= ATT_MEAN, (err.max(), err.mean())
+
+
 # ------------------------------------------------------------------------------ decode selection path
 @pytest.mark.parametrize("fused", [True, False])
 @pytest.mark.parametrize("t,tau", [(64 * 5 + 1, 4), (64 * 5 + 32, 4), (64 * 6, 4), (64 * 70 + 9, 12),

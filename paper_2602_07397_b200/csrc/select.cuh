@@ -4,8 +4,9 @@
 // Integer work only, hence bit-exact.  Shared by select.cu and decode_select.cu.
 //
 // One CTA of kThreads = 256 threads per row:
-//   * 4 radix passes of 8 bits on one shared histogram (match.any aggregation on the top byte, which
-//     falls into a handful of bins for rescaled scores), a 256-thread suffix scan picks the bin;
+//   * 4 radix passes of 8 bits on one shared histogram (plain shared-memory atomics; a warp whose lanes
+//     all hit the same bin sends one add), a 256-thread suffix scan picks the bin; rows of up to 2048
+//     candidates keep their keys in registers, so only the histogram touches memory;
 //   * one ordered compaction: every thread owns a contiguous index range, a block scan of the
 //     (certain, equal-to-threshold) counts gives each range its output offset.
 #pragma once
@@ -57,6 +58,19 @@ __device__ __forceinline__ RowJob make_job(int n_cand, int diag, bool force_last
 
 __device__ __forceinline__ bool is_forced(const RowJob& J, int j) { return j == J.f0 || j == J.f1; }
 
+// One histogram update per lane (bin 256 = none).  Shared-memory atomics of a warp to distinct bins run in
+// parallel and to a few bins fast enough (measured: faster than match.any aggregation, which costs one
+// round per distinct value); only the degenerate row whose keys all fall into one bin would serialise
+// 32 ways on every update, so a warp that agrees on its bin sends a single add.
+__device__ __forceinline__ void hist_add(Scratch& S, uint32_t bin, int lane) {
+  const uint32_t b0 = __shfl_sync(0xffffffffu, bin, 0);
+  if (__all_sync(0xffffffffu, bin == b0)) {
+    if (lane == 0 && b0 < 256u) atomicAdd(&S.hist[b0], 32u);
+  } else if (bin < 256u) {
+    atomicAdd(&S.hist[bin], 1u);
+  }
+}
+
 // After the 4 passes `thr` is the key of the need-th largest non-forced candidate and `n_gt` the
 // number of non-forced candidates with a strictly larger key.  All threads return the same values.
 template <typename Load>
@@ -77,14 +91,7 @@ __device__ void radix_threshold(Load load, const RowJob& J, Scratch& S, uint32_t
         const uint32_t k = order_key(load(j));
         if ((k & mask_hi) == prefix) bin = (k >> shift) & 0xffu;
       }
-      if (pass == 0) {
-        // the top byte (sign + 7 exponent bits) of rescaled scores falls into a handful of bins:
-        // aggregate equal bins in the warp (match.any costs one round per distinct value)
-        const uint32_t peers = __match_any_sync(0xffffffffu, bin);
-        if (bin < 256u && lane == __ffs(peers) - 1) atomicAdd(&S.hist[bin], (uint32_t)__popc(peers));
-      } else if (bin < 256u) {
-        atomicAdd(&S.hist[bin], 1u);              // lower bytes spread over the bins
-      }
+      hist_add(S, bin, lane);
     }
     __syncthreads();
     // thread b owns bin b: count, then an inclusive suffix sum over bins b..255
@@ -101,6 +108,63 @@ __device__ void radix_threshold(Load load, const RowJob& J, Scratch& S, uint32_t
     const uint32_t above = suf - cnt;                   // candidates in strictly higher bins
     if ((int)above < remaining && (int)suf >= remaining) { S.bcast[0] = (uint32_t)tid; S.bcast[1] = above; }
     __syncthreads();
+    SW_STAMP(11 + pass);
+    prefix |= S.bcast[0] << shift;
+    n_gt += (int)S.bcast[1];
+    remaining -= (int)S.bcast[1];
+  }
+  thr = prefix;
+  n_gt_out = n_gt;
+}
+
+// Register variant for rows of at most kRegKeys * kThreads candidates (b <= 2048): every thread keeps the
+// keys of its contiguous index range [lo, hi) in registers, so the four passes and the compaction touch
+// memory only for the histogram.  cmask: bit e set = index lo + e is a non-forced candidate.
+constexpr int kRegKeys = 8;
+__device__ __forceinline__ void radix_threshold_regs(const uint32_t (&key)[kRegKeys], uint32_t cmask, const RowJob& J,
+                                                     Scratch& S, uint32_t& thr, int& n_gt_out) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  uint32_t prefix = 0;
+  int remaining = J.need;
+  int n_gt = 0;
+  for (int pass = 0; pass < 4; ++pass) {
+    const int shift = 24 - 8 * pass;
+    S.hist[tid] = 0;
+    __syncthreads();
+    const uint32_t mask_hi = (pass == 0) ? 0u : (0xffffffffu << (shift + 8));
+    uint32_t bin[kRegKeys];
+    bool same = true;
+#pragma unroll
+    for (int e = 0; e < kRegKeys; ++e) {
+      const bool in = ((cmask >> e) & 1u) && (key[e] & mask_hi) == prefix;
+      bin[e] = in ? ((key[e] >> shift) & 0xffu) : 256u;
+      same = same && bin[e] == bin[0];
+    }
+    // plain shared-memory atomics (distinct bins of a warp run in parallel); only a warp whose 256 keys all
+    // fall into one bin -- the degenerate row of equal scores -- would serialise, so it sends a single add
+    const uint32_t b0 = __shfl_sync(0xffffffffu, bin[0], 0);
+    if (__all_sync(0xffffffffu, same && bin[0] == b0)) {
+      if (lane == 0 && b0 < 256u) atomicAdd(&S.hist[b0], 32u * kRegKeys);
+    } else {
+#pragma unroll
+      for (int e = 0; e < kRegKeys; ++e)
+        if (bin[e] < 256u) atomicAdd(&S.hist[bin[e]], 1u);
+    }
+    __syncthreads();
+    const uint32_t cnt = S.hist[tid];
+    uint32_t suf = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t v = __shfl_down_sync(0xffffffffu, suf, o);
+      if (lane + o < 32) suf += v;
+    }
+    if (lane == 0) S.warp_tot[warp] = suf;
+    __syncthreads();
+    for (int w = warp + 1; w < kWarps; ++w) suf += S.warp_tot[w];
+    const uint32_t above = suf - cnt;
+    if ((int)above < remaining && (int)suf >= remaining) { S.bcast[0] = (uint32_t)tid; S.bcast[1] = above; }
+    __syncthreads();
+    SW_STAMP(11 + pass);
     prefix |= S.bcast[0] << shift;
     n_gt += (int)S.bcast[1];
     remaining -= (int)S.bcast[1];
@@ -118,14 +182,66 @@ __device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out
   int n_gt = 0;
   const int n_free = J.n_cand - (J.f0 >= 0) - (J.f1 >= 0);
   const bool take_all = J.need >= n_free;
+  // ordered compaction: thread t owns indices [t*per, (t+1)*per)
+  const int per = (J.n_cand + kThreads - 1) / kThreads;
+  const int lo = min(tid * per, J.n_cand), hi = min(lo + per, J.n_cand);
   SW_STAMP(7);
+  if (per <= kRegKeys) {
+    uint32_t key[kRegKeys];
+    uint32_t cmask = 0, fmask = 0;
+#pragma unroll
+    for (int e = 0; e < kRegKeys; ++e) {
+      const int j = lo + e;
+      key[e] = 0;
+      if (j < hi) {
+        if (is_forced(J, j)) fmask |= 1u << e;
+        else { cmask |= 1u << e; key[e] = order_key(load(j)); }
+      }
+    }
+    if (!take_all && J.need > 0) radix_threshold_regs(key, cmask, J, S, thr, n_gt);
+    SW_STAMP(8);
+    const int eq_quota = J.need - n_gt;
+    uint32_t cert = fmask, eqm = 0;                   // bit e: index lo + e is certainly in / equals the threshold
+#pragma unroll
+    for (int e = 0; e < kRegKeys; ++e) {
+      if ((cmask >> e) & 1u) {
+        if (take_all) cert |= 1u << e;
+        else if (J.need > 0) {
+          if (key[e] > thr) cert |= 1u << e;
+          else if (key[e] == thr) eqm |= 1u << e;
+        }
+      }
+    }
+    unsigned long long v = ((unsigned long long)__popc(eqm) << 32) | (unsigned)__popc(cert), incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned long long u = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += u;
+    }
+    if (lane == 31) S.warp_scan[warp] = incl;
+    __syncthreads();
+    SW_STAMP(9);
+    unsigned long long base = 0;
+    for (int w = 0; w < warp; ++w) base += S.warp_scan[w];
+    const unsigned long long excl = base + incl - v;
+    int c_before = (int)(excl & 0xffffffffu), e_before = (int)(excl >> 32);
+#pragma unroll
+    for (int e = 0; e < kRegKeys; ++e) {
+      const bool c = (cert >> e) & 1u, q = (eqm >> e) & 1u;
+      const int pos = c_before + min(e_before, eq_quota);
+      if ((c || (q && e_before < eq_quota)) && pos < tau_max) out[pos] = lo + e;
+      c_before += c; e_before += q;
+    }
+    SW_STAMP(10);
+    for (int p = J.budget + tid; p < tau_max; p += kThreads) out[p] = -1;
+    if (tid == 0) *count_out = J.budget;
+    __syncthreads();                          // scratch may be reused by the caller
+    return;
+  }
   if (!take_all && J.need > 0) radix_threshold(load, J, S, thr, n_gt);
   SW_STAMP(8);
   const int eq_quota = J.need - n_gt;       // equal-key candidates to take, lowest index first
 
-  // ordered compaction: thread t owns indices [t*per, (t+1)*per)
-  const int per = (J.n_cand + kThreads - 1) / kThreads;
-  const int lo = min(tid * per, J.n_cand), hi = min(lo + per, J.n_cand);
   auto classify = [&](int j, bool& certain, bool& eq) {
     certain = false; eq = false;
     if (is_forced(J, j)) { certain = true; return; }

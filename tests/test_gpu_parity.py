@@ -266,6 +266,28 @@ def test_select_topk_negative_nan_inf(sw):
     assert np.array_equal(idx.cpu().numpy(), ref_idx) and np.array_equal(cnt.cpu().numpy(), ref_cnt)
 
 
+@pytest.mark.parametrize("b", [300, 2048, 2500])
+def test_select_topk_degenerate_and_clustered_rows(sw, b):
+    """Rows whose scores are all equal (ties go to the lower index), two-valued, or packed into one binade
+    (every radix pass sees heavy bin contention); b = 2500 takes the path that re-reads the row instead of
+    keeping it in registers.  Bit-exact against the oracle."""
+    rng = np.random.RandomState(b)
+    B, tau = 64, max(3, b // 5)
+    R = np.tril(rng.rand(b, b)).astype(np.float32)
+    R[b - 1, :] = 0.25                                        # all equal
+    R[b - 2, :] = np.where(rng.rand(b) < 0.5, 0.5, 0.25)      # two values
+    R[b - 3, :] = (1.0 + rng.rand(b) * 2.0 ** -12).astype(np.float32)   # one binade, 11 significant bits
+    R[b - 4, :] = 0.0
+    R = np.tril(R)
+    flags = O.DEFAULT_FLAGS
+    L = sw.make_layout([b * B], B)
+    idx = torch.empty(b, tau, dtype=torch.int32, device="cuda"); cnt = torch.empty(b, dtype=torch.int32, device="cuda")
+    sw.sw_select_topk(L, dev(R.ravel()), dev(np.asarray([tau], np.int32)), tau, flags, idx, cnt)
+    ref_idx, ref_cnt = O.select_topk(R.astype(np.float64), tau, flags)
+    assert np.array_equal(cnt.cpu().numpy(), ref_cnt)
+    assert np.array_equal(idx.cpu().numpy(), ref_idx)
+
+
 # ------------------------------------------------------------------------------ prefill attention
 def random_lists(rng, b, tau, causal=True):
     R = rng.rand(b, b)

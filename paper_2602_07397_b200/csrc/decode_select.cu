@@ -152,6 +152,26 @@ decode_select_kernel(const Params p) {
   if (tid < D) s_sign[tid] = p.signs ? (float)p.signs[tid] : 1.f;
   if (tid < p.r && tid < 128) s_cols[tid] = p.cols[tid];
 
+  // first batch of key-sketch rows of Steps 3-4 (up to 8 x 16 bytes per thread): requested here, ahead of
+  // the W stream in the memory queues; column b_q is patched from shared memory at use
+  const float* ksb = p.ks + (int64_t)seq * mb * p.r;
+  const int q4 = p.r >> 2;                            // float4s per sketch row
+  const bool vec_scores = (p.r & 3) == 0 && q4 <= 32 && (reinterpret_cast<uintptr_t>(ksb) & 15u) == 0;
+  constexpr int kU = 8;
+  float4 kv0[kU];
+  if (vec_scores) {
+    const int per_pass = kTile * q4, total = p.slots * per_pass;
+#pragma unroll
+    for (int u = 0; u < kU; ++u) {
+      const int i = u * kThreads + tid;
+      const int pass = i / per_pass, tile = tile_of(pass);
+      const int j = tile * kTile + (i - pass * per_pass) / q4;
+      kv0[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (i < total && tile < n_tiles && j < hi && j != bq)
+        kv0[u] = *reinterpret_cast<const float4*>(ksb + (int64_t)j * p.r + (tid & (q4 - 1)) * 4);
+    }
+  }
+
   // ---- W stream (Step 5 operand): rows [m_lo, b_q) of this CTA's column tiles, 64-row TMA boxes.
   // Nothing in it depends on this step's q/k, so the first kStages - 1 chunks are requested up front
   // and land while Steps 2-4 run.
@@ -221,16 +241,13 @@ decode_select_kernel(const Params p) {
 
   SW_STAMP(1);
   // ---- Steps 3-4: the new row of scores for this CTA's columns ------------------------------------
-  const float* ksb = p.ks + (int64_t)seq * mb * p.r;
   float lmax = -INFINITY;
-  const int q4 = p.r >> 2;                            // float4s per sketch row
-  if ((p.r & 3) == 0 && q4 <= 32 && (reinterpret_cast<uintptr_t>(ksb) & 15u) == 0) {
+  if (vec_scores) {
     // q4 adjacent lanes share one column: all of a tile's sketch rows are requested before the first
     // use (one memory latency per pass), partial dots meet in a fixed xor butterfly
     const int per_pass = kTile * q4, total = p.slots * per_pass;
     const int part = tid & (q4 - 1);
     const float4 qv = *reinterpret_cast<const float4*>(s_qt + part * 4);
-    constexpr int kU = 8;
     for (int i0 = 0; i0 < total; i0 += kU * kThreads) {
       float4 kv[kU];
       bool ok[kU];
@@ -240,8 +257,8 @@ decode_select_kernel(const Params p) {
         const int pass = i / per_pass, tile = tile_of(pass);
         const int j = tile * kTile + (i - pass * per_pass) / q4;
         ok[u] = i < total && tile < n_tiles && j < hi;
-        kv[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (ok[u]) {
+        kv[u] = (i0 == 0) ? kv0[u] : make_float4(0.f, 0.f, 0.f, 0.f);
+        if (ok[u] && (i0 != 0 || j == bq)) {
           const float* kp2 = (j == bq) ? s_kt : ksb + (int64_t)j * p.r;
           kv[u] = *reinterpret_cast<const float4*>(kp2 + part * 4);
         }

@@ -20,6 +20,10 @@
 // The O rescale is lazy: the running max is only raised (and O multiplied) when it grew by more than
 // 2^8, which keeps P within bf16/fp32 range and is exact after the final 1/l; a rescale first waits
 // for PV(k-1) of its tile (o_ready barrier).
+// A quarter of the exp2 runs on the FMA pipe (ex2_poly2), because MUFU ex2 at 16/clk/SM costs as many
+// cycles per chunk as the chunk's MMAs.  The Q tile is requested before the set-up barrier; the bf16
+// output leaves through the (then free) Q buffer and one TMA store per d-half and tile.
+// kTiles = 1 builds the variant with one 128-row tile per CTA and two CTAs per SM (measured slower).
 #include "common.cuh"
 #include "sm100.cuh"
 
@@ -84,12 +88,6 @@ __device__ __forceinline__ float ex2(float x) {
 // well under the bf16 rounding of P), n added into the exponent field.  Takes MUFU work off the
 // softmax warps: ex2.approx runs at 16/clk/SM, which at 64 exps per row and key chunk costs exactly
 // as many cycles as the chunk's two MMAs.
-#ifndef SW_EARLY_Q
-#define SW_EARLY_Q 1
-#endif
-#ifndef SW_TMA_EPI
-#define SW_TMA_EPI 1
-#endif
 #ifndef SW_POLY_MASK
 #define SW_POLY_MASK 0x88
 #endif
@@ -167,9 +165,9 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     mbar_init(BAR(kBarDone), kTiles);
     fence_barrier_init();
     // the Q tile does not depend on the chunk list: request it before the set-up barrier
-    if (SW_EARLY_Q) mbar_arrive_expect_tx(BAR(kBarQ), kQBytes);
-    if (SW_EARLY_Q) tma_load_3d(sQ, &map_q, BAR(kBarQ), 0, kvh * 4, q_tok0);
-    if (SW_EARLY_Q) tma_load_3d(sQ + kQBytes / 2, &map_q, BAR(kBarQ), 64, kvh * 4, q_tok0);
+    mbar_arrive_expect_tx(BAR(kBarQ), kQBytes);
+    tma_load_3d(sQ, &map_q, BAR(kBarQ), 0, kvh * 4, q_tok0);
+    tma_load_3d(sQ + kQBytes / 2, &map_q, BAR(kBarQ), 64, kvh * 4, q_tok0);
   } else if (warp == 2) {
     tmem_alloc<kTmemCols>(smem_u32((const void*)s_tmem));
   } else if (warp == 3) {
@@ -221,11 +219,6 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     // (the whole warp runs the loop; one elected lane issues the copies)
     if (n > 0) {
       const bool leader = elect_one();
-      if (!SW_EARLY_Q && leader) {
-        mbar_arrive_expect_tx(BAR(kBarQ), kQBytes);
-        tma_load_3d(sQ, &map_q, BAR(kBarQ), 0, kvh * 4, q_tok0);
-        tma_load_3d(sQ + kQBytes / 2, &map_q, BAR(kBarQ), 64, kvh * 4, q_tok0);
-      }
       int c = 0;
       auto push = [&](const CUtensorMap* m, int chunk) {
         const int st = c % kStages;
@@ -247,7 +240,7 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
         if (k + 2 < n) push(&map_k, k + 2);
       }
     } else {
-      if (SW_EARLY_Q) mbar_wait(BAR(kBarQ), 0);   // nothing to attend to: let the early Q load land before exit
+      mbar_wait(BAR(kBarQ), 0);          // nothing to attend to: let the early Q load land before exit
     }
   } else if (warp == 1 || (warp == 3 && kTiles == 2)) {
     // ===================== MMA issuers: warp 1 -> tile 0, warp 3 -> tile 1 =====================
@@ -438,7 +431,7 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     // MMA has completed) and one TMA store per d-half: row-per-thread global stores took ~6000 cycles
     // per CTA.  Ragged tiles and fp32 output keep the direct stores.
     const bool tile_full = q_tok0 + t * 32 + 31 <= q_last;
-    if (SW_TMA_EPI && n_iter > 0 && tile_full && !p.out_f32) {
+    if (n_iter > 0 && tile_full && !p.out_f32) {
       const int R = t * 128 + row;                         // row of the 256-row tile = 4 * token + head
       uint8_t* sO = base + (size_t)R * 128;
 #pragma unroll

@@ -10,6 +10,10 @@
 // distributed shared memory: (max, sum-exp) of the score row, the max-abs of r, and finally the r
 // values themselves, which every CTA pushes into rank 0's shared memory where the radix select
 // (select.cuh) runs.  Three cluster barriers in total.
+// The cached W streams through a cp.async ring (5 x 16 KB per CTA, two CTAs per SM), its first chunks
+// and the key-sketch rows of the score row are requested before anything else; the new row of W is
+// stored as row b_q of the cache (Alg. 2 Step 4).  DESIGN.md sec. 6.2 has the measurements behind
+// these choices.
 #include <cooperative_groups.h>
 
 #include <algorithm>

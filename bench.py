@@ -173,6 +173,8 @@ def main():
     ap.add_argument("--no-decode", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--prefill-kernel", default="auto", choices=["auto", "generic", "tcgen05"],
+                    help="kernel of sw_sparse_attn_prefill (all are CUDA kernels of libsw; default: the library's choice)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -193,6 +195,8 @@ def main():
         dist = dist_
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
+    pkg.sw_set_prefill_kernel({"auto": pkg.SW_PREFILL_AUTO, "generic": pkg.SW_PREFILL_GENERIC,
+                               "tcgen05": pkg.SW_PREFILL_TCGEN05}[args.prefill_kernel])
     peaks = load_peaks()
     sampler = ClockSampler(local_rank)
     res = prefill_bench(pkg, args, rank, world, dist, sampler, peaks)

@@ -494,13 +494,17 @@ def test_sparse_attn_decode_paged(sw, ts, h_q, h_kv, d, B, tau):
 @pytest.mark.parametrize("t,tau", [(64 * 5 + 1, 4), (64 * 5 + 32, 4), (64 * 6, 4), (64 * 70 + 9, 12),
                                    (64 * 300 + 1, 40), (64 * 301, 40),
                                    # max_blocks % 4 == 0: the cp.async ring of the fused kernel (else plain loads)
-                                   (64 * 7 + 3, 4), (64 * 71 + 9, 12), (64 * 299 + 5, 40), (64 * 300, 40)])
+                                   (64 * 7 + 3, 4), (64 * 71 + 9, 12), (64 * 299 + 5, 40), (64 * 300, 40),
+                                   # block size 128 (given as a negative t: |t| tokens)
+                                   (-(128 * 9 + 77), 4), (-(128 * 40), 9)])
 def test_decode_selection_matches_literal_alg2(sw, t, tau, fused):
     """GPU decode selection -- the fused sw_decode_select launch, or the five row-vector calls (sketch_append x2,
     block_scores_row, walk_update_row, select_topk_row) -- against the oracle's literal full-matrix Alg. 2,
     three layers, caches built by the GPU prefill path.  The larger t span several column tiles per cluster CTA."""
     cfg = gen.CONFIGS[2]
     B, r, s, d, h_q, h_kv = cfg.B, cfg.r, cfg.s, cfg.d, 8, 2
+    if t < 0:
+        t, B = -t, 128
     signs, cols, H = H_of(d, r, seed=3)
     flags = O.DEFAULT_FLAGS
     n_pre = t - 1

@@ -541,17 +541,18 @@ def test_decode_selection_matches_literal_alg2(sw, t, tau, fused):
         assert bq in got
 
 
+@pytest.mark.parametrize("nblk", [3, 299])
 @pytest.mark.parametrize("fused", [True, False])
-def test_decode_many_steps_across_a_block_boundary(sw, fused):
+def test_decode_many_steps_across_a_block_boundary(sw, fused, nblk):
     """Twelve consecutive decode steps, two layers, caches carried on the GPU with no maintenance other
     than the calls themselves: the running key-block mean / sketch and the cached-W row of the current
-    block (Alg. 2 Step 4) are updated in place, a block completes at t = 256 and a new one starts at 257.
+    block (Alg. 2 Step 4) are updated in place, a block completes at step 7 and a new one starts at step 8.
     Every step is compared with the oracle's literal Alg. 2 carrying its own caches."""
     cfg = gen.CONFIGS[2]
     B, r, s, d, h_q, h_kv, tau, layers = cfg.B, cfg.r, cfg.s, cfg.d, 8, 2, 3, 2
     signs, cols, H = H_of(d, r, seed=3)
     flags = O.DEFAULT_FLAGS
-    t0, steps = 64 * 3 + 58, 12
+    t0, steps = 64 * nblk + 58, 12                           # nblk = 299: 300 blocks, the cp.async W stream
     n_pre, t_end = t0 - 1, t0 + steps - 1
     b_pre, mb = O.num_blocks(n_pre, B), O.num_blocks(t_end, B)
     assert mb == b_pre + 1

@@ -285,6 +285,10 @@ SW_API int32_t sw_sparse_attn_prefill(const sw_layout* L, const sw_tensor* q, co
   a.idx = idx; a.count = count; a.tau_max = tau_max;
   a.softmax_scale = softmax_scale; a.flags = flags;
   a.out = out; a.out_dtype = q->dtype; a.lse = lse;
+  // kernel choice depends on shapes only: decide (and fail) before anything is launched
+  const bool fits = attn_prefill_sm100_supported(a);
+  if (g_prefill_kernel == SW_PREFILL_TCGEN05 && !fits)
+    return fail(SW_ERR_UNSUPPORTED, "sw_sparse_attn_prefill: SW_PREFILL_TCGEN05 needs d = 128 and h_q = 4 h_kv");
   if (q->dtype == SW_F32) {
     // P17: attention operands are rounded to bf16 by a cast pre-pass
     const size_t need = sw_workspace_bytes(SW_OP_ATTN_PREFILL, L, q->heads, k->heads, q->d, tau_max, SW_F32);
@@ -309,9 +313,6 @@ SW_API int32_t sw_sparse_attn_prefill(const sw_layout* L, const sw_tensor* q, co
     a.k_stride_tok = k->stride_tok; a.k_stride_head = k->stride_head;
     a.v_stride_tok = v->stride_tok; a.v_stride_head = v->stride_head;
   }
-  const bool fits = attn_prefill_sm100_supported(a);
-  if (g_prefill_kernel == SW_PREFILL_TCGEN05 && !fits)
-    return fail(SW_ERR_UNSUPPORTED, "sw_sparse_attn_prefill: SW_PREFILL_TCGEN05 needs d = 128 and h_q = 4 h_kv");
   if (fits && g_prefill_kernel != SW_PREFILL_GENERIC) {
     g_prefill_used = SW_PREFILL_TCGEN05;
     return launch_attn_prefill_sm100(a, st);

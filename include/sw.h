@@ -134,7 +134,11 @@ SW_API int32_t sw_block_scores(const sw_layout* L, const float* qs, const float*
 /* Decode form, Alg. 2 Steps 3-4: the new query row of W for block
  * b_q = (t-1)/B against key blocks 0..b_q of the same sequence.
  * q_tok: dev fp32 [batch, r].  ks: dev fp32 [batch, max_blocks, r].
- * w_row: dev fp32 [batch, max_blocks] (entries > b_q written as 0).  Needs !SW_POW_MATRIX. */
+ * w_row: dev fp32 [batch, max_blocks] (entries > b_q written as 0).  Needs !SW_POW_MATRIX and SW_CAUSAL
+ * (SW_ERR_UNSUPPORTED otherwise): all decode row-mode calls are defined under the block-causal mask only.
+ * Without it Alg. 2 Step 4(ii) rewrites column b_curr of the cached scores for every
+ * earlier query block, which changes the softmax of all those rows; the row-vector form does not carry that
+ * (under SW_CAUSAL the column is masked and the update is a no-op, P11). */
 SW_API int32_t sw_block_scores_row(int32_t batch, int32_t block, int32_t max_blocks, const float* q_tok,
                             const float* ks, const int32_t* seqlens, int32_t r, int32_t s,
                             uint32_t flags, float* w_row, sw_stream_t stream);
@@ -163,7 +167,8 @@ SW_API int32_t sw_walk_update(const sw_layout* L, const float* R_prev, const flo
  * (rows < b_q are read).  w_row, r_prev, r_out: dev fp32 [batch, max_blocks].
  * Cache update of Alg. 2 Step 4 ("update cached A^"): w_row is also stored as row b_q
  * of W_cache (zeros right of the diagonal), so that when the token completes block b_q the cache holds
- * that block's row for the following steps -- the row the literal algorithm leaves behind (P11). */
+ * that block's row for the following steps -- the row the literal algorithm leaves behind (P11).
+ * Needs SW_CAUSAL (see sw_block_scores_row). */
 SW_API int32_t sw_walk_update_row(int32_t batch, int32_t block, int32_t max_blocks, const float* r_prev,
                            float* W_cache, int64_t stride_seq, const float* w_row,
                            const int32_t* seqlens, uint32_t flags, float* r_out, sw_stream_t stream);
@@ -198,13 +203,19 @@ SW_API int32_t sw_select_topk_row(int32_t batch, int32_t block, int32_t max_bloc
  * and ks [batch, max_blocks, r] are updated in place for block b_curr, and the new row of W is stored
  * as row b_q of W_cache (as sw_walk_update_row does), so consecutive decode steps -- across block
  * boundaries too -- need no other cache maintenance than appending K/V.  r_prev (NULL = e_{b_q}),
- * r_out: dev fp32 [batch, max_blocks].  Needs !SW_POW_MATRIX. */
+ * r_out: dev fp32 [batch, max_blocks].  Needs !SW_POW_MATRIX and SW_CAUSAL (see sw_block_scores_row).
+ * ws: dev scratch of sw_decode_select_workspace_bytes(batch, max_blocks) bytes (SW_ERR_WORKSPACE if smaller):
+ * the raw score row, the partial sums of the W stream and one completion counter per sequence.  The
+ * counters (the first 512 + 4 * batch bytes) must be ZERO when the call starts -- zero the buffer once after
+ * allocating it -- and every completed call leaves them zero again, so one buffer serves all layers and
+ * steps issued on the same stream (calls that share a workspace must not overlap).  batch <= 1024. */
 SW_API int32_t sw_decode_select(int32_t batch, int32_t block, int32_t max_blocks, const sw_tensor* q,
                          const sw_tensor* k_new, const int32_t* seqlens, const int8_t* signs,
                          const int32_t* cols, int32_t r, float scale, int32_t s, uint32_t flags,
                          float* kbar, float* ks, float* W_cache, int64_t stride_seq,
                          const float* r_prev, float* r_out, const int32_t* tau, int32_t tau_max,
-                         int32_t* idx, int32_t* count, sw_stream_t stream);
+                         int32_t* idx, int32_t* count, void* ws, size_t ws_bytes, sw_stream_t stream);
+SW_API size_t sw_decode_select_workspace_bytes(int32_t batch, int32_t max_blocks);
 
 /* ---------------------------------------------------------------------------------------
  * (5) Block-sparse attention, prefill -- Alg. 1 Step 8; "zero outside selected

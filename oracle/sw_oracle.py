@@ -31,7 +31,10 @@ Pins (tests/test_oracle_pins.py; ``-m "not gpu"``):
                              (torch SDPA fp64); rows of P sum to 1 (PAPER.md:513);
                              order invariance; LSE merge of disjoint lists
   decode_* ................. decode output == row t of prefill attention given the
-                             same S; row-vector walk == row b_q of literal Alg. 2
+                             same S; row-vector walk == row b_q of literal Alg. 2;
+                             column update + running query mean of Alg. 2 Step 4
+                              == block scores rebuilt from scratch
+                             with CAUSAL off (explicit double loop)
   PARITY UNPINNED (no printed number / closed form in the paper): the choice of
   readings P4 (element-wise power), P5 (softmax on block scores), P7 (forced
   blocks inside the tau budget), P9 (row rescale), P11 (row b_q wins), P13

@@ -29,7 +29,7 @@ SW_OP_SKETCH, SW_OP_BLOCK_SCORES, SW_OP_WALK_UPDATE, SW_OP_SELECT_TOPK, SW_OP_AT
 EXPORTS = [
     "sw_sketch", "sw_sketch_append", "sw_block_scores", "sw_block_scores_row", "sw_walk_update",
     "sw_walk_update_row", "sw_select_topk", "sw_select_topk_row", "sw_decode_select", "sw_sparse_attn_prefill",
-    "sw_sparse_attn_decode", "sw_sparse_attn_decode_paged", "sw_workspace_bytes", "sw_decode_workspace_bytes", "sw_decode_num_splits",
+    "sw_sparse_attn_decode", "sw_sparse_attn_decode_paged", "sw_workspace_bytes", "sw_decode_workspace_bytes", "sw_decode_select_workspace_bytes", "sw_decode_num_splits",
     "sw_set_prefill_kernel", "sw_get_prefill_kernel_used", "sw_set_walk_kernel", "sw_get_walk_kernel_used",
     "sw_last_error", "sw_version", "sw_launch_count",
 ]
@@ -70,13 +70,14 @@ def _load() -> C.CDLL:
         "sw_select_topk": (i32, [LP, vp, vp, i32, u32, vp, vp, vp]),
         "sw_select_topk_row": (i32, [i32, i32, i32, vp, vp, vp, i32, u32, vp, vp, vp]),
         "sw_decode_select": (i32, [i32, i32, i32, TP, TP, vp, vp, vp, i32, f32, i32, u32, vp, vp, vp, i64, vp, vp,
-                                   vp, i32, vp, vp, vp]),
+                                   vp, i32, vp, vp, vp, sz, vp]),
         "sw_sparse_attn_prefill": (i32, [LP, TP, TP, TP, vp, vp, i32, f32, u32, vp, vp, vp, sz, vp]),
         "sw_sparse_attn_decode": (i32, [i32, i32, TP, TP, TP, i64, vp, vp, vp, i32, f32, vp, vp, vp, sz, vp]),
         "sw_sparse_attn_decode_paged": (i32, [i32, i32, TP, TP, TP, i64, vp, i32, vp, vp, vp, i32, f32, vp, vp, vp, sz,
                                               vp]),
         "sw_workspace_bytes": (sz, [i32, LP, i32, i32, i32, i32, i32]),
         "sw_decode_workspace_bytes": (sz, [i32, i32, i32, i32, i32]),
+        "sw_decode_select_workspace_bytes": (sz, [i32, i32]),
         "sw_decode_num_splits": (i32, [i32, i32, i32, i32]),
         "sw_set_prefill_kernel": (i32, [i32]),
         "sw_get_prefill_kernel_used": (i32, []),
@@ -245,12 +246,13 @@ def sw_select_topk_row(batch, block, max_blocks, r, seqlens, tau, tau_max, flags
 
 
 def sw_decode_select(batch, block, max_blocks, q, k_new, seqlens, signs, cols, r, scale, s, flags, kbar, ks,
-                     W_cache, stride_seq, r_prev, r_out, tau, tau_max, idx, count, stream=None) -> None:
+                     W_cache, stride_seq, r_prev, r_out, tau, tau_max, idx, count, ws, stream=None) -> None:
+    """ws: uint8 tensor of sw_decode_select_workspace_bytes(batch, max_blocks) bytes, zero-filled once by the caller."""
     qt, kt = _tensor(q), _tensor(k_new)
     _check(_lib.sw_decode_select(batch, block, max_blocks, C.byref(qt), C.byref(kt), _ptr(seqlens), _ptr(signs),
                                  _ptr(cols), r, scale, s, flags, _ptr(kbar), _ptr(ks), _ptr(W_cache), stride_seq,
                                  _ptr(r_prev), _ptr(r_out), _ptr(tau), tau_max, _ptr(idx), _ptr(count),
-                                 _stream(stream)))
+                                 _ptr(ws), 0 if ws is None else ws.numel() * ws.element_size(), _stream(stream)))
 
 
 def sw_workspace_bytes(op, L: Optional[Layout], h_q=0, h_kv=0, d=0, tau_max=0, dtype=SW_BF16) -> int:
@@ -260,6 +262,10 @@ def sw_workspace_bytes(op, L: Optional[Layout], h_q=0, h_kv=0, d=0, tau_max=0, d
 
 def sw_decode_workspace_bytes(batch, h_q, h_kv, d, tau_max) -> int:
     return _lib.sw_decode_workspace_bytes(batch, h_q, h_kv, d, tau_max)
+
+
+def sw_decode_select_workspace_bytes(batch, max_blocks) -> int:
+    return _lib.sw_decode_select_workspace_bytes(batch, max_blocks)
 
 
 def sw_decode_num_splits(batch, h_kv, d, tau_max) -> int:

@@ -25,11 +25,12 @@ int32_t fail(int32_t code, const char* fmt, ...) {
   return code;
 }
 
-static int g_sms = 0;
+static std::atomic<int> g_sms{0};
 
 int32_t check_arch() {
-  static int cached_dev = -1;
-  static int32_t cached = SW_ERR_ARCH;
+  // per-thread cache keyed by the current device: no shared mutable state between host threads
+  static thread_local int cached_dev = -1;
+  static thread_local int32_t cached = SW_ERR_ARCH;
   int dev = -1;
   if (cudaGetDevice(&dev) != cudaSuccess) {
     cudaGetLastError();
@@ -41,13 +42,13 @@ int32_t check_arch() {
   cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   cached_dev = dev;
-  g_sms = sms;
+  g_sms.store(sms, std::memory_order_relaxed);
   cached = (major == 10) ? SW_OK : SW_ERR_ARCH;
   if (cached != SW_OK) set_error("device %d is sm_%d%d; libsw is built for sm_100a only", dev, major, minor);
   return cached;
 }
 
-int num_sms() { return g_sms > 0 ? g_sms : 148; }
+int num_sms() { const int n = g_sms.load(std::memory_order_relaxed); return n > 0 ? n : 148; }
 
 static std::atomic<uint64_t> g_launches{0};
 void count_launch(int n) { g_launches.fetch_add((uint64_t)n, std::memory_order_relaxed); }
@@ -102,7 +103,7 @@ using namespace sw;
     if (_s != SW_OK) return _s;       \
   } while (0)
 
-static int32_t g_prefill_kernel = SW_PREFILL_AUTO;
+static std::atomic<int32_t> g_prefill_kernel{SW_PREFILL_AUTO};   // process-wide test / benchmark switch
 static thread_local int32_t g_prefill_used = 0;
 
 extern "C" {
@@ -154,6 +155,9 @@ SW_API int32_t sw_block_scores_row(int32_t batch, int32_t block, int32_t max_blo
   SW_REQUIRE(q_tok && ks && seqlens && w_row, SW_ERR_INVALID_ARG, "NULL argument");
   SW_REQUIRE(r >= 1 && r <= 128 && s >= 1, SW_ERR_INVALID_ARG, "r = %d / s = %d", r, s);
   SW_REQUIRE(!(flags & SW_POW_MATRIX), SW_ERR_UNSUPPORTED, "row mode needs the element-wise power (P4)");
+  SW_REQUIRE(flags & SW_CAUSAL, SW_ERR_UNSUPPORTED,
+             "decode row mode needs SW_CAUSAL: without the block-causal mask Alg. 2 Step 4(ii) (PAPER.md:822-824) "
+             "rewrites a column of the cached scores, which the row-vector form does not carry (P11)");
   SW_TRY(check_arch());
   return launch_block_scores_row(batch, block, max_blocks, q_tok, ks, seqlens, r, s, flags, w_row,
                                  (cudaStream_t)stream);
@@ -181,6 +185,9 @@ SW_API int32_t sw_walk_update_row(int32_t batch, int32_t block, int32_t max_bloc
   SW_REQUIRE(block == 64 || block == 128, SW_ERR_UNSUPPORTED, "block size %d not in {64,128}", block);
   SW_REQUIRE(W_cache && w_row && seqlens && r_out, SW_ERR_INVALID_ARG, "NULL argument");
   SW_REQUIRE(r_out != r_prev, SW_ERR_INVALID_ARG, "r_out must not alias r_prev");
+  SW_REQUIRE(flags & SW_CAUSAL, SW_ERR_UNSUPPORTED,
+             "decode row mode needs SW_CAUSAL: without the block-causal mask Alg. 2 Step 4(ii) (PAPER.md:822-824) "
+             "rewrites a column of the cached scores, which the row-vector form does not carry (P11)");
   SW_TRY(check_arch());
   return launch_walk_row(batch, block, max_blocks, r_prev, W_cache, stride_seq, w_row, seqlens, flags,
                          r_out, (cudaStream_t)stream);
@@ -212,7 +219,7 @@ SW_API int32_t sw_decode_select(int32_t batch, int32_t block, int32_t max_blocks
                          const int32_t* cols, int32_t r, float scale, int32_t s, uint32_t flags, float* kbar,
                          float* ks, float* W_cache, int64_t stride_seq, const float* r_prev,
                          float* r_out, const int32_t* tau, int32_t tau_max, int32_t* idx, int32_t* count,
-                         sw_stream_t stream) {
+                         void* ws, size_t ws_bytes, sw_stream_t stream) {
   SW_REQUIRE(batch >= 0 && max_blocks >= 1, SW_ERR_INVALID_ARG, "batch %d / max_blocks %d", batch, max_blocks);
   SW_REQUIRE(block == 64 || block == 128, SW_ERR_UNSUPPORTED, "block size %d not in {64,128}", block);
   SW_TRY(validate_tensor(q, "q"));
@@ -223,12 +230,15 @@ SW_API int32_t sw_decode_select(int32_t batch, int32_t block, int32_t max_blocks
   SW_REQUIRE(r_out != r_prev, SW_ERR_INVALID_ARG, "r_out must not alias r_prev");
   SW_REQUIRE(s >= 1 && tau_max >= 1, SW_ERR_INVALID_ARG, "s = %d / tau_max = %d", s, tau_max);
   SW_REQUIRE(!(flags & SW_POW_MATRIX), SW_ERR_UNSUPPORTED, "row mode needs the element-wise power (P4)");
+  SW_REQUIRE(flags & SW_CAUSAL, SW_ERR_UNSUPPORTED,
+             "decode row mode needs SW_CAUSAL: without the block-causal mask Alg. 2 Step 4(ii) (PAPER.md:822-824) "
+             "rewrites a column of the cached scores, which the row-vector form does not carry (P11)");
   SW_TRY(check_arch());
   DecodeSelectArgs a;
   a.batch = batch; a.block = block; a.max_blocks = max_blocks; a.q = *q; a.k = *k_new; a.seqlens = seqlens;
   a.signs = signs; a.cols = cols; a.r = r; a.scale = scale; a.s = s; a.flags = flags; a.kbar = kbar; a.ks = ks;
   a.W_cache = W_cache; a.stride_seq = stride_seq; a.r_prev = r_prev; a.r_out = r_out; a.tau = tau;
-  a.tau_max = tau_max; a.idx = idx; a.count = count;
+  a.tau_max = tau_max; a.idx = idx; a.count = count; a.ws = ws; a.ws_bytes = ws_bytes;
   return launch_decode_select(a, (cudaStream_t)stream);
 }
 
@@ -249,6 +259,10 @@ SW_API size_t sw_workspace_bytes(int32_t op, const sw_layout* L, int32_t h_q, in
     default:
       return 0;
   }
+}
+
+SW_API size_t sw_decode_select_workspace_bytes(int32_t batch, int32_t max_blocks) {
+  return (batch > 0 && max_blocks > 0) ? decode_select_ws_bytes(batch, max_blocks) : 0;
 }
 
 SW_API int32_t sw_decode_num_splits(int32_t batch, int32_t h_kv, int32_t d, int32_t tau_max) {
@@ -287,7 +301,8 @@ SW_API int32_t sw_sparse_attn_prefill(const sw_layout* L, const sw_tensor* q, co
   a.out = out; a.out_dtype = q->dtype; a.lse = lse;
   // kernel choice depends on shapes only: decide (and fail) before anything is launched
   const bool fits = attn_prefill_sm100_supported(a);
-  if (g_prefill_kernel == SW_PREFILL_TCGEN05 && !fits)
+  const int32_t want = g_prefill_kernel.load();
+  if (want == SW_PREFILL_TCGEN05 && !fits)
     return fail(SW_ERR_UNSUPPORTED, "sw_sparse_attn_prefill: SW_PREFILL_TCGEN05 needs d = 128 and h_q = 4 h_kv");
   if (q->dtype == SW_F32) {
     // P17: attention operands are rounded to bf16 by a cast pre-pass
@@ -313,7 +328,7 @@ SW_API int32_t sw_sparse_attn_prefill(const sw_layout* L, const sw_tensor* q, co
     a.k_stride_tok = k->stride_tok; a.k_stride_head = k->stride_head;
     a.v_stride_tok = v->stride_tok; a.v_stride_head = v->stride_head;
   }
-  if (fits && g_prefill_kernel != SW_PREFILL_GENERIC) {
+  if (fits && want != SW_PREFILL_GENERIC) {
     g_prefill_used = SW_PREFILL_TCGEN05;
     return launch_attn_prefill_sm100(a, st);
   }
@@ -324,9 +339,7 @@ SW_API int32_t sw_sparse_attn_prefill(const sw_layout* L, const sw_tensor* q, co
 SW_API int32_t sw_set_prefill_kernel(int32_t which) {
   SW_REQUIRE(which >= SW_PREFILL_AUTO && which <= SW_PREFILL_TCGEN05, SW_ERR_INVALID_ARG,
              "sw_set_prefill_kernel: unknown value %d", which);
-  const int32_t prev = g_prefill_kernel;
-  g_prefill_kernel = which;
-  return prev;
+  return g_prefill_kernel.exchange(which);
 }
 SW_API int32_t sw_get_prefill_kernel_used(void) { return g_prefill_used; }
 

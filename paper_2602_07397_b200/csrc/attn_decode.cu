@@ -5,47 +5,16 @@
 // cp.async ring, and the tiny QK^T / PV products run on mma.sync m16n8k16 with the GQA group in
 // the M dimension.  Partial (O, m, l) per split are merged by log-sum-exp in a second kernel.
 #include "common.cuh"
+#include "mma_sync.cuh"
 
 namespace {
+
+using namespace swmma;
 
 constexpr int kThreads = 128;       // 4 warps, each owns 16 keys of every 64-key tile
 constexpr int KT = 64;
 constexpr int kStages = 3;
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool valid) {
-  const int sz = valid ? 16 : 0;
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(sz));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() {
-  asm volatile("cp.async.wait_group %0;" ::"n"(N));
-}
-__device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], uint32_t addr) {
-  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
-}
-__device__ __forceinline__ void ldsm_x4_t(uint32_t (&r)[4], uint32_t addr) {
-  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
-}
-__device__ __forceinline__ void mma_bf16(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
-  asm volatile(
-      "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, "
-      "{%0,%1,%2,%3};"
-      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-      : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
-}
-__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
-  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
-  return *reinterpret_cast<uint32_t*>(&v);
-}
-template <int D>
-__device__ __forceinline__ uint32_t tile_off(int row, int chunk) {
-  return (uint32_t)(row * (D * 2) + (((chunk & ~7) | ((chunk ^ row) & 7)) << 4));
-}
 
 // Partial results: Opart [batch, h_q, nsplit, D] fp32 (unnormalised), ML [batch, h_q, nsplit, 2]
 template <int D>
@@ -300,11 +269,7 @@ static int32_t launch_decode_t(int batch, int block, const sw_tensor& q, const s
   const size_t ring = (size_t)kStages * 2 * KT * D * 2;
   const size_t merge = (size_t)(4 * 16 * D + 4 * 16 * 2) * sizeof(float);
   const size_t smem = ring > merge ? ring : merge;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(attn_decode_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr_set = true;
-  }
+  if (int32_t rc = allow_dynamic_smem(attn_decode_kernel<D>, smem, "sw_sparse_attn_decode smem attribute")) return rc;
   float* Opart = reinterpret_cast<float*>(ws);
   float* ML = Opart + (size_t)batch * q.heads * nsplit * D;
   dim3 grid(nsplit, kc.heads, batch);

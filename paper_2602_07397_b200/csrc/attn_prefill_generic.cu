@@ -6,49 +6,16 @@
 // CTA = 4 warps = one 64-token query tile of one q-head; it walks the selected key blocks of its
 // query block (idx/count from sw_select_topk) in 64-key tiles, double-buffered with cp.async.
 #include "common.cuh"
+#include "mma_sync.cuh"
 
 namespace {
+
+using namespace swmma;
 
 constexpr int kThreads = 128;
 constexpr int QT = 64;         // query rows per CTA
 constexpr int KT = 64;         // keys per tile
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool valid) {
-  const int sz = valid ? 16 : 0;     // src-size 0 => zero fill
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(sz));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() {
-  asm volatile("cp.async.wait_group %0;" ::"n"(N));
-}
-__device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], uint32_t addr) {
-  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
-}
-__device__ __forceinline__ void ldsm_x4_t(uint32_t (&r)[4], uint32_t addr) {
-  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
-}
-__device__ __forceinline__ void mma_bf16(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
-  asm volatile(
-      "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, "
-      "{%0,%1,%2,%3};"
-      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-      : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
-}
-__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
-  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
-  return *reinterpret_cast<uint32_t*>(&v);
-}
-
-// [rows][D] bf16 tile, 16-byte chunks XOR-swizzled by (row & 7): conflict-free ldmatrix
-template <int D>
-__device__ __forceinline__ uint32_t tile_off(int row, int chunk) {
-  return (uint32_t)(row * (D * 2) + (((chunk & ~7) | ((chunk ^ row) & 7)) << 4));
-}
 
 template <int D>
 __device__ __forceinline__ void load_tile(uint32_t s_base, const __nv_bfloat16* g, int64_t stride_tok,
@@ -304,11 +271,7 @@ static int32_t launch_generic_t(const AttnPrefillArgs& a, cudaStream_t st) {
   const int total_slots = L.total_blocks * TPB;
   const size_t smem = 5 * 64 * D * 2;
   auto kern = attn_prefill_generic_kernel<D, OutT>;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr_set = true;
-  }
+  if (int32_t rc = allow_dynamic_smem(kern, smem, "sw_sparse_attn_prefill(generic) smem attribute")) return rc;
   dim3 grid(total_slots, a.h_q);
   const float scale_log2 = a.softmax_scale * 1.4426950408889634f;
   count_launch();

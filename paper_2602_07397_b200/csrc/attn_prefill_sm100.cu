@@ -55,13 +55,6 @@ constexpr int kBarO = kBarP + 4;              // [t] PV(k) done             (tcg
 constexpr int kBarDone = kBarO + 2;           // all MMAs done
 constexpr int kNumBars = kBarDone + 1;
 
-#ifdef SW_TRACE
-__device__ long long g_trace[8][4096];          // [stream][event]
-#define TRACE(stream, slot) do { if (blockIdx.x == gridDim.x / 2 && blockIdx.y == 0 && lane == 0 && (slot) < 4096) g_trace[stream][slot] = clock64(); } while (0)
-#else
-#define TRACE(stream, slot) do {} while (0)
-#endif
-
 struct Params {
   const int32_t* cu_seqlens;
   const int32_t* cu_blocks;
@@ -154,7 +147,6 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   if (q_valid <= 0) return;
   const int q_last = q_tok0 + q_valid - 1;
 
-  if (warp == 4) TRACE(4, 0);
   // ---- one-time setup ------------------------------------------------------------------------
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&map_q); prefetch_tmap(&map_k); prefetch_tmap(&map_v); prefetch_tmap(&map_o);
@@ -209,7 +201,6 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   // operands in uniform registers instead of broadcasting them per instruction
   const uint32_t tm = __shfl_sync(0xffffffffu, *s_tmem, 0);
   const int n = __shfl_sync(0xffffffffu, *s_nchunks, 0);
-  if (warp == 4) TRACE(4, 1);
 
   if (warp < 4) {
   reg_dealloc<64>();
@@ -304,21 +295,17 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
         if (lane == 0) { w_bar = BAR(kBarP + t * 2 + buf); w_par = ph; }
         if (lane == 1) { w_bar = BAR(kBarFull + sv); w_par = pv; }
         if (lane == 2 && more) { w_bar = BAR(kBarFull + sk); w_par = pk; }
-        TRACE(2 + t, 4 * k + 0);
         {
-          uint32_t spins = 0;
+          SW_WATCHDOG_DECL;
           while (true) {
             const bool ok = (w_bar == 0) || mbar_try_wait(w_bar, w_par);
             if (__all_sync(0xffffffffu, ok)) break;
-            if (++spins > (1u << 26)) __trap();
+            SW_WATCHDOG_TICK;
           }
         }
         tc_fence_after();
-        TRACE(2 + t, 4 * k + 1);
         issue_pv(buf, sKV + sv * kTileBytes, k > 0, sv);
-        TRACE(2 + t, 4 * k + 2);
         if (more) issue_qk(buf, sKV + sk * kTileBytes, sk);
-        TRACE(2 + t, 4 * k + 3);
       }
       if (leader) mma_commit(BAR(kBarDone));
       __syncwarp();
@@ -340,15 +327,12 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
 
     for (int k = 0; k < n; ++k) {
       const int buf = k & 1, ph = (k >> 1) & 1;
-      if (w4 == 0) TRACE(t, 4 * k + 0);
       mbar_wait(BAR(kBarS + t * 2 + buf), ph);
       tc_fence_after();
-      if (w4 == 0) TRACE(t, 4 * k + 1);
       uint32_t s[64];
       tmem_ld32(t_s + buf * 64, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
       tmem_ld32(t_s + buf * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&s[32]));
       tmem_wait_ld();
-      if (w4 == 0) TRACE(t, 4 * k + 2);
       // masks: only chunks that touch the diagonal or the end of the sequence
       {
         const int k0 = s_list[k];
@@ -411,17 +395,16 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(BAR(kBarP + t * 2 + buf));
-      if (w4 == 0) TRACE(t, 4 * k + 3);
     }
 
     // epilogue: O / l -> bf16 -> global
-    if (warp == 4) TRACE(4, 2);
     if (n > 0) {
       mbar_wait(BAR(kBarDone), 0);
       tc_fence_after();
     }
-    if (warp == 4) TRACE(4, 3);
     const int n_iter = n;
+    // a row that never saw a visible key is 0 (ex2_poly2 returns 2^-125, not 0, for a masked column)
+    if (m_run == -INFINITY) l_run = 0.f;
     const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
     const bool valid = q_pos <= q_last;
     const int64_t o_off = ((int64_t)q_pos * p.h_q + head) * 128;
@@ -493,20 +476,12 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
           l_run > 0.f ? (m_run + log2f(l_run)) * 0.6931471805599453f : -INFINITY;
   }
 
-  if (warp == 4) TRACE(4, 4);
   tc_fence_before();
   __syncthreads();
-  if (warp == 4) TRACE(4, 5);
   if (warp == 2) tmem_dealloc<kTmemCols>(tm);
 }
 
 }  // namespace
-
-#ifdef SW_TRACE
-extern "C" __attribute__((visibility("default"))) int sw_debug_read_trace(long long* host, size_t bytes) {
-  return (int)cudaMemcpyFromSymbol(host, g_trace, bytes);
-}
-#endif
 
 namespace sw {
 
@@ -533,13 +508,8 @@ int32_t launch_attn_prefill_sm100(const AttnPrefillArgs& a, cudaStream_t st) {
   } else {
     mo = mq;                                   // unused by the fp32 epilogue
   }
-  static bool attr_set = false;
-  if (!attr_set) {
-    if (cudaFuncSetAttribute(attn_prefill_sm100_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes) !=
-        cudaSuccess)
-      return check_launch("sw_sparse_attn_prefill(sm100) smem attribute");
-    attr_set = true;
-  }
+  if (int32_t rc = allow_dynamic_smem(attn_prefill_sm100_kernel, kSmemBytes, "sw_sparse_attn_prefill(sm100) smem attribute"))
+    return rc;
   Params p;
   p.cu_seqlens = L.cu_seqlens; p.cu_blocks = L.cu_blocks; p.idx = a.idx; p.count = a.count;
   p.out = a.out; p.lse = a.lse; p.out_f32 = (a.out_dtype == SW_F32) ? 1 : 0;

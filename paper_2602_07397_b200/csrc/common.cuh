@@ -25,6 +25,16 @@ uint64_t launches();           // kernels launched by this library (sw_launch_co
     if (!(cond)) return sw::fail((code), __VA_ARGS__); \
   } while (0)
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device property of a kernel.  It is set before every
+// launch (a host-side table update, not a stream operation; legal during graph capture), so a process that
+// drives several GPUs needs no per-device bookkeeping.
+template <typename Kern>
+static inline int32_t allow_dynamic_smem(Kern kern, size_t bytes, const char* what) {
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess)
+    return check_launch(what);
+  return SW_OK;
+}
+
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 static inline bool is_pow2(int x) { return x > 0 && (x & (x - 1)) == 0; }
 static inline int cdiv(int a, int b) { return (a + b - 1) / b; }
@@ -78,8 +88,11 @@ struct DecodeSelectArgs {
   const int32_t* tau;
   int tau_max;
   int32_t *idx, *count;
+  void* ws;
+  size_t ws_bytes;
 };
 int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st);
+size_t decode_select_ws_bytes(int batch, int max_blocks);
 
 struct AttnPrefillArgs {
   const sw_layout* L;

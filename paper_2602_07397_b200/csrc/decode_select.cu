@@ -3,66 +3,38 @@
 // row-vector walk r^k = r^{k-1} W'^k (Step 5), the max-abs rescale (P9) and the
 // top-tau selection (Step 6).  HBM-bound on the cached W (4 b^2/2 bytes per sequence).
 //
-// One thread-block cluster per sequence.  The key-block columns are cut into 64-column tiles dealt
-// to the CTAs of the cluster boustrophedon-wise (tile p*C + rank on even passes, p*C + C-1-rank on
-// odd ones) so that the triangular W traffic is balanced; a CTA computes the scores, the walk and
-// the rescaled r for its own columns only.  Row-global quantities cross the cluster through
-// distributed shared memory: (max, sum-exp) of the score row, the max-abs of r, and finally the r
-// values themselves, which every CTA pushes into rank 0's shared memory where the radix select
-// (select.cuh) runs.  Three cluster barriers in total.
-// The cached W streams through a cp.async ring (5 x 16 KB per CTA, two CTAs per SM), its first chunks
-// and the key-sketch rows of the score row are requested before anything else; the new row of W is
-// stored as row b_q of the cache (Alg. 2 Step 4).  DESIGN.md sec. 6.2 has the measurements behind
-// these choices.
-#include <cooperative_groups.h>
-
+// The whole grid (two CTAs per SM) streams the cached W, whatever the batch: the work of the batch is
+// cut into items -- one 64-row x 64-column chunk of the block-causal part of W each (rows [64 c, b_q) of
+// column tile c), at least one item per column tile -- numbered over all sequences, and CTA i takes the
+// contiguous range [i T / G, (i+1) T / G) of the T items.  A CTA accumulates r_prev[m] W[m][j] over its
+// chunks of one column tile in registers and leaves one 64-float partial per (tile, CTA) in the workspace
+// (fixed slots, fixed summation order: deterministic).  The first item of every column tile also carries the
+// "score duty": q~_t (and, on the tile that holds b_q, the running key-block mean and its sketch) and the
+// raw scores of its 64 columns.  Nothing waits on another CTA: every CTA counts the items it has finished
+// per sequence with one atomic, and the CTA that completes a sequence runs that sequence's tail -- softmax
+// statistics of the score row, W_new = A^s, r = sum of partials + r_prev[b_q] W_new, rescale, radix select
+// (select.cuh) -- on a row of at most max_blocks floats in shared memory.  The counters live in the
+// caller's workspace and are left at zero by every completed call.
+// The cached W streams through a cp.async ring (5 x 16 KB per CTA), requested before the score duty runs;
+// the new row of W is stored as row b_q of the cache (Alg. 2 Step 4).  DESIGN.md sec. 6.2 has the
+// measurements behind these choices.
 #include <algorithm>
 
 #include "common.cuh"
-
-// Phase stamps for tuning (compiled in only with -DSW_PHASE_PROF; the product build has none).
-#ifdef SW_PHASE_PROF
-__device__ unsigned long long g_sw_prof[4096 * 16];
-extern "C" __attribute__((visibility("default"))) void* sw_debug_prof_ptr() {
-  void* p = nullptr;
-  cudaGetSymbolAddress(&p, g_sw_prof);
-  return p;
-}
-#define SW_STAMP(k)                                                                 \
-  do {                                                                              \
-    if (threadIdx.x == 0) {                                                         \
-      unsigned long long t_;                                                        \
-      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                        \
-      g_sw_prof[(blockIdx.x & 4095) * 16 + (k)] = t_;                               \
-    }                                                                               \
-  } while (0)
-#else
-#define SW_STAMP(k) do { } while (0)
-#endif
-
 #include "select.cuh"
 #include "sketch_common.cuh"
 #include "sm100.cuh"
-
-namespace cg = cooperative_groups;
 
 namespace {
 
 constexpr int kThreads = 256;
 constexpr int kTile = 64;            // columns per tile
 constexpr int kRowGroups = 16;       // row lanes of the vector-matrix product
-constexpr int kUnroll = 8;           // independent 16-byte loads in flight per thread
-constexpr int kMaxCluster = 16;
-// W stream: cp.async ring of kStages chunks of 64 rows x 64 columns fp32 (16 KB).  Measured on B200
-// (one CTA per SM streaming HBM): cp.async 16 KB x 8 stages 6.8 TB/s, 8 KB x 8 5.5 TB/s; a TMA ring
-// (cp.async.bulk[.tensor] + mbarrier) pays ~0.27 us per box whatever its size, so it needs >= 32 KB
-// boxes, and the 128-bit register loads used before held only 32 KB per SM in flight (1.7 TB/s).
-// 5 stages keep the CTA under ~105 KB of shared memory so that two CTAs fit on an SM: one GPC of the
-// B200 has fewer than 16 free SMs, and with one CTA per SM only 7 clusters of 16 were co-resident.
 constexpr int kChunkRows = 64;
 constexpr int kStages = 5;
 constexpr int kChunkBytes = kChunkRows * kTile * 4;
 constexpr int kPieces = kChunkBytes / 16 / kThreads;     // 16-byte cp.async pieces per thread per chunk
+constexpr int kMaxBatch = 1024;      // per-sequence item counts are scanned in shared memory
 
 struct Params {
   const void* q;  int64_t q_stride_seq, q_stride_head;  int h_q;
@@ -75,9 +47,37 @@ struct Params {
   const float* r_prev;  float* r_out;
   const int32_t* tau;  int tau_max;
   int32_t* idx;  int32_t* count;
-  int B, max_blocks, slots;
+  int batch, B, max_blocks;
   int use_async;                     // W streamed by cp.async (needs 16-byte aligned rows), else plain loads
+  // workspace
+  unsigned int* ws_cnt;              // [batch] items finished per sequence (zero between calls)
+  float* ws_scores;                  // [batch][mbp] raw scores of the new row
+  float* ws_part;                    // [batch][tiles_max][slots][64] partial walk sums
+  int mbp, tiles_max, slots;
 };
+
+// Item bookkeeping of one sequence.  b_q = 64 a + e; column tile c < a has rows [64 c, b_q): a - c + (e > 0)
+// chunks; tile a (the one that holds b_q) has (e > 0) chunks and always one item.  Without a walk
+// (r_prev = NULL) every tile is a single score-only item.
+struct SeqInfo {
+  int bq, a, eps;
+  __device__ __forceinline__ int chunks(int tile, bool walk) const { return walk ? (tile < a ? a - tile + eps : eps) : 0; }
+  __device__ __forceinline__ int items(int tile, bool walk) const { return max(1, chunks(tile, walk)); }
+  __device__ __forceinline__ int items_before(int tile, bool walk) const {        // tile <= a
+    return walk ? tile * a - tile * (tile - 1) / 2 + tile * eps : tile;
+  }
+  __device__ __forceinline__ int total(bool walk) const { return walk ? a * (a + 1) / 2 + a * eps + 1 : a + 1; }
+};
+__device__ __forceinline__ SeqInfo seq_info(const int32_t* seqlens, int seq, int B) {
+  SeqInfo s;
+  const int t = __ldg(seqlens + seq);
+  s.bq = (t - 1) / B;                                  // block of the new token = b_curr
+  s.a = s.bq / kTile;
+  s.eps = (s.bq % kTile) != 0;
+  return s;
+}
+// CTA that owns global item g when T items are dealt to G CTAs as [i T / G, (i+1) T / G)
+__device__ __forceinline__ int cta_of(long long g, int T, int G) { return (int)(((g + 1) * G - 1) / T); }
 
 __device__ __forceinline__ float block_max(float v, float* s_red) {
   v = swd::warp_max(v);
@@ -100,389 +100,391 @@ __device__ __forceinline__ float block_sum(float v, float* s_red) {
   return m;
 }
 
-template <typename T, int D>
-__global__ void __launch_bounds__(kThreads)
+template <typename TIn, int D>
+__global__ void __launch_bounds__(kThreads, 2)
 decode_select_kernel(const Params p) {
-  cg::cluster_group cluster = cg::this_cluster();
-  const int C = (int)cluster.num_blocks();
-  const int rk = (int)cluster.block_rank();
-  const int seq = blockIdx.x / C;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-
-  extern __shared__ __align__(128) uint8_t smem_raw[];
-  const int mbp = ((p.max_blocks + kTile - 1) / kTile) * kTile + kChunkRows;   // zero-padded r_prev
-  float* s_rprev = reinterpret_cast<float*>(smem_raw);                 // [mbp]
-  float* s_w = s_rprev + mbp;                                          // [slots][64]: S -> w -> r
-  float* s_part = s_w + p.slots * kTile;                               // [kRowGroups][64]
-  uint8_t* s_ring = reinterpret_cast<uint8_t*>(
-      (reinterpret_cast<uintptr_t>(s_part + kRowGroups * kTile) + 127) & ~(uintptr_t)127);   // [kStages][16 KB]
-  float* s_rfull = reinterpret_cast<float*>(s_ring);                   // [max_blocks] on rank 0, after the walk
-  __shared__ __align__(16) float s_vec[D], s_veck[D], s_qt[128], s_kt[128], s_sign[D];
-  __shared__ float s_hq[kThreads / D][D], s_hk[kThreads / D][D];
-  __shared__ int32_t s_cols[128];
-  __shared__ float s_red[kThreads / 32];
-  __shared__ float s_stat[2], s_amax[1];
-  __shared__ swsel::Scratch scratch;
-
-  const int t = __ldg(p.seqlens + seq);
-  const int bq = (t - 1) / p.B;                      // block of the new token = b_curr
-  const int nb = (t + p.B - 1) / p.B;
-  const int cnt_in_block = (t - 1) % p.B;            // tokens already in block b_curr
-  const bool causal = p.flags & SW_CAUSAL, soft = p.flags & SW_SCORE_SOFTMAX;
-  const int hi = causal ? bq + 1 : nb;               // columns that can be unmasked
-  const int n_tiles = (hi + kTile - 1) / kTile;
-  const int mb = p.max_blocks;
-  auto tile_of = [&](int pass) { return pass * C + ((pass & 1) ? C - 1 - rk : rk); };
-  // the CTA that owns column b_q also owns the key-side update of Step 2
-  const int bq_tile = bq / kTile, bq_pass = bq_tile / C;
-  const bool owns_bq = tile_of(bq_pass) == bq_tile;
-
-  // ---- operand loads of Steps 2-3, issued before anything waits: head values of q and k (heads dealt
-  // to kGroups thread groups), the old running mean, the SRHT signs and columns
-  constexpr int kGroups = kThreads / D, kHeadRegs = 16;
-  const int hx = tid % D, hx_g = tid / D;
-  const T* qp = reinterpret_cast<const T*>(p.q) + (int64_t)seq * p.q_stride_seq + hx;
-  const T* kp = reinterpret_cast<const T*>(p.k) + (int64_t)seq * p.k_stride_seq + hx;
-  float qreg[kHeadRegs], kreg[kHeadRegs];
-#pragma unroll
-  for (int u = 0; u < kHeadRegs; ++u) {
-    const int h = hx_g + u * kGroups;
-    qreg[u] = (h < p.h_q) ? (float)qp[(int64_t)h * p.q_stride_head] : 0.f;
-    kreg[u] = (owns_bq && h < p.h_kv) ? (float)kp[(int64_t)h * p.k_stride_head] : 0.f;
-  }
-  float kbar_old = 0.f;
-  if (owns_bq && cnt_in_block != 0 && tid >= 128 && tid < 128 + D)
-    kbar_old = p.kbar[((int64_t)seq * mb + bq) * D + (tid - 128)];
-  if (tid < D) s_sign[tid] = p.signs ? (float)p.signs[tid] : 1.f;
-  if (tid < p.r && tid < 128) s_cols[tid] = p.cols[tid];
-
-  // first batch of key-sketch rows of Steps 3-4 (up to 8 x 16 bytes per thread): requested here, ahead of
-  // the W stream in the memory queues; column b_q is patched from shared memory at use
-  const float* ksb = p.ks + (int64_t)seq * mb * p.r;
-  const int q4 = p.r >> 2;                            // float4s per sketch row
-  const bool vec_scores = (p.r & 3) == 0 && q4 <= 32 && (reinterpret_cast<uintptr_t>(ksb) & 15u) == 0;
-  constexpr int kU = 8;
-  float4 kv0[kU];
-  if (vec_scores) {
-    const int per_pass = kTile * q4, total = p.slots * per_pass;
-#pragma unroll
-    for (int u = 0; u < kU; ++u) {
-      const int i = u * kThreads + tid;
-      const int pass = i / per_pass, tile = tile_of(pass);
-      const int j = tile * kTile + (i - pass * per_pass) / q4;
-      kv0[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (i < total && tile < n_tiles && j < hi && j != bq)
-        kv0[u] = *reinterpret_cast<const float4*>(ksb + (int64_t)j * p.r + (tid & (q4 - 1)) * 4);
-    }
-  }
-
-  // ---- W stream (Step 5 operand): rows [m_lo, b_q) of this CTA's column tiles, 64-row TMA boxes.
-  // Nothing in it depends on this step's q/k, so the first kStages - 1 chunks are requested up front
-  // and land while Steps 2-4 run.
+  const int G = (int)gridDim.x;
   const bool walk = p.r_prev != nullptr;
   const bool async = walk && p.use_async;
-  auto chunks_of = [&](int pass) {
-    const int tile = tile_of(pass);
-    const int m_lo = causal ? tile * kTile : 0;
-    return (tile < n_tiles && bq > m_lo) ? (bq - m_lo + kChunkRows - 1) / kChunkRows : 0;
+  const bool soft = p.flags & SW_SCORE_SOFTMAX;
+  const int mb = p.max_blocks;
+
+  extern __shared__ __align__(128) uint8_t smem_raw[];
+  float* s_rprev = reinterpret_cast<float*>(smem_raw);                 // [mbp + 64] r_prev of the current sequence
+  float* s_part = s_rprev + p.mbp + kChunkRows;                        // [kRowGroups][64]
+  uint8_t* s_ring = reinterpret_cast<uint8_t*>(
+      (reinterpret_cast<uintptr_t>(s_part + kRowGroups * kTile) + 127) & ~(uintptr_t)127);   // [kStages][16 KB]
+  float* s_row = reinterpret_cast<float*>(s_ring);                     // [mbp] tail only (the ring is idle then)
+  __shared__ __align__(16) float s_vec[D], s_qt[128], s_kt[128], s_sign[D];
+  __shared__ float s_hx[kThreads / D][D];
+  __shared__ int32_t s_cols[128];
+  __shared__ float s_red[kThreads / 32];
+  __shared__ int s_pref[kMaxBatch + 1];                                // exclusive prefix of items per sequence
+  __shared__ int s_scan[kThreads / 32];
+  __shared__ int s_last;                                               // this CTA has at least one tail to run
+  __shared__ unsigned s_tailmask[kMaxBatch / 32];                      // sequences whose tail this CTA runs
+  __shared__ swsel::Scratch scratch;
+
+  // ---- item counts of all sequences: exclusive prefix in shared memory ------------------------------
+  {
+    constexpr int kPer = kMaxBatch / kThreads;
+    int v[kPer], sum = 0;
+#pragma unroll
+    for (int e = 0; e < kPer; ++e) {
+      const int sq = tid * kPer + e;
+      v[e] = (sq < p.batch) ? seq_info(p.seqlens, sq, p.B).total(walk) : 0;
+      sum += v[e];
+    }
+    int incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int u = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += u;
+    }
+    if (lane == 31) s_scan[warp] = incl;
+    if (tid < D) s_sign[tid] = p.signs ? (float)p.signs[tid] : 1.f;
+    if (tid < kMaxBatch / 32) s_tailmask[tid] = 0u;
+    if (tid == 0) s_last = 0;
+    if (tid < p.r && tid < 128) s_cols[tid] = p.cols[tid];
+    __syncthreads();
+    int base = 0;
+    for (int w = 0; w < warp; ++w) base += s_scan[w];
+    int run = base + incl - sum;
+#pragma unroll
+    for (int e = 0; e < kPer; ++e) {
+      const int sq = tid * kPer + e;
+      if (sq <= p.batch) s_pref[sq] = run;
+      run += v[e];
+    }
+    __syncthreads();
+  }
+  const int T = s_pref[p.batch];
+  const int g_begin = (int)((long long)blockIdx.x * T / G), g_end = (int)((long long)(blockIdx.x + 1) * T / G);
+  const int n_my = g_end - g_begin;
+  if (n_my == 0) return;
+
+  // ---- cursors over this CTA's items (thread-uniform) -------------------------------------------------
+  struct Cursor { int seq, tile, chunk; SeqInfo si; };
+  auto locate = [&](int g) {
+    Cursor c;
+    int lo = 0, hi = p.batch - 1;
+    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_pref[mid] <= g) lo = mid; else hi = mid - 1; }
+    c.seq = lo;
+    c.si = seq_info(p.seqlens, lo, p.B);
+    const int local = g - s_pref[lo];
+    int tl = 0, th = c.si.a;
+    while (tl < th) { const int mid = (tl + th + 1) >> 1; if (c.si.items_before(mid, walk) <= local) tl = mid; else th = mid - 1; }
+    c.tile = tl;
+    c.chunk = local - c.si.items_before(tl, walk);
+    return c;
   };
-  const float* Wseq = p.W + (int64_t)seq * p.w_stride_seq;
-  int pr_pass = 0, pr_chunk = 0, pr_issued = 0;       // producer cursor (same in every thread)
+  auto advance = [&](Cursor& c) {
+    if (++c.chunk >= c.si.items(c.tile, walk)) {
+      c.chunk = 0;
+      if (++c.tile > c.si.a) {
+        c.tile = 0;
+        if (++c.seq < p.batch) c.si = seq_info(p.seqlens, c.seq, p.B);
+      }
+    }
+  };
+  Cursor cc = locate(g_begin), pc = cc;
+
+  // ---- W stream: chunk = rows [64 tile + 64 chunk, +64) x columns [64 tile, +64) of the sequence's cached W
+  int p_left = n_my, issued = 0;
   auto issue_next = [&]() {                           // all threads: request the next chunk (or an empty group)
-    while (pr_pass < p.slots && pr_chunk >= chunks_of(pr_pass)) { ++pr_pass; pr_chunk = 0; }
-    if (pr_pass < p.slots) {
-      const int tile = tile_of(pr_pass);
-      const int m0 = (causal ? tile * kTile : 0) + pr_chunk * kChunkRows;
-      const uint32_t dst = sm100::smem_u32(s_ring + (size_t)(pr_issued % kStages) * kChunkBytes);
+    while (p_left > 0 && pc.si.chunks(pc.tile, walk) == 0) { advance(pc); --p_left; }
+    if (p_left > 0) {
+      const float* Wseq = p.W + (int64_t)pc.seq * p.w_stride_seq;
+      const int m0 = (pc.tile + pc.chunk) * kTile;
+      const uint32_t dst = sm100::smem_u32(s_ring + (size_t)(issued % kStages) * kChunkBytes);
 #pragma unroll
       for (int u = 0; u < kPieces; ++u) {
-        const int pc = u * kThreads + tid, rr = pc >> 4, c4 = tile * kTile + (pc & 15) * 4;
-        if (m0 + rr < bq && c4 < mb)                  // rows >= b_q / columns >= max_blocks are never read
-          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + pc * 16),
+        const int pcs = u * kThreads + tid, rr = pcs >> 4, c4 = pc.tile * kTile + (pcs & 15) * 4;
+        if (m0 + rr < pc.si.bq && c4 < mb)            // rows >= b_q / columns >= max_blocks are never read
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + pcs * 16),
                        "l"(Wseq + (int64_t)(m0 + rr) * mb + c4) : "memory");
       }
-      ++pr_issued; ++pr_chunk;
+      ++issued; advance(pc); --p_left;
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
   };
   if (async)
     for (int i = 0; i < kStages - 1; ++i) issue_next();
 
-  SW_STAMP(0);
-  // ---- Steps 2-3: head means, running key-block mean, sketches ----------------------------------
-  // (the q / k / signs / cols loads were issued before the W prologue: one memory latency for all)
-  {
-    float sq = 0.f, sk = 0.f;
+  // head mean of x[seq] (all heads) -> s_vec (fp32), by all threads
+  constexpr int kGroups = kThreads / D;
+  auto head_mean = [&](const void* base, int64_t stride_seq, int64_t stride_head, int heads, int seq) {
+    const int hx = tid % D, hg = tid / D;
+    const TIn* xp = reinterpret_cast<const TIn*>(base) + (int64_t)seq * stride_seq + hx;
+    constexpr int kRegs = 16;
+    float v[kRegs];
 #pragma unroll
-    for (int u = 0; u < kHeadRegs; ++u) { sq += qreg[u]; sk += kreg[u]; }
-    for (int h = hx_g + kHeadRegs * kGroups; h < p.h_q; h += kGroups) sq += (float)qp[(int64_t)h * p.q_stride_head];
-    if (owns_bq)
-      for (int h = hx_g + kHeadRegs * kGroups; h < p.h_kv; h += kGroups) sk += (float)kp[(int64_t)h * p.k_stride_head];
-    s_hq[hx_g][hx] = sq;
-    s_hk[hx_g][hx] = sk;
-  }
-  __syncthreads();
-  if (tid < D) {
-    float sq = 0.f;
+    for (int u = 0; u < kRegs; ++u) {
+      const int h = hg + u * kGroups;
+      v[u] = (h < heads) ? (float)xp[(int64_t)h * stride_head] : 0.f;
+    }
+    float sm = 0.f;
 #pragma unroll
-    for (int g = 0; g < kGroups; ++g) sq += s_hq[g][tid];
-    s_vec[tid] = sq / (float)p.h_q;
-  } else if (owns_bq && tid >= 128 && tid < 128 + D) {
-    const int x = tid - 128;
-    float sk = 0.f;
-#pragma unroll
-    for (int g = 0; g < kGroups; ++g) sk += s_hk[g][x];
-    const float avg = sk / (float)p.h_kv;
-    const float m = (cnt_in_block == 0) ? avg : ((float)cnt_in_block * kbar_old + avg) / (float)(cnt_in_block + 1);
-    p.kbar[((int64_t)seq * mb + bq) * D + x] = m;
-    s_veck[x] = m;
-  }
-  __syncthreads();
-  swsk::sketch_tail<D>(s_vec, s_sign, s_cols, p.r, p.scale, s_qt);      // q~_t
-  if (owns_bq)
-    swsk::sketch_tail<D>(s_veck, s_sign, s_cols, p.r, p.scale, s_kt, p.ks + ((int64_t)seq * mb + bq) * p.r, 4);
-  __syncthreads();
-
-  SW_STAMP(1);
-  // ---- Steps 3-4: the new row of scores for this CTA's columns ------------------------------------
-  float lmax = -INFINITY;
-  if (vec_scores) {
-    // q4 adjacent lanes share one column: all of a tile's sketch rows are requested before the first
-    // use (one memory latency per pass), partial dots meet in a fixed xor butterfly
-    const int per_pass = kTile * q4, total = p.slots * per_pass;
-    const int part = tid & (q4 - 1);
-    const float4 qv = *reinterpret_cast<const float4*>(s_qt + part * 4);
-    for (int i0 = 0; i0 < total; i0 += kU * kThreads) {
-      float4 kv[kU];
-      bool ok[kU];
-#pragma unroll
-      for (int u = 0; u < kU; ++u) {
-        const int i = i0 + u * kThreads + tid;
-        const int pass = i / per_pass, tile = tile_of(pass);
-        const int j = tile * kTile + (i - pass * per_pass) / q4;
-        ok[u] = i < total && tile < n_tiles && j < hi;
-        kv[u] = (i0 == 0) ? kv0[u] : make_float4(0.f, 0.f, 0.f, 0.f);
-        if (ok[u] && (i0 != 0 || j == bq)) {
-          const float* kp2 = (j == bq) ? s_kt : ksb + (int64_t)j * p.r;
-          kv[u] = *reinterpret_cast<const float4*>(kp2 + part * 4);
-        }
-      }
-#pragma unroll
-      for (int u = 0; u < kU; ++u) {
-        const int i = i0 + u * kThreads + tid;
-        if (i0 + u * kThreads >= total) break;                          // warp-uniform
-        float acc = fmaf(qv.w, kv[u].w, fmaf(qv.z, kv[u].z, fmaf(qv.y, kv[u].y, qv.x * kv[u].x)));
-        for (int o = q4 >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        const float sc = ok[u] ? acc * p.inv_sqrt_r : -INFINITY;
-        if (part == 0 && i < total) s_w[i / q4] = sc;                   // = s_w[pass * kTile + column]
-        lmax = fmaxf(lmax, sc);
-      }
-    }
-  } else {
-    for (int pass = 0; pass < p.slots; ++pass) {
-      const int tile = tile_of(pass);
-      for (int cj = warp; cj < kTile; cj += kThreads / 32) {
-        const int j = tile * kTile + cj;
-        float sc = -INFINITY;
-        if (tile < n_tiles && j < hi) {
-          const float* kp = (j == bq) ? s_kt : ksb + (int64_t)j * p.r;
-          float acc = 0.f;
-          for (int c = lane; c < p.r; c += 32) acc = fmaf(s_qt[c], kp[c], acc);
-          sc = swd::warp_sum(acc) * p.inv_sqrt_r;
-        }
-        if (lane == 0) s_w[pass * kTile + cj] = sc;
-        lmax = fmaxf(lmax, sc);
-      }
-    }
-  }
-  __syncthreads();
-  SW_STAMP(2);
-  if (soft) {
-    const float m_i = block_max(lmax, s_red);
-    float e = 0.f;
-    for (int i = tid; i < p.slots * kTile; i += kThreads) {
-      const float sc = s_w[i];
-      if (sc > -INFINITY) e += expf(sc - m_i);
-    }
-    const float l_i = block_sum(e, s_red);
-    if (tid == 0) { s_stat[0] = m_i; s_stat[1] = l_i; }
-    cluster.sync();
-    float m_r = -INFINITY, l_r = 0.f;
-    if (tid < C) {
-      const float* rs = cluster.map_shared_rank(s_stat, tid);
-      m_r = rs[0]; l_r = rs[1];
-    }
-    const float m = block_max(m_r, s_red);
-    const float l = block_sum((m_r > -INFINITY) ? l_r * expf(m_r - m) : 0.f, s_red);
-    const float inv_l = 1.f / l;
-    for (int i = tid; i < p.slots * kTile; i += kThreads) {
-      const float sc = s_w[i];
-      s_w[i] = (sc > -INFINITY) ? swd::powi(expf(sc - m) * inv_l, p.s) : 0.f;
-    }
-  } else {
-    cluster.sync();                                   // keep the barrier count uniform
-    for (int i = tid; i < p.slots * kTile; i += kThreads) {
-      const float sc = s_w[i];
-      s_w[i] = (sc > -INFINITY) ? swd::powi(sc, p.s) : 0.f;
-    }
-  }
-  __syncthreads();
-  // Alg. 2 Step 4 cache update: the new row becomes row b_q of the cached W, zeros right
-  // of the diagonal.  Row b_q is never read while b_q is the current block (the walk reads rows < b_q).
-  {
-    float* wrow = p.W + (int64_t)seq * p.w_stride_seq + (int64_t)bq * mb;
-    for (int i = tid; i < p.slots * kTile; i += kThreads) {
-      const int pass = i / kTile;
-      const int j = tile_of(pass) * kTile + (i - pass * kTile);
-      if (j < mb) wrow[j] = s_w[i];                    // masked columns hold 0 already
-    }
-  }
-
-  SW_STAMP(3);
-  // ---- Step 5: r_out[j] = sum_{m < b_q} r_prev[m] W[m][j] + r_prev[b_q] w[j] --------------------------
-  float lamax = 0.f;
-  if (p.r_prev != nullptr) {
-    const float* rp = p.r_prev + (int64_t)seq * mb;
-    for (int i = tid; i < mbp; i += kThreads) s_rprev[i] = (i <= bq) ? __ldg(rp + i) : 0.f;
+    for (int u = 0; u < kRegs; ++u) sm += v[u];
+    for (int h = hg + kRegs * kGroups; h < heads; h += kGroups) sm += (float)xp[(int64_t)h * stride_head];
+    s_hx[hg][hx] = sm;
     __syncthreads();
-    const float* Wm = p.W + (int64_t)seq * p.w_stride_seq;
-    const int cq = tid & 15, rg = tid >> 4;
-    const bool vec_ok = (mb & 3) == 0 && ((reinterpret_cast<uintptr_t>(Wm) & 15u) == 0);
-    int cons = 0;                                     // chunks consumed so far (cp.async path)
-    for (int pass = 0; pass < p.slots; ++pass) {
-      const int tile = tile_of(pass);
-      const int col0 = tile * kTile;
-      float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (async) {
-        const int m_lo = causal ? col0 : 0;
-        const int nch = chunks_of(pass);
-        for (int ch = 0; ch < nch; ++ch, ++cons) {
-          asm volatile("cp.async.wait_group %0;" ::"n"(kStages - 2) : "memory");   // chunk `cons` has landed
-          __syncthreads();                            // ... for every thread; chunk cons-1 is fully consumed
-          issue_next();                               // refill the stage chunk cons-1 occupied
-          const int m0 = m_lo + ch * kChunkRows;
-          const int rows = min(kChunkRows, bq - m0);  // rows >= b_q are not part of the product
-          const float* box = reinterpret_cast<const float*>(s_ring + (size_t)(cons % kStages) * kChunkBytes);
+    if (tid < D) {
+      float a = 0.f;
 #pragma unroll
-          for (int u = 0; u < kChunkRows / kRowGroups; ++u) {
-            const int rr = rg + u * kRowGroups;
-            if (rr < rows) {
-              const float4 v = *reinterpret_cast<const float4*>(box + rr * kTile + cq * 4);
-              const float a = s_rprev[m0 + rr];
-              acc.x = fmaf(a, v.x, acc.x);
-              acc.y = fmaf(a, v.y, acc.y);
-              acc.z = fmaf(a, v.z, acc.z);
-              acc.w = fmaf(a, v.w, acc.w);
+      for (int g = 0; g < kGroups; ++g) a += s_hx[g][tid];
+      s_vec[tid] = a / (float)heads;
+    }
+    __syncthreads();
+  };
+
+  const int q4 = p.r >> 2;                            // float4s per sketch row
+  int cur_seq = -1, qt_seq = -1, done_in_seq = 0, consumed = 0;
+  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  bool acc_live = false;
+  const int cq = tid & 15, rg = tid >> 4;
+
+  // tail of one sequence (this CTA finished its last item): Steps 4-6 on the whole row
+  auto run_tail = [&](int seq) {
+    const SeqInfo si = seq_info(p.seqlens, seq, p.B);
+    const int bq = si.bq, hi = bq + 1;
+    __threadfence();
+    const float* sc = p.ws_scores + (int64_t)seq * p.mbp;
+    float lmax = -INFINITY;
+    for (int j = tid; j < hi; j += kThreads) { const float v = __ldcg(sc + j); s_row[j] = v; lmax = fmaxf(lmax, v); }
+    float m = 0.f, inv_l = 1.f;
+    if (soft) {
+      m = block_max(lmax, s_red);
+      float e = 0.f;
+      for (int j = tid; j < hi; j += kThreads) e += expf(s_row[j] - m);
+      inv_l = 1.f / block_sum(e, s_red);
+    }
+    // W_new = A^s; Alg. 2 Step 4 cache update: the new row becomes row b_q of the cached W,
+    // zeros right of the diagonal.  Row b_q is never read while b_q is the current block.
+    float* wrow = p.W + (int64_t)seq * p.w_stride_seq + (int64_t)bq * mb;
+    const float rq = walk ? __ldg(p.r_prev + (int64_t)seq * mb + bq) : 1.f;
+    const int base_g = s_pref[seq];
+    float lamax = 0.f;
+    for (int j = tid; j < mb; j += kThreads) {
+      float w = 0.f, v = 0.f;
+      if (j < hi) {
+        const float sj = s_row[j];
+        w = swd::powi(soft ? expf(sj - m) * inv_l : sj, p.s);
+        // Step 5: r_out[j] = sum_{m < b_q} r_prev[m] W[m][j] + r_prev[b_q] w[j]; the partial sums in slot order
+        const int tile = j / kTile, nch = si.chunks(tile, walk);
+        if (nch > 0) {
+          const long long f0 = base_g + si.items_before(tile, walk);
+          const int i0 = cta_of(f0, T, G), i1 = cta_of(f0 + nch - 1, T, G);
+          const float* pp = p.ws_part + (((int64_t)seq * p.tiles_max + tile) * p.slots) * kTile + (j & (kTile - 1));
+          for (int sl = 0; sl <= i1 - i0; ++sl) v += __ldcg(pp + sl * kTile);
+        }
+        v = fmaf(rq, w, v);
+        s_row[j] = v;
+        lamax = fmaxf(lamax, fabsf(v));
+      }
+      wrow[j] = w;
+    }
+    const float amax = block_max(lamax, s_red);           // (its barriers also publish s_row)
+    const bool rescale = (p.flags & SW_ROWNORM) && amax > 0.f;
+    float* ro = p.r_out + (int64_t)seq * mb;
+    for (int j = tid; j < mb; j += kThreads) {
+      float v = 0.f;
+      if (j < hi) { v = rescale ? s_row[j] / amax : s_row[j]; s_row[j] = v; }
+      ro[j] = v;
+    }
+    __syncthreads();
+    // Step 6: S = TopK(r[0..b_q), tau - |forced|) U {b_q} (U {0})
+    const int tt = max(0, min(__ldg(p.tau + seq), p.tau_max));
+    swsel::RowJob J = swsel::make_job(hi, bq, true, p.flags & SW_FORCE_FIRST, tt);
+    const float* row = s_row;
+    swsel::select_row([row](int j) { return row[j]; }, J, p.idx + (int64_t)seq * p.tau_max, p.tau_max,
+                      p.count + seq, scratch);
+    if (tid == 0) p.ws_cnt[seq] = 0;                      // leave the counter ready for the next call
+    __syncthreads();
+  };
+
+  // this CTA has finished `done_in_seq` items of sequence `seq`: publish, and take the tail if it was the last
+  auto finish_seq = [&](int seq) {
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+      const unsigned total = (unsigned)(s_pref[seq + 1] - s_pref[seq]);
+      const unsigned old = atomicAdd(p.ws_cnt + seq, (unsigned)done_in_seq);
+      // the tail runs after this CTA's streaming work (its row buffer aliases the ring)
+      if (old + (unsigned)done_in_seq == total) { s_tailmask[seq >> 5] |= 1u << (seq & 31); s_last = 1; }
+    }
+    done_in_seq = 0;
+  };
+
+  for (int it = 0; it < n_my; ++it) {
+    const SeqInfo& si = cc.si;
+    const int seq = cc.seq, tile = cc.tile, bq = si.bq;
+    if (seq != cur_seq) {
+      if (cur_seq >= 0) finish_seq(cur_seq);
+      cur_seq = seq;
+      __syncthreads();
+      if (walk) {
+        const float* rp = p.r_prev + (int64_t)seq * mb;
+        for (int i = tid; i < p.mbp + kChunkRows; i += kThreads) s_rprev[i] = (i <= bq) ? __ldg(rp + i) : 0.f;
+      }
+    }
+    if (cc.chunk == 0) {
+      // ---- score duty of (seq, tile): Steps 2-4 for columns [64 tile, 64 tile + 64) ------------------------
+      if (qt_seq != seq) {
+        head_mean(p.q, p.q_stride_seq, p.q_stride_head, p.h_q, seq);
+        swsk::sketch_tail<D>(s_vec, s_sign, s_cols, p.r, p.scale, s_qt);       // q~_t
+        qt_seq = seq;
+        __syncthreads();
+      }
+      if (tile == si.a) {
+        // the tile that holds column b_q owns the key-side update of Step 2
+        const int cnt = (__ldg(p.seqlens + seq) - 1) % p.B;                    // tokens already in block b_curr
+        float kbar_old = 0.f;
+        float* kb = p.kbar + ((int64_t)seq * mb + bq) * D;
+        if (cnt != 0 && tid < D) kbar_old = kb[tid];
+        head_mean(p.k, p.k_stride_seq, p.k_stride_head, p.h_kv, seq);
+        if (tid < D) {
+          const float avg = s_vec[tid];
+          const float mn = (cnt == 0) ? avg : ((float)cnt * kbar_old + avg) / (float)(cnt + 1);
+          kb[tid] = mn;
+          s_vec[tid] = mn;
+        }
+        __syncthreads();
+        swsk::sketch_tail<D>(s_vec, s_sign, s_cols, p.r, p.scale, s_kt, p.ks + ((int64_t)seq * mb + bq) * p.r);
+        __syncthreads();
+      }
+      const float* ksb = p.ks + (int64_t)seq * mb * p.r;
+      float* sc = p.ws_scores + (int64_t)seq * p.mbp;
+      const int hi = bq + 1, col0 = tile * kTile;
+      const bool vec_scores = (p.r & 3) == 0 && q4 <= 32 && (reinterpret_cast<uintptr_t>(ksb) & 15u) == 0;
+      if (vec_scores) {
+        // q4 adjacent lanes share one column; all loads of the tile are issued before the first use
+        const int part = tid & (q4 - 1), per_pass = kThreads / q4;
+        const float4 qv = *reinterpret_cast<const float4*>(s_qt + part * 4);
+        constexpr int kU = 8;
+        for (int c0 = 0; c0 < kTile; c0 += kU * per_pass) {
+          float4 kv[kU];
+#pragma unroll
+          for (int u = 0; u < kU; ++u) {
+            const int cj = c0 + u * per_pass + tid / q4, j = col0 + cj;
+            kv[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (cj < kTile && j < hi) {
+              const float* kp2 = (j == bq) ? s_kt : ksb + (int64_t)j * p.r;
+              kv[u] = *reinterpret_cast<const float4*>(kp2 + part * 4);
             }
+          }
+#pragma unroll
+          for (int u = 0; u < kU; ++u) {
+            if (c0 + u * per_pass >= kTile) break;                              // warp-uniform
+            const int cj = c0 + u * per_pass + tid / q4, j = col0 + cj;
+            float a = fmaf(qv.w, kv[u].w, fmaf(qv.z, kv[u].z, fmaf(qv.y, kv[u].y, qv.x * kv[u].x)));
+            for (int o = q4 >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+            if (part == 0 && cj < kTile && j < hi) sc[j] = a * p.inv_sqrt_r;
           }
         }
-      } else
-      if (tile < n_tiles) {
-        const int m_lo = causal ? col0 : 0;           // W[m][j] = 0 for m < j
-        const int c4 = col0 + cq * 4;
-        if (vec_ok && col0 + kTile <= mb) {
-          int m = m_lo + rg;
-          for (; m + (kUnroll - 1) * kRowGroups < bq; m += kUnroll * kRowGroups) {
-            uint4 v[kUnroll];
-#pragma unroll
-            for (int u = 0; u < kUnroll; ++u)
-              v[u] = swd::ld_nc_v4(Wm + (int64_t)(m + u * kRowGroups) * mb + c4);
-#pragma unroll
-            for (int u = 0; u < kUnroll; ++u) {
-              const float a = s_rprev[m + u * kRowGroups];
-              acc.x = fmaf(a, __uint_as_float(v[u].x), acc.x);
-              acc.y = fmaf(a, __uint_as_float(v[u].y), acc.y);
-              acc.z = fmaf(a, __uint_as_float(v[u].z), acc.z);
-              acc.w = fmaf(a, __uint_as_float(v[u].w), acc.w);
-            }
-          }
-          for (; m < bq; m += kRowGroups) {
-            const uint4 v = swd::ld_nc_v4(Wm + (int64_t)m * mb + c4);
-            const float a = s_rprev[m];
-            acc.x = fmaf(a, __uint_as_float(v.x), acc.x);
-            acc.y = fmaf(a, __uint_as_float(v.y), acc.y);
-            acc.z = fmaf(a, __uint_as_float(v.z), acc.z);
-            acc.w = fmaf(a, __uint_as_float(v.w), acc.w);
-          }
-        } else {
-          for (int m = m_lo + rg; m < bq; m += kRowGroups) {
-            const float a = s_rprev[m];
-            const float* wr = Wm + (int64_t)m * mb;
-            if (c4 + 0 < mb) acc.x = fmaf(a, __ldg(wr + c4 + 0), acc.x);
-            if (c4 + 1 < mb) acc.y = fmaf(a, __ldg(wr + c4 + 1), acc.y);
-            if (c4 + 2 < mb) acc.z = fmaf(a, __ldg(wr + c4 + 2), acc.z);
-            if (c4 + 3 < mb) acc.w = fmaf(a, __ldg(wr + c4 + 3), acc.w);
+      } else {
+        for (int cj = warp; cj < kTile; cj += kThreads / 32) {
+          const int j = col0 + cj;
+          if (j < hi) {
+            const float* kp = (j == bq) ? s_kt : ksb + (int64_t)j * p.r;
+            float a = 0.f;
+            for (int c = lane; c < p.r; c += 32) a = fmaf(s_qt[c], kp[c], a);
+            a = swd::warp_sum(a);
+            if (lane == 0) sc[j] = a * p.inv_sqrt_r;
           }
         }
       }
+    }
+    const int nch = si.chunks(tile, walk);
+    if (nch > 0) {
+      // ---- Step 5, one chunk: acc[j] += sum_m r_prev[m] W[m][j] over rows [m0, m0 + 64) ---------------------
+      const int m0 = (tile + cc.chunk) * kTile;
+      const int rows = min(kChunkRows, bq - m0);
+      if (async) {
+        asm volatile("cp.async.wait_group %0;" ::"n"(kStages - 2) : "memory");   // chunk `consumed` has landed
+        __syncthreads();                              // ... for every thread; the previous chunk is fully consumed
+        issue_next();                                 // refill the stage the previous chunk occupied
+        const float* box = reinterpret_cast<const float*>(s_ring + (size_t)(consumed % kStages) * kChunkBytes);
+#pragma unroll
+        for (int u = 0; u < kChunkRows / kRowGroups; ++u) {
+          const int rr = rg + u * kRowGroups;
+          if (rr < rows) {
+            const float4 v = *reinterpret_cast<const float4*>(box + rr * kTile + cq * 4);
+            const float a = s_rprev[m0 + rr];
+            acc.x = fmaf(a, v.x, acc.x);
+            acc.y = fmaf(a, v.y, acc.y);
+            acc.z = fmaf(a, v.z, acc.z);
+            acc.w = fmaf(a, v.w, acc.w);
+          }
+        }
+        ++consumed;
+      } else {
+        __syncthreads();                              // s_rprev is complete
+        const float* Wm = p.W + (int64_t)seq * p.w_stride_seq;
+        const int c4 = tile * kTile + cq * 4;
+        for (int rr = rg; rr < rows; rr += kRowGroups) {
+          const float a = s_rprev[m0 + rr];
+          const float* wr = Wm + (int64_t)(m0 + rr) * mb;
+          if (c4 + 0 < mb) acc.x = fmaf(a, __ldg(wr + c4 + 0), acc.x);
+          if (c4 + 1 < mb) acc.y = fmaf(a, __ldg(wr + c4 + 1), acc.y);
+          if (c4 + 2 < mb) acc.z = fmaf(a, __ldg(wr + c4 + 2), acc.z);
+          if (c4 + 3 < mb) acc.w = fmaf(a, __ldg(wr + c4 + 3), acc.w);
+        }
+      }
+      acc_live = true;
+    }
+    ++done_in_seq;
+    const bool tile_ends = (it == n_my - 1) || (cc.chunk + 1 >= si.items(tile, walk));
+    if (tile_ends && acc_live) {
+      // one partial per (tile, CTA): slot = rank of this CTA among the CTAs that share the tile
       *reinterpret_cast<float4*>(s_part + rg * kTile + cq * 4) = acc;
       __syncthreads();
       if (tid < kTile) {
         float v = 0.f;
 #pragma unroll
         for (int g = 0; g < kRowGroups; ++g) v += s_part[g * kTile + tid];      // fixed order
-        const int j = col0 + tid;
-        v = (tile < n_tiles && j < hi) ? fmaf(s_rprev[bq], s_w[pass * kTile + tid], v) : 0.f;
-        s_w[pass * kTile + tid] = v;
-        lamax = fmaxf(lamax, fabsf(v));
+        const long long f0 = s_pref[seq] + si.items_before(tile, walk);
+        const int slot = (int)blockIdx.x - cta_of(f0, T, G);
+        p.ws_part[(((int64_t)seq * p.tiles_max + tile) * p.slots + slot) * kTile + tid] = v;
       }
       __syncthreads();
+      acc = make_float4(0.f, 0.f, 0.f, 0.f);
+      acc_live = false;
     }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-  } else {
-    // r^{-1} = e_{b_q}: the product is row b_q of W', i.e. the new row itself
-    for (int i = tid; i < p.slots * kTile; i += kThreads) lamax = fmaxf(lamax, fabsf(s_w[i]));
+    advance(cc);
   }
-
-  SW_STAMP(4);
-  // ---- P9 rescale, write r_out, gather the row on rank 0 ---------------------------------------------
-  const float amax_i = block_max(lamax, s_red);
-  if (tid == 0) s_amax[0] = amax_i;
-  cluster.sync();
-  float a_r = 0.f;
-  if (tid < C) a_r = *cluster.map_shared_rank(s_amax, tid);
-  const float amax = block_max(a_r, s_red);
-  const bool rescale = (p.flags & SW_ROWNORM) && amax > 0.f;
-  float* ro = p.r_out + (int64_t)seq * mb;
-  float* rfull0 = cluster.map_shared_rank(s_rfull, 0);
-  for (int i = tid; i < p.slots * kTile; i += kThreads) {
-    const int pass = i / kTile;
-    const int tile = tile_of(pass);
-    const int j = tile * kTile + (i - pass * kTile);
-    if (tile < n_tiles && j < mb) {
-      const float v = rescale ? s_w[i] / amax : s_w[i];
-      ro[j] = v;
-      if (j < hi) rfull0[j] = v;
-    }
-  }
-  for (int j = n_tiles * kTile + rk * kThreads + tid; j < mb; j += C * kThreads) ro[j] = 0.f;
-  cluster.sync();
-  SW_STAMP(5);
-
-  // ---- Step 6 on rank 0: S = TopK(r[0..b_q), tau - |forced|) U {b_q} (U {0}) ----------------------------
-  if (rk == 0) {
-    const int tt = max(0, min(__ldg(p.tau + seq), p.tau_max));
-    swsel::RowJob J = swsel::make_job(hi, bq, true, p.flags & SW_FORCE_FIRST, tt);
-    const float* row = s_rfull;
-    swsel::select_row([row](int j) { return row[j]; }, J, p.idx + (int64_t)seq * p.tau_max, p.tau_max,
-                      p.count + seq, scratch);
-  }
-  SW_STAMP(6);
+  const int seq_first = locate(g_begin).seq;
+  finish_seq(cur_seq);
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  __syncthreads();
+  if (s_last)
+    for (int sq = seq_first; sq <= cur_seq; ++sq)
+      if ((s_tailmask[sq >> 5] >> (sq & 31)) & 1u) run_tail(sq);
 }
 
 }  // namespace
 
 namespace sw {
 
-static int pick_cluster(int batch, int max_blocks) {
-  const int tiles = cdiv(max_blocks, kTile);
-  int c = kMaxCluster;
-  while (c > 1 && (c > tiles || (int64_t)batch * c > 2 * num_sms())) c >>= 1;
-  return c;
+static int ds_grid(int batch, int max_blocks) {
+  const int a = (max_blocks - 1) / kTile;
+  const long long items = (long long)batch * ((long long)a * (a + 1) / 2 + a + 1);
+  return (int)std::min<long long>(items, 2LL * num_sms());
+}
+
+size_t decode_select_ws_bytes(int batch, int max_blocks) {
+  const size_t tiles = (size_t)cdiv(max_blocks, kTile), mbp = tiles * kTile;
+  return 256 + (((size_t)batch * 4 + 255) & ~(size_t)255) + sizeof(float) * (size_t)batch * mbp +
+         sizeof(float) * (size_t)batch * tiles * tiles * kTile;
 }
 
 int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st) {
   if (a.batch == 0) return SW_OK;
+  if (a.batch > kMaxBatch) return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: batch %d > %d", a.batch, kMaxBatch);
+  const size_t need = decode_select_ws_bytes(a.batch, a.max_blocks);
+  if (a.ws == nullptr || a.ws_bytes < need)
+    return fail(SW_ERR_WORKSPACE, "sw_decode_select: workspace %zu < %zu bytes", a.ws_bytes, need);
   Params p;
   p.q = a.q.ptr; p.q_stride_seq = a.q.stride_tok; p.q_stride_head = a.q.stride_head; p.h_q = a.q.heads;
   p.k = a.k.ptr; p.k_stride_seq = a.k.stride_tok; p.k_stride_head = a.k.stride_head; p.h_kv = a.k.heads;
@@ -490,7 +492,14 @@ int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st) {
   p.inv_sqrt_r = 1.0f / sqrtf((float)a.r);
   p.s = a.s; p.flags = a.flags; p.kbar = a.kbar; p.ks = a.ks; p.W = a.W_cache; p.w_stride_seq = a.stride_seq;
   p.r_prev = a.r_prev; p.r_out = a.r_out; p.tau = a.tau; p.tau_max = a.tau_max; p.idx = a.idx; p.count = a.count;
-  p.B = a.block; p.max_blocks = a.max_blocks;
+  p.batch = a.batch; p.B = a.block; p.max_blocks = a.max_blocks;
+  p.tiles_max = cdiv(a.max_blocks, kTile); p.mbp = p.tiles_max * kTile; p.slots = p.tiles_max;
+  uint8_t* w = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(a.ws) + 255) & ~(uintptr_t)255);
+  p.ws_cnt = reinterpret_cast<unsigned int*>(w);
+  w += ((size_t)a.batch * 4 + 255) & ~(size_t)255;
+  p.ws_scores = reinterpret_cast<float*>(w);
+  w += sizeof(float) * (size_t)a.batch * p.mbp;
+  p.ws_part = reinterpret_cast<float*>(w);
 
   void (*kern)(const Params) = nullptr;
   const int d = a.q.d;
@@ -501,32 +510,14 @@ int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st) {
   else return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: dtype %d / d %d", a.q.dtype, d);
 
   // cp.async stream of the cached W needs 16-byte aligned row pieces; otherwise the plain-load path runs
-  p.use_async = a.r_prev != nullptr && a.W_cache != nullptr && aligned16(a.W_cache) && (a.max_blocks & 3) == 0 &&
-                (a.stride_seq & 3) == 0;
+  p.use_async = a.r_prev != nullptr && aligned16(a.W_cache) && (a.max_blocks & 3) == 0 && (a.stride_seq & 3) == 0;
 
-  int C = pick_cluster(a.batch, a.max_blocks);
-  for (;; C >>= 1) {
-    p.slots = cdiv(cdiv(a.max_blocks, kTile), C);
-    const size_t mbp = (size_t)cdiv(a.max_blocks, kTile) * kTile + kChunkRows;
-    const size_t ring = std::max(p.use_async ? (size_t)kStages * kChunkBytes : 0, sizeof(float) * (size_t)((a.max_blocks + 3) & ~3));
-    const size_t smem = sizeof(float) * (mbp + (size_t)p.slots * kTile + kRowGroups * kTile) + 128 + ring;
-    if (smem > 220 * 1024) return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: max_blocks %d too large", a.max_blocks);
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (C > 8) cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(a.batch * C);
-    cfg.blockDim = dim3(kThreads);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr; cfg.numAttrs = 1;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, p);
-    if (e == cudaSuccess) { count_launch(); break; }
-    cudaGetLastError();
-    if (C == 1) return fail(SW_ERR_CUDA, "sw_decode_select: %s", cudaGetErrorString(e));
-  }
+  const size_t ring = std::max((size_t)kStages * kChunkBytes, sizeof(float) * (size_t)p.mbp);
+  const size_t smem = sizeof(float) * ((size_t)p.mbp + kChunkRows + kRowGroups * kTile) + 128 + ring;
+  if (smem > 200 * 1024) return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: max_blocks %d too large", a.max_blocks);
+  if (int32_t rc = allow_dynamic_smem(kern, smem, "sw_decode_select smem attribute")) return rc;
+  count_launch();
+  kern<<<ds_grid(a.batch, a.max_blocks), kThreads, smem, st>>>(p);
   return check_launch("sw_decode_select");
 }
 

@@ -236,12 +236,8 @@ static size_t scores_smem_bytes() {
 int32_t launch_block_scores(const sw_layout& L, const float* qs, const float* ks, int r, int s,
                             uint32_t flags, float* W, float* A, cudaStream_t st) {
   if (L.total_blocks == 0) return SW_OK;
-  static bool attr_set = false;
   const size_t smem = scores_smem_bytes();
-  if (!attr_set) {
-    cudaFuncSetAttribute(score_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr_set = true;
-  }
+  if (int32_t rc = allow_dynamic_smem(score_tile_kernel, smem, "sw_block_scores smem attribute")) return rc;
   dim3 grid(cdiv(L.max_blocks, kCols), cdiv(L.max_blocks, kRows), L.batch);
   count_launch(2);
   score_tile_kernel<<<grid, kThreads, smem, st>>>(qs, ks, r, flags, L.cu_blocks, L.cu_sq, W, 1.0f / sqrtf((float)r));

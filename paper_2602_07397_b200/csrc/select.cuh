@@ -13,10 +13,6 @@
 
 #include <stdint.h>
 
-#ifndef SW_STAMP
-#define SW_STAMP(k) do { } while (0)
-#endif
-
 namespace swsel {
 
 constexpr int kThreads = 256;
@@ -108,7 +104,6 @@ __device__ void radix_threshold(Load load, const RowJob& J, Scratch& S, uint32_t
     const uint32_t above = suf - cnt;                   // candidates in strictly higher bins
     if ((int)above < remaining && (int)suf >= remaining) { S.bcast[0] = (uint32_t)tid; S.bcast[1] = above; }
     __syncthreads();
-    SW_STAMP(11 + pass);
     prefix |= S.bcast[0] << shift;
     n_gt += (int)S.bcast[1];
     remaining -= (int)S.bcast[1];
@@ -164,7 +159,6 @@ __device__ __forceinline__ void radix_threshold_regs(const uint32_t (&key)[kRegK
     const uint32_t above = suf - cnt;
     if ((int)above < remaining && (int)suf >= remaining) { S.bcast[0] = (uint32_t)tid; S.bcast[1] = above; }
     __syncthreads();
-    SW_STAMP(11 + pass);
     prefix |= S.bcast[0] << shift;
     n_gt += (int)S.bcast[1];
     remaining -= (int)S.bcast[1];
@@ -185,7 +179,6 @@ __device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out
   // ordered compaction: thread t owns indices [t*per, (t+1)*per)
   const int per = (J.n_cand + kThreads - 1) / kThreads;
   const int lo = min(tid * per, J.n_cand), hi = min(lo + per, J.n_cand);
-  SW_STAMP(7);
   if (per <= kRegKeys) {
     uint32_t key[kRegKeys];
     uint32_t cmask = 0, fmask = 0;
@@ -199,7 +192,6 @@ __device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out
       }
     }
     if (!take_all && J.need > 0) radix_threshold_regs(key, cmask, J, S, thr, n_gt);
-    SW_STAMP(8);
     const int eq_quota = J.need - n_gt;
     uint32_t cert = fmask, eqm = 0;                   // bit e: index lo + e is certainly in / equals the threshold
 #pragma unroll
@@ -220,7 +212,6 @@ __device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out
     }
     if (lane == 31) S.warp_scan[warp] = incl;
     __syncthreads();
-    SW_STAMP(9);
     unsigned long long base = 0;
     for (int w = 0; w < warp; ++w) base += S.warp_scan[w];
     const unsigned long long excl = base + incl - v;
@@ -232,14 +223,12 @@ __device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out
       if ((c || (q && e_before < eq_quota)) && pos < tau_max) out[pos] = lo + e;
       c_before += c; e_before += q;
     }
-    SW_STAMP(10);
     for (int p = J.budget + tid; p < tau_max; p += kThreads) out[p] = -1;
     if (tid == 0) *count_out = J.budget;
     __syncthreads();                          // scratch may be reused by the caller
     return;
   }
   if (!take_all && J.need > 0) radix_threshold(load, J, S, thr, n_gt);
-  SW_STAMP(8);
   const int eq_quota = J.need - n_gt;       // equal-key candidates to take, lowest index first
 
   auto classify = [&](int j, bool& certain, bool& eq) {
@@ -266,7 +255,6 @@ __device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out
   }
   if (lane == 31) S.warp_scan[warp] = incl;
   __syncthreads();
-  SW_STAMP(9);
   unsigned long long base = 0;
   for (int w = 0; w < warp; ++w) base += S.warp_scan[w];
   const unsigned long long excl = base + incl - v;
@@ -278,7 +266,6 @@ __device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out
     if ((c || (e && e_before < eq_quota)) && pos < tau_max) out[pos] = j;
     c_before += c; e_before += e;
   }
-  SW_STAMP(10);
   for (int p = J.budget + tid; p < tau_max; p += kThreads) out[p] = -1;
   if (tid == 0) *count_out = J.budget;
   __syncthreads();                            // scratch may be reused by the caller

@@ -44,13 +44,19 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
       : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
   return ok != 0;
 }
-// Bounded wait: a protocol bug traps (the launch fails with an error) instead of hanging the GPU.
+// Waits spin on try_wait.  With -DSW_DEBUG_WATCHDOG a wait that exceeds 2^26 polls traps (a protocol bug then
+// fails the launch instead of hanging the GPU); the product build has no such bound, so a legitimately slow
+// wait (compute-sanitizer, a debugger, time-sliced sharing) cannot kill the context.
+#ifdef SW_DEBUG_WATCHDOG
+#define SW_WATCHDOG_DECL uint32_t sw_spins_ = 0
+#define SW_WATCHDOG_TICK do { if (++sw_spins_ > (1u << 26)) __trap(); } while (0)
+#else
+#define SW_WATCHDOG_DECL do { } while (0)
+#define SW_WATCHDOG_TICK do { } while (0)
+#endif
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  if (mbar_try_wait(bar, parity)) return;
-  uint32_t spins = 0;
-  while (!mbar_try_wait(bar, parity)) {
-    if (++spins > (1u << 26)) __trap();
-  }
+  SW_WATCHDOG_DECL;
+  while (!mbar_try_wait(bar, parity)) SW_WATCHDOG_TICK;
 }
 
 // ---- TMA ---------------------------------------------------------------------------------------

@@ -271,12 +271,7 @@ int32_t launch_walk_tc(int b, const float* A, const float* Bm, float* dst, float
   const bool ok = make_map_f32(&mrh, Rhi, b, b, BM, false) && make_map_f32(&mrl, Rlo, b, b, BM, false) &&
                   make_map_f32(&mwh, Whi, b, b, BK, true) && make_map_f32(&mwl, Wlo, b, b, BK, true);
   if (!ok) return fail(SW_ERR_CUDA, "sw_walk_update: cuTensorMapEncodeTiled failed");
-  static bool attr_set = false;
-  if (!attr_set) {
-    if (cudaFuncSetAttribute(walk_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes) != cudaSuccess)
-      return check_launch("sw_walk_update(tcgen05) smem attribute");
-    attr_set = true;
-  }
+  if (int32_t rc = allow_dynamic_smem(walk_tc_kernel, kSmemBytes, "sw_walk_update(tcgen05) smem attribute")) return rc;
   Params p;
   p.out = dst; p.b = b; p.nt = cdiv(b, BM); p.causal = causal;
   p.n_work = causal ? p.nt * (p.nt + 1) / 2 : p.nt * p.nt;

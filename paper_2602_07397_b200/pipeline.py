@@ -109,6 +109,9 @@ class DecodePipeline:
         self.count = torch.empty(batch, dtype=torch.int32, device=device)
         nb = sw.sw_decode_workspace_bytes(batch, h_q, h_kv, d, self.tau_max)
         self.attn_ws = torch.empty(max(nb, 16), dtype=torch.uint8, device=device)
+        # sw_decode_select scratch: zero-filled once (its completion counters return to zero after every call)
+        self.select_ws = torch.zeros(sw.sw_decode_select_workspace_bytes(batch, max_blocks), dtype=torch.uint8,
+                                     device=device)
 
     def reset(self) -> None:
         self.cur = -1
@@ -123,7 +126,7 @@ class DecodePipeline:
             r_prev = None if self.cur < 0 else self.rvec[self.cur]
             sw.sw_decode_select(b, B, mb, q, k_new, seqlens, self.signs, self.cols, self.r, self.sketch_scale,
                                 self.s, self.flags, kbar, ks, W_cache, W_cache.stride(0), r_prev, self.rvec[nxt],
-                                self.tau, self.tau_max, self.idx, self.count, stream)
+                                self.tau, self.tau_max, self.idx, self.count, self.select_ws, stream)
             self.cur = nxt
             return
         sw.sw_sketch_append(b, B, mb, k_new, seqlens, self.signs, self.cols, self.r, self.sketch_scale,

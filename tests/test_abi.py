@@ -66,6 +66,19 @@ def test_validation_happens_before_any_device_work(pkg):
     assert lib.sw_sketch(C.byref(lay), C.byref(t), None, 16, 64, 0.125, 16, None, None) == pkg.SW_ERR_INVALID_ARG
 
 
+def test_decode_row_mode_rejects_non_causal(pkg):
+    """Alg. 2 Step 4(ii) is not carried by the row-vector form: without SW_CAUSAL the three
+    decode calls that depend on it return SW_ERR_UNSUPPORTED (before looking at the device)."""
+    lib = pkg.binding._lib
+    nc = pkg.SW_DEFAULT_FLAGS & ~pkg.SW_CAUSAL
+    assert lib.sw_block_scores_row(1, 64, 4, 16, 16, 16, 64, 2, nc, 16, None) == pkg.SW_ERR_UNSUPPORTED
+    assert b"SW_CAUSAL" in lib.sw_last_error()
+    assert lib.sw_walk_update_row(1, 64, 4, 16, 32, 16, 16, 16, nc, 48, None) == pkg.SW_ERR_UNSUPPORTED
+    t = pkg.binding._Tensor(16, pkg.SW_BF16, 8, 128, 1024, 128)
+    assert lib.sw_decode_select(1, 64, 4, C.byref(t), C.byref(t), 16, None, 16, 64, 0.125, 2, nc, 16, 16, 16, 16, None,
+                                16, 16, 2, 16, 16, 16, 4096, None) == pkg.SW_ERR_UNSUPPORTED
+
+
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU behaviour")
 def test_no_cpu_fallback_without_gpu(pkg):
     """Valid arguments but no device: the call must fail loudly (SW_ERR_ARCH), never compute on the host."""

@@ -489,31 +489,91 @@ def test_sparse_attn_decode_paged(sw, ts, h_q, h_kv, d, B, tau):
         assert err.max() <= ATT_MAX and err.mean() <= ATT_MEAN, (err.max(), err.mean())
 
 
+# ------------------------------------------------------------------------------ paper default s = 8, heavy tails
+def heavy_tailed_sketches(seed, b, r, sigma=4.0, sink=6.0):
+    """Sketch rows whose block-score rows are heavy-tailed: S ~ sigma N(0, 1) (spread of ~6 sigma >= 12 over a
+    row, PAPER.md:117 Assumption 2.3) plus a sink column 0.  fp32."""
+    rng = np.random.RandomState(seed)
+    a = math.sqrt(sigma)
+    qs = (rng.randn(b, r) * a).astype(np.float32)
+    ks = (rng.randn(b, r) * a).astype(np.float32)
+    qs[:, 0] = math.sqrt(sink) * r ** 0.25
+    ks[:, 0] = 0.0
+    ks[0, 0] = math.sqrt(sink) * r ** 0.25
+    return qs, ks
+
+
+@pytest.mark.parametrize("b", [128, 512, 1024])
+@pytest.mark.parametrize("flags", [O.DEFAULT_FLAGS, O.DEFAULT_FLAGS | O.POW_MATRIX])
+def test_selection_chain_paper_default_s8_heavy_tails(sw, b, flags):
+    """Block scores -> walk -> top-tau at the paper's s = 8 on heavy-tailed score rows, three layers
+    with R carried, against the fp64 oracle.  In fp32 W = A^8 leaves the normal range for A < ~2e-5 (reading
+    P20 in DESIGN.md): such entries are <= 1e-37 of the row maximum, far inside the 1e-3 value tolerance, and
+    the candidates they decide between are near-ties in north_star's sense (within 1e-3 of the row max of each
+    other), which is what the set comparison allows."""
+    r, B, s, layers = 64, 64, 8, 3
+    if flags & O.POW_MATRIX:
+        s = 3
+    tau = O.tau_from_density(0.10, b)
+    L = sw.make_layout([b * B], B)
+    ws = torch.empty(sw.sw_workspace_bytes(sw.SW_OP_WALK_UPDATE, L), dtype=torch.uint8, device="cuda")
+    R_prev_gpu, R_ref = None, None
+    tau_d = dev(np.asarray([tau], np.int32))
+    for layer in range(layers):
+        qs, ks = heavy_tailed_sketches(50 + layer, b, r)
+        S = O.block_scores(qs.astype(np.float64), ks.astype(np.float64))
+        assert np.ptp(S[b - 1]) >= 12.0
+        A_ref = O.masked_softmax(S, flags)
+        W_ref = A_ref if (flags & O.POW_MATRIX) else O.power(A_ref, s, flags)
+        R_ref = O.walk_update(R_ref, A_ref, s, flags)
+        W = torch.empty(L.total_sq, device="cuda"); R = torch.empty(L.total_sq, device="cuda")
+        sw.sw_block_scores(L, dev(qs), dev(ks), r, s, flags, W, None)
+        sw.sw_walk_update(L, R_prev_gpu, W, s, flags, R, ws)
+        idx = torch.empty(b, tau, dtype=torch.int32, device="cuda"); cnt = torch.empty(b, dtype=torch.int32, device="cuda")
+        sw.sw_select_topk(L, R, tau_d, tau, flags, idx, cnt)
+        torch.cuda.synchronize()
+        assert rowwise_close(W.cpu().numpy().reshape(b, b), W_ref)
+        assert rowwise_close(R.cpu().numpy().reshape(b, b), R_ref)
+        idx_ref, cnt_ref = O.select_topk(R_ref, tau, flags)
+        idx_g, cnt_g = idx.cpu().numpy(), cnt.cpu().numpy()
+        assert np.array_equal(cnt_g, cnt_ref)
+        for i in range(b):
+            assert near_tie_only(idx_g[i, :cnt_g[i]], idx_ref[i, :cnt_ref[i]], R_ref[i], {0, i}), (layer, i)
+            # everything the oracle ranks clearly above the cut is selected by the GPU too
+            clear = [j for j in idx_ref[i, :cnt_ref[i]] if R_ref[i, j] > 2 * REL * np.abs(R_ref[i]).max()]
+            assert set(clear) <= set(idx_g[i, :cnt_g[i]].tolist())
+        R_prev_gpu = R
+
+
 # ------------------------------------------------------------------------------ decode selection path
-@pytest.mark.parametrize("fused", [True, False])
-@pytest.mark.parametrize("t,tau", [(64 * 5 + 1, 4), (64 * 5 + 32, 4), (64 * 6, 4), (64 * 70 + 9, 12),
-                                   (64 * 300 + 1, 40), (64 * 301, 40),
-                                   # max_blocks % 4 == 0: the cp.async ring of the fused kernel (else plain loads)
-                                   (64 * 7 + 3, 4), (64 * 71 + 9, 12), (64 * 299 + 5, 40), (64 * 300, 40),
-                                   # block size 128 (given as a negative t: |t| tokens)
-                                   (-(128 * 9 + 77), 4), (-(128 * 40), 9)])
-def test_decode_selection_matches_literal_alg2(sw, t, tau, fused):
-    """GPU decode selection -- the fused sw_decode_select launch, or the five row-vector calls (sketch_append x2,
-    block_scores_row, walk_update_row, select_topk_row) -- against the oracle's literal full-matrix Alg. 2,
-    three layers, caches built by the GPU prefill path.  The larger t span several column tiles per cluster CTA."""
+def near_tie_only(got, sel, ref_r, forced):
+    """Selected sets may differ only at near-ties: every index in the symmetric difference lies within
+    1e-3 of the row max of the lowest selected free score (north_star)."""
+    got = np.asarray(got); sel = np.asarray(sel)
+    if np.array_equal(got, sel):
+        return True
+    free = [j for j in sel.tolist() if j not in forced]
+    kth = min(ref_r[free]) if free else 0.0
+    scale = np.abs(ref_r).max()
+    return all(abs(ref_r[j] - kth) <= REL * scale for j in set(got.tolist()) ^ set(sel.tolist()))
+
+
+def decode_case(sw, t, tau, fused, flags, B=64, s=None, layers=3, scale_q=1.0):
+    """GPU decode selection against the oracle's literal full-matrix Alg. 2, ``layers`` layers with the walk row
+    carried, caches built by the GPU prefill path."""
     cfg = gen.CONFIGS[2]
-    B, r, s, d, h_q, h_kv = cfg.B, cfg.r, cfg.s, cfg.d, 8, 2
-    if t < 0:
-        t, B = -t, 128
+    r, d, h_q, h_kv = cfg.r, cfg.d, 8, 2
+    s = cfg.s if s is None else s
     signs, cols, H = H_of(d, r, seed=3)
-    flags = O.DEFAULT_FLAGS
     n_pre = t - 1
     b_pre, mb = O.num_blocks(n_pre, B), O.num_blocks(t, B)
     dp = sw.DecodePipeline(1, mb, h_q, h_kv, d, B, r, s, [tau], signs, cols, flags)
     R_full = None
-    for layer in range(3):
+    bq = (t - 1) // B
+    forced = {bq} | ({0} if flags & O.FORCE_FIRST else set())
+    for layer in range(layers):
         torch.manual_seed(100 + layer)
-        Q = (torch.randn(t, h_q, d) + 0.5).bfloat16(); K = (torch.randn(t, h_kv, d) + 0.5).bfloat16()
+        Q = ((torch.randn(t, h_q, d) + 0.5) * scale_q).bfloat16(); K = (torch.randn(t, h_kv, d) + 0.5).bfloat16()
         # caches from the GPU prefill selection path over the first t-1 tokens
         pp = sw.PrefillPipeline([n_pre], h_q, h_kv, d, B, r, s, 0.5, signs, cols, flags)
         pp.select(Q[:n_pre].cuda(), K[:n_pre].cuda())
@@ -529,16 +589,70 @@ def test_decode_selection_matches_literal_alg2(sw, t, tau, fused):
         pre = O.prefill_selection(Qn[:n_pre], Kn[:n_pre], None, B=B, H_d=H, s=s, tau=tau, flags=flags)
         sel, R_full, cache2 = O.decode_layer_literal(Qn[t - 1], Kn[t - 1], O.DecodeCache(pre.qbar, pre.kbar, pre.S), t,
                                                      R_full, B=B, H_d=H, s=s, tau=tau, flags=flags)
-        bq = (t - 1) // B
         assert rowwise_close(kbar[0].cpu().numpy(), cache2.kbar)
-        assert rowwise_close(dp.rvec[dp.cur][0, :bq + 1].cpu().numpy()[None], R_full[bq][None, :bq + 1], rel=2e-3)
+        r_gpu = dp.rvec[dp.cur][0].cpu().numpy()
+        assert rowwise_close(r_gpu[None, :bq + 1], R_full[bq][None, :bq + 1]), \
+            np.abs(r_gpu[:bq + 1] - R_full[bq][:bq + 1]).max() / np.abs(R_full[bq]).max()
+        assert (r_gpu[bq + 1:] == 0).all()
         got = dp.idx[0, :dp.count[0].item()].cpu().numpy()
-        ref_r = R_full[bq]
-        if not np.array_equal(got, sel):                     # only near-ties may differ
-            diff = set(got.tolist()) ^ set(sel.tolist())
-            thr = np.sort(ref_r[1:bq])[::-1][tau - 3]        # (tau-2)-th largest non-forced candidate
-            assert all(abs(ref_r[j] - thr) <= 1e-3 * np.abs(ref_r).max() for j in diff)
+        assert dp.count[0].item() == len(sel) and (dp.idx[0, len(sel):] == -1).all()
+        assert near_tie_only(got, sel, R_full[bq], forced), (got, sel)
         assert bq in got
+        if fused:                                        # the completion counters are back at zero
+            assert int(dp.select_ws[:512 + 4].view(torch.int32).abs().sum()) == 0
+
+
+@pytest.mark.parametrize("fused", [True, False])
+@pytest.mark.parametrize("t,tau", [(64 * 5 + 1, 4), (64 * 5 + 32, 4), (64 * 6, 4), (64 * 70 + 9, 12),
+                                   (64 * 300 + 1, 40), (64 * 301, 40),
+                                   # max_blocks % 4 == 0: the cp.async ring of the fused kernel (else plain loads)
+                                   (64 * 7 + 3, 4), (64 * 71 + 9, 12), (64 * 299 + 5, 40), (64 * 300, 40),
+                                   # b_q a multiple of 64: the column tile of b_q has no row of the cached W
+                                   (64 * 64 + 1, 12), (64 * 128 + 17, 30),
+                                   # block size 128 (given as a negative t: |t| tokens)
+                                   (-(128 * 9 + 77), 4), (-(128 * 40), 9)])
+def test_decode_selection_matches_literal_alg2(sw, t, tau, fused):
+    """GPU decode selection -- the fused sw_decode_select launch, or the five row-vector calls (sketch_append x2,
+    block_scores_row, walk_update_row, select_topk_row) -- against the oracle's literal full-matrix Alg. 2,
+    three layers, caches built by the GPU prefill path.  The larger t span several column tiles and CTAs."""
+    B = 64
+    if t < 0:
+        t, B = -t, 128
+    decode_case(sw, t, tau, fused, O.DEFAULT_FLAGS, B=B)
+
+
+@pytest.mark.parametrize("fused", [True, False])
+@pytest.mark.parametrize("flags", [O.DEFAULT_FLAGS & ~O.SCORE_SOFTMAX, O.DEFAULT_FLAGS & ~O.FORCE_FIRST,
+                                   O.DEFAULT_FLAGS & ~O.ROWNORM, O.CAUSAL | O.SCORE_SOFTMAX])
+@pytest.mark.parametrize("t,tau", [(64 * 5 + 32, 4), (64 * 71 + 9, 12), (64 * 300, 40)])
+def test_decode_selection_flag_variants(sw, t, tau, fused, flags):
+    """The readings other than the default on the decode path: raw signed scores (P5), no forced first block
+    (P7), no row rescale (P9), nothing forced but the current block."""
+    decode_case(sw, t, tau, fused, flags)
+
+
+@pytest.mark.parametrize("fused", [True, False])
+@pytest.mark.parametrize("t,tau", [(64 * 71 + 9, 12), (64 * 300, 40)])
+def test_decode_selection_paper_default_s8(sw, t, tau, fused):
+    """The paper's walk exponent s = 8, element-wise, on the decode path."""
+    decode_case(sw, t, tau, fused, O.DEFAULT_FLAGS, s=8)
+
+
+def test_decode_select_non_causal_is_rejected(sw):
+    """Alg. 2 Step 4(ii) is not carried by the row-vector form (P11): SW_ERR_UNSUPPORTED."""
+    cfg = gen.CONFIGS[2]
+    signs, cols, _ = H_of(cfg.d, cfg.r, seed=3)
+    flags = O.DEFAULT_FLAGS & ~O.CAUSAL
+    mb, t = 6, 64 * 5 + 7
+    for fused in (True, False):
+        dp = sw.DecodePipeline(1, mb, 8, 2, cfg.d, 64, cfg.r, 2, [3], signs, cols, flags)
+        q = torch.randn(1, 8, cfg.d).bfloat16().cuda(); k = torch.randn(1, 2, cfg.d).bfloat16().cuda()
+        kbar = torch.zeros(1, mb, cfg.d, device="cuda"); ks = torch.zeros(1, mb, cfg.r, device="cuda")
+        Wc = torch.zeros(1, mb, mb, device="cuda")
+        with pytest.raises(sw.SwError) as e:
+            dp.select(q, k, dev(np.asarray([t], np.int32)), kbar, ks, Wc, fused=fused)
+        assert e.value.code == sw.SW_ERR_UNSUPPORTED
+        assert (kbar == 0).all() and (Wc == 0).all()         # nothing was launched
 
 
 @pytest.mark.parametrize("nblk", [3, 299])
@@ -585,7 +699,7 @@ def test_decode_many_steps_across_a_block_boundary(sw, fused, nblk):
             sel, R_full, ora[l] = O.decode_layer_literal(gen.to_numpy_f64(Q[l][t - 1]), gen.to_numpy_f64(K[l][t - 1]),
                                                          ora[l], t, R_full, B=B, H_d=H, s=s, tau=tau, flags=flags)
             assert rowwise_close(kbar[0, :bq + 1].cpu().numpy(), ora[l].kbar[:bq + 1])
-            assert rowwise_close(dp.rvec[dp.cur][0, :bq + 1].cpu().numpy()[None], R_full[bq][None, :bq + 1], rel=2e-3)
+            assert rowwise_close(dp.rvec[dp.cur][0, :bq + 1].cpu().numpy()[None], R_full[bq][None, :bq + 1])
             # the cached row of the current block is the new row of W (what a later step will read)
             W_ref = O.power(O.masked_softmax(ora[l].S, flags), s, flags)
             assert rowwise_close(Wc[0, bq, :bq + 1].cpu().numpy()[None], W_ref[bq][None, :bq + 1])

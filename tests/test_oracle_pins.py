@@ -495,6 +495,64 @@ def test_decode_row_walk_equals_literal_alg2_row(t):
         assert np.allclose(cache2.S[b_q, :b_q + 1], a_new[:b_q + 1], atol=1e-13)
 
 
+@pytest.mark.parametrize("t", [3 * 16 + 1, 3 * 16 + 7, 4 * 16, 16 + 1])
+@pytest.mark.parametrize("steps", [1, 3])
+def test_decode_literal_column_update_and_running_query_mean(t, steps):
+    """Alg. 2 Step 4(ii) ("update last column ... c_new = Q~ k~_{b_curr}") and the
+    running mean of the decode-time q_avg (P11), pinned with CAUSAL off so that neither is masked out:
+    after decoding tokens t .. t+steps-1 the cached score matrix must equal the block scores rebuilt from
+    scratch over all tokens seen so far -- plain double loop S[i, j] = q~_i . k~_j / sqrt(r) on the block
+    means of the raw tokens -- except row b_q, which holds the single-token row of the latest step
+    (PAPER.md:814-821), and the cached query reps must equal the block means of Q."""
+    B, hq, hkv, d, r, s, tau = 16, 4, 2, 8, 4, 2, 3
+    rng = np.random.RandomState(100 * t + steps)
+    signs = rng.randint(0, 2, d) * 2 - 1
+    cols = np.array([1, 2, 4, 7])
+    H = O.srht_matrix(d, signs, cols, 1.0 / math.sqrt(r))
+    flags = O.SCORE_SOFTMAX | O.FORCE_FIRST | O.FORCE_LAST | O.ROWNORM       # CAUSAL off
+    t_end = t + steps - 1
+    Q, K = rng.randn(t_end, hq, d), rng.randn(t_end, hkv, d)
+    pre = O.prefill_selection(Q[:t - 1], K[:t - 1], None, B=B, H_d=H, s=s, tau=tau, flags=flags)
+    cache = O.DecodeCache(pre.qbar, pre.kbar, pre.S)
+    for tt in range(t, t_end + 1):
+        sel, R, cache = O.decode_layer_literal(Q[tt - 1], K[tt - 1], cache, tt, None, B=B, H_d=H, s=s, tau=tau,
+                                               flags=flags)
+        b = O.num_blocks(tt, B)
+        b_q = (tt - 1) // B
+        # from scratch, written out: head mean, block mean, explicit Hadamard sums, double loop
+        qbar = np.zeros((b, d)); kbar = np.zeros((b, d))
+        for i in range(b):
+            lo, hi = i * B, min((i + 1) * B, tt)
+            qbar[i] = Q[lo:hi].mean(axis=1).mean(axis=0)
+            kbar[i] = K[lo:hi].mean(axis=1).mean(axis=0)
+        assert np.allclose(cache.qbar, qbar, atol=1e-13)
+        assert np.allclose(cache.kbar, kbar, atol=1e-13)
+
+        def sk(v):
+            return np.array([sum(v[x] * signs[x] * (-1) ** bin(x & c).count("1") for x in range(d)) for c in cols]) / math.sqrt(r)
+
+        S = np.zeros((b, b))
+        for i in range(b):
+            for j in range(b):
+                S[i, j] = sk(qbar[i]) @ sk(kbar[j]) / math.sqrt(r)
+        # P11: a block that completed during decode keeps, left of and on the diagonal, the single-token row
+        # of its last token (row b_q wins; the later column updates only write columns > i of that row)
+        for i in range((t - 1) // B, b_q):
+            q_last = Q[(i + 1) * B - 1].mean(axis=0)
+            for j in range(i + 1):
+                S[i, j] = sk(q_last) @ sk(kbar[j]) / math.sqrt(r)
+        q_tok = Q[tt - 1].mean(axis=0)
+        for j in range(b):
+            S[b_q, j] = sk(q_tok) @ sk(kbar[j]) / math.sqrt(r)
+        assert cache.S.shape == (b, b)
+        assert np.allclose(cache.S, S, atol=1e-12), np.abs(cache.S - S).max()
+        # the column really changed (the pin would be vacuous otherwise) unless the block has just started
+        if b_q > 0 and (tt - 1) % B != 0:
+            stale = sk(qbar[0]) @ sk(K[b_q * B:tt - 1].mean(axis=1).mean(axis=0)) / math.sqrt(r)
+            assert abs(stale - S[0, b_q]) > 1e-9
+        assert R.shape == (b, b) and b_q in sel
+
+
 def test_prefill_layer_end_to_end_full_density_is_dense():
     n, B, hq, hkv, d, r = 128, 16, 4, 2, 8, 4
     Q, K, V = RNG.randn(n, hq, d), RNG.randn(n, hkv, d), RNG.randn(n, hkv, d)

@@ -3,21 +3,23 @@
 // row-vector walk r^k = r^{k-1} W'^k (Step 5), the max-abs rescale (P9) and the
 // top-tau selection (Step 6).  HBM-bound on the cached W (4 b^2/2 bytes per sequence).
 //
-// The whole grid (two CTAs per SM) streams the cached W, whatever the batch: the work of the batch is
-// cut into items -- one 64-row x 64-column chunk of the block-causal part of W each (rows [64 c, b_q) of
-// column tile c), at least one item per column tile -- numbered over all sequences, and CTA i takes the
-// contiguous range [i T / G, (i+1) T / G) of the T items.  A CTA accumulates r_prev[m] W[m][j] over its
-// chunks of one column tile in registers and leaves one 64-float partial per (tile, CTA) in the workspace
-// (fixed slots, fixed summation order: deterministic).  The first item of every column tile also carries the
-// "score duty": q~_t (and, on the tile that holds b_q, the running key-block mean and its sketch) and the
-// raw scores of its 64 columns.  Nothing waits on another CTA: every CTA counts the items it has finished
-// per sequence with one atomic, and the CTA that completes a sequence runs that sequence's tail -- softmax
-// statistics of the score row, W_new = A^s, r = sum of partials + r_prev[b_q] W_new, rescale, radix select
-// (select.cuh) -- on a row of at most max_blocks floats in shared memory.  The counters live in the
-// caller's workspace and are left at zero by every completed call.
-// The cached W streams through a cp.async ring (5 x 16 KB per CTA), requested before the score duty runs;
-// the new row of W is stored as row b_q of the cache (Alg. 2 Step 4).  DESIGN.md sec. 6.2 has the
-// measurements behind these choices.
+// The whole grid (two CTAs per SM) works on the batch, whatever its size.  Two kinds of work are dealt out:
+//  * chunks: 64 rows x 64 columns of the block-causal part of the cached W (rows [64 c, b_q) of column tile
+//    c), numbered over all sequences; CTA i streams the contiguous range [i T / G, (i+1) T / G) of the T
+//    chunks through a cp.async ring, accumulates r_prev[m] W[m][j] over the chunks of one column tile in
+//    registers and leaves one 64-float partial per (tile, CTA) in the workspace (fixed slots, fixed
+//    summation order: deterministic);
+//  * duties: one per (sequence, column tile), dealt the same way: q~_t (and, on the tile that holds b_q, the
+//    running key-block mean and its sketch) and the raw scores of the tile's 64 columns.
+// A CTA runs its duties first.  Every load they need (head values, key-sketch rows, the old mean) and the
+// r_prev rows of the stream are requested BEFORE the first chunks of the W stream: on an SM that keeps
+// ~160 KB of the stream in flight a load issued behind it waits ~3 us (queue depth / per-SM bandwidth).
+// Nothing waits on another CTA: every CTA counts what it has finished per sequence with one atomic, and
+// the CTA that completes a sequence runs its tail -- softmax statistics of the score row, W_new = A^s,
+// r = sum of partials + r_prev[b_q] W_new, rescale, radix select (select.cuh) -- on a row of at most
+// max_blocks floats in shared memory.  The counters live in the caller's workspace and are left at zero by
+// every completed call.  The new row of W is stored as row b_q of the cache (Alg. 2 Step 4).
+// DESIGN.md sec. 6.2 has the measurements behind these choices.
 #include <algorithm>
 
 #include "common.cuh"
@@ -31,10 +33,13 @@ constexpr int kThreads = 256;
 constexpr int kTile = 64;            // columns per tile
 constexpr int kRowGroups = 16;       // row lanes of the vector-matrix product
 constexpr int kChunkRows = 64;
-constexpr int kStages = 5;
+constexpr int kStages = 4;            // 4 x 16 KB ring + two r_prev rows + the prefix tables: two CTAs per SM
 constexpr int kChunkBytes = kChunkRows * kTile * 4;
 constexpr int kPieces = kChunkBytes / 16 / kThreads;     // 16-byte cp.async pieces per thread per chunk
-constexpr int kMaxBatch = 1024;      // per-sequence item counts are scanned in shared memory
+constexpr int kMaxBatch = 512;       // sequence lengths and per-sequence work counts live in shared memory
+constexpr int kMaxTiles = 255;       // column tiles per sequence (max_blocks <= 16320)
+constexpr int kHeadRegs = 16;        // head values a thread holds while the loads of a duty are in flight
+constexpr int kKU = 4;               // key-sketch float4s per thread and duty (64 columns x r <= 64)
 
 struct Params {
   const void* q;  int64_t q_stride_seq, q_stride_head;  int h_q;
@@ -50,34 +55,37 @@ struct Params {
   int batch, B, max_blocks;
   int use_async;                     // W streamed by cp.async (needs 16-byte aligned rows), else plain loads
   // workspace
-  unsigned int* ws_cnt;              // [batch] items finished per sequence (zero between calls)
+  unsigned int* ws_cnt;              // [batch] duties + chunks finished per sequence (zero between calls)
   float* ws_scores;                  // [batch][mbp] raw scores of the new row
   float* ws_part;                    // [batch][tiles_max][slots][64] partial walk sums
   int mbp, tiles_max, slots;
 };
 
-// Item bookkeeping of one sequence.  b_q = 64 a + e; column tile c < a has rows [64 c, b_q): a - c + (e > 0)
-// chunks; tile a (the one that holds b_q) has (e > 0) chunks and always one item.  Without a walk
-// (r_prev = NULL) every tile is a single score-only item.
+// Work bookkeeping of one sequence.  b_q = 64 a + e; column tile c < a has rows [64 c, b_q): a - c + (e > 0)
+// chunks; tile a (the one that holds b_q) has (e > 0) chunks.  a + 1 duties.  No chunks without a walk
+// (r_prev = NULL).
 struct SeqInfo {
   int bq, a, eps;
   __device__ __forceinline__ int chunks(int tile, bool walk) const { return walk ? (tile < a ? a - tile + eps : eps) : 0; }
-  __device__ __forceinline__ int items(int tile, bool walk) const { return max(1, chunks(tile, walk)); }
-  __device__ __forceinline__ int items_before(int tile, bool walk) const {        // tile <= a
-    return walk ? tile * a - tile * (tile - 1) / 2 + tile * eps : tile;
+  __device__ __forceinline__ int chunks_before(int tile, bool walk) const {        // tile <= a
+    return walk ? tile * a - tile * (tile - 1) / 2 + tile * eps : 0;
   }
-  __device__ __forceinline__ int total(bool walk) const { return walk ? a * (a + 1) / 2 + a * eps + 1 : a + 1; }
+  __device__ __forceinline__ int total_chunks(bool walk) const { return walk ? a * (a + 1) / 2 + a * eps + eps : 0; }
+  __device__ __forceinline__ int duties() const { return a + 1; }
 };
 __device__ __forceinline__ SeqInfo seq_info(const int32_t* seqlens, int seq, int B) {
   SeqInfo s;
-  const int t = __ldg(seqlens + seq);
+  const int t = seqlens[seq];                          // (a shared-memory copy after the first pass)
   s.bq = (t - 1) / B;                                  // block of the new token = b_curr
   s.a = s.bq / kTile;
   s.eps = (s.bq % kTile) != 0;
   return s;
 }
-// CTA that owns global item g when T items are dealt to G CTAs as [i T / G, (i+1) T / G)
-__device__ __forceinline__ int cta_of(long long g, int T, int G) { return (int)(((g + 1) * G - 1) / T); }
+// CTA that owns item g when T items are dealt to G CTAs as [i T / G, (i+1) T / G)
+__device__ __forceinline__ int cta_of(long long g, int T, int G) {
+  const long long num = (g + 1) * G - 1;
+  return (num < (1ll << 31)) ? (int)((unsigned)num / (unsigned)T) : (int)(num / T);
+}
 
 __device__ __forceinline__ float block_max(float v, float* s_red) {
   v = swd::warp_max(v);
@@ -99,20 +107,25 @@ __device__ __forceinline__ float block_sum(float v, float* s_red) {
   for (int w = 0; w < kThreads / 32; ++w) m += s_red[w];
   return m;
 }
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 
 template <typename TIn, int D>
 __global__ void __launch_bounds__(kThreads, 2)
 decode_select_kernel(const Params p) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int G = (int)gridDim.x;
+  const int G = (int)gridDim.x, me = (int)blockIdx.x;
   const bool walk = p.r_prev != nullptr;
   const bool async = walk && p.use_async;
   const bool soft = p.flags & SW_SCORE_SOFTMAX;
   const int mb = p.max_blocks;
+  const int rstride = p.mbp + kChunkRows;
 
   extern __shared__ __align__(128) uint8_t smem_raw[];
-  float* s_rprev = reinterpret_cast<float*>(smem_raw);                 // [mbp + 64] r_prev of the current sequence
-  float* s_part = s_rprev + p.mbp + kChunkRows;                        // [kRowGroups][64]
+  float* s_rprev = reinterpret_cast<float*>(smem_raw);                 // [2][mbp + 64] r_prev of two sequences
+  float* s_part = s_rprev + 2 * rstride;                               // [kRowGroups][64]
   uint8_t* s_ring = reinterpret_cast<uint8_t*>(
       (reinterpret_cast<uintptr_t>(s_part + kRowGroups * kTile) + 127) & ~(uintptr_t)127);   // [kStages][16 KB]
   float* s_row = reinterpret_cast<float*>(s_ring);                     // [mbp] tail only (the ring is idle then)
@@ -120,80 +133,97 @@ decode_select_kernel(const Params p) {
   __shared__ float s_hx[kThreads / D][D];
   __shared__ int32_t s_cols[128];
   __shared__ float s_red[kThreads / 32];
-  __shared__ int s_pref[kMaxBatch + 1];                                // exclusive prefix of items per sequence
-  __shared__ int s_scan[kThreads / 32];
-  __shared__ int s_last;                                               // this CTA has at least one tail to run
+  __shared__ int s_pref[kMaxBatch + 1];                                // exclusive prefix of chunks per sequence
+  __shared__ int s_dpref[kMaxBatch + 1];                               // exclusive prefix of duties per sequence
+  __shared__ int s_len[kMaxBatch];                                     // sequence lengths (read once from HBM)
+  __shared__ int s_scan[2][kThreads / 32];
+  __shared__ int s_flag;                                               // this CTA completed some sequence
   __shared__ unsigned s_tailmask[kMaxBatch / 32];                      // sequences whose tail this CTA runs
+  __shared__ unsigned char s_nslot[kMaxTiles + 1];                     // tail: partials per column tile
   __shared__ swsel::Scratch scratch;
 
-  // ---- item counts of all sequences: exclusive prefix in shared memory ------------------------------
+  // ---- chunk and duty counts of all sequences: exclusive prefixes in shared memory -------------------
   {
     constexpr int kPer = kMaxBatch / kThreads;
-    int v[kPer], sum = 0;
+    int vc[kPer], vd[kPer], sc = 0, sd = 0;
 #pragma unroll
     for (int e = 0; e < kPer; ++e) {
       const int sq = tid * kPer + e;
-      v[e] = (sq < p.batch) ? seq_info(p.seqlens, sq, p.B).total(walk) : 0;
-      sum += v[e];
+      vc[e] = 0; vd[e] = 0;
+      if (sq < p.batch) {
+        s_len[sq] = __ldg(p.seqlens + sq);
+        const SeqInfo si = seq_info(s_len, sq, p.B);
+        vc[e] = si.total_chunks(walk); vd[e] = si.duties();
+      }
+      sc += vc[e]; sd += vd[e];
     }
-    int incl = sum;
+    int ic = sc, id = sd;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const int u = __shfl_up_sync(0xffffffffu, incl, o);
-      if (lane >= o) incl += u;
+      const int uc = __shfl_up_sync(0xffffffffu, ic, o), ud = __shfl_up_sync(0xffffffffu, id, o);
+      if (lane >= o) { ic += uc; id += ud; }
     }
-    if (lane == 31) s_scan[warp] = incl;
+    if (lane == 31) { s_scan[0][warp] = ic; s_scan[1][warp] = id; }
     if (tid < D) s_sign[tid] = p.signs ? (float)p.signs[tid] : 1.f;
     if (tid < kMaxBatch / 32) s_tailmask[tid] = 0u;
-    if (tid == 0) s_last = 0;
+    if (tid == 0) s_flag = 0;
     if (tid < p.r && tid < 128) s_cols[tid] = p.cols[tid];
     __syncthreads();
-    int base = 0;
-    for (int w = 0; w < warp; ++w) base += s_scan[w];
-    int run = base + incl - sum;
+    int bc = 0, bd = 0;
+    for (int w = 0; w < warp; ++w) { bc += s_scan[0][w]; bd += s_scan[1][w]; }
+    int rc = bc + ic - sc, rd = bd + id - sd;
 #pragma unroll
     for (int e = 0; e < kPer; ++e) {
       const int sq = tid * kPer + e;
-      if (sq <= p.batch) s_pref[sq] = run;
-      run += v[e];
+      if (sq <= p.batch) { s_pref[sq] = rc; s_dpref[sq] = rd; }
+      rc += vc[e]; rd += vd[e];
     }
     __syncthreads();
   }
-  const int T = s_pref[p.batch];
-  const int g_begin = (int)((long long)blockIdx.x * T / G), g_end = (int)((long long)(blockIdx.x + 1) * T / G);
+  const int T = s_pref[p.batch], ND = s_dpref[p.batch];
+  const int g_begin = (int)((long long)me * T / G), g_end = (int)((long long)(me + 1) * T / G);
+  const int d_begin = (int)((long long)me * ND / G), d_end = (int)((long long)(me + 1) * ND / G);
   const int n_my = g_end - g_begin;
-  if (n_my == 0) return;
+  if (n_my == 0 && d_begin == d_end) return;
 
-  // ---- cursors over this CTA's items (thread-uniform) -------------------------------------------------
+  auto find_seq = [&](const int* pref, int g) {
+    int lo = 0, hi = p.batch - 1;
+    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (pref[mid] <= g) lo = mid; else hi = mid - 1; }
+    return lo;
+  };
+
+  // ---- cursors over this CTA's chunks (thread-uniform) ------------------------------------------------
   struct Cursor { int seq, tile, chunk; SeqInfo si; };
   auto locate = [&](int g) {
     Cursor c;
-    int lo = 0, hi = p.batch - 1;
-    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_pref[mid] <= g) lo = mid; else hi = mid - 1; }
-    c.seq = lo;
-    c.si = seq_info(p.seqlens, lo, p.B);
-    const int local = g - s_pref[lo];
+    c.seq = find_seq(s_pref, g);
+    c.si = seq_info(s_len, c.seq, p.B);
+    const int local = g - s_pref[c.seq];
     int tl = 0, th = c.si.a;
-    while (tl < th) { const int mid = (tl + th + 1) >> 1; if (c.si.items_before(mid, walk) <= local) tl = mid; else th = mid - 1; }
+    while (tl < th) { const int mid = (tl + th + 1) >> 1; if (c.si.chunks_before(mid, walk) <= local) tl = mid; else th = mid - 1; }
     c.tile = tl;
-    c.chunk = local - c.si.items_before(tl, walk);
+    c.chunk = local - c.si.chunks_before(tl, walk);
     return c;
   };
   auto advance = [&](Cursor& c) {
-    if (++c.chunk >= c.si.items(c.tile, walk)) {
+    ++c.chunk;
+    while (c.seq < p.batch && c.chunk >= c.si.chunks(c.tile, walk)) {
       c.chunk = 0;
       if (++c.tile > c.si.a) {
         c.tile = 0;
-        if (++c.seq < p.batch) c.si = seq_info(p.seqlens, c.seq, p.B);
+        if (++c.seq < p.batch) c.si = seq_info(s_len, c.seq, p.B);
       }
     }
   };
-  Cursor cc = locate(g_begin), pc = cc;
+  Cursor cc, pc;
+  cc.seq = cc.tile = cc.chunk = 0; cc.si.bq = cc.si.a = cc.si.eps = 0;
+  int seq_first = 0;
+  if (n_my > 0) { cc = locate(g_begin); seq_first = cc.seq; }
+  pc = cc;
 
   // ---- W stream: chunk = rows [64 tile + 64 chunk, +64) x columns [64 tile, +64) of the sequence's cached W
   int p_left = n_my, issued = 0;
   auto issue_next = [&]() {                           // all threads: request the next chunk (or an empty group)
-    while (p_left > 0 && pc.si.chunks(pc.tile, walk) == 0) { advance(pc); --p_left; }
     if (p_left > 0) {
       const float* Wseq = p.W + (int64_t)pc.seq * p.w_stride_seq;
       const int m0 = (pc.tile + pc.chunk) * kTile;
@@ -202,54 +232,258 @@ decode_select_kernel(const Params p) {
       for (int u = 0; u < kPieces; ++u) {
         const int pcs = u * kThreads + tid, rr = pcs >> 4, c4 = pc.tile * kTile + (pcs & 15) * 4;
         if (m0 + rr < pc.si.bq && c4 < mb)            // rows >= b_q / columns >= max_blocks are never read
-          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + pcs * 16),
-                       "l"(Wseq + (int64_t)(m0 + rr) * mb + c4) : "memory");
+          cp_async16(dst + pcs * 16, Wseq + (int64_t)(m0 + rr) * mb + c4);
       }
       ++issued; advance(pc); --p_left;
     }
-    asm volatile("cp.async.commit_group;" ::: "memory");
+    cp_async_commit();
   };
-  if (async)
-    for (int i = 0; i < kStages - 1; ++i) issue_next();
-
-  // head mean of x[seq] (all heads) -> s_vec (fp32), by all threads
-  constexpr int kGroups = kThreads / D;
-  auto head_mean = [&](const void* base, int64_t stride_seq, int64_t stride_head, int heads, int seq) {
-    const int hx = tid % D, hg = tid / D;
-    const TIn* xp = reinterpret_cast<const TIn*>(base) + (int64_t)seq * stride_seq + hx;
-    constexpr int kRegs = 16;
-    float v[kRegs];
-#pragma unroll
-    for (int u = 0; u < kRegs; ++u) {
-      const int h = hg + u * kGroups;
-      v[u] = (h < heads) ? (float)xp[(int64_t)h * stride_head] : 0.f;
+  // r_prev of the first two sequences of this CTA's chunk range (group 0 of the cp.async stream), then the
+  // first kStages - 1 chunks.  Called once, after the loads of the last duty have been issued.
+  auto start_stream = [&]() {
+    if (n_my == 0) return;                            // (no chunks without a walk)
+    for (int q2 = 0; q2 < 2; ++q2) {
+      const int sq = seq_first + q2;
+      if (sq < p.batch && (q2 == 0 || s_pref[sq] < g_end)) {
+        const float* rp = p.r_prev + (int64_t)sq * mb;
+        if (async)
+          for (int i = tid * 4; i < mb; i += kThreads * 4) cp_async16(sm100::smem_u32(s_rprev + q2 * rstride + i), rp + i);
+        else
+          for (int i = tid; i < mb; i += kThreads) s_rprev[q2 * rstride + i] = __ldg(rp + i);
+      }
     }
-    float sm = 0.f;
-#pragma unroll
-    for (int u = 0; u < kRegs; ++u) sm += v[u];
-    for (int h = hg + kRegs * kGroups; h < heads; h += kGroups) sm += (float)xp[(int64_t)h * stride_head];
-    s_hx[hg][hx] = sm;
-    __syncthreads();
-    if (tid < D) {
-      float a = 0.f;
-#pragma unroll
-      for (int g = 0; g < kGroups; ++g) a += s_hx[g][tid];
-      s_vec[tid] = a / (float)heads;
+    if (async) {
+      cp_async_commit();
+      for (int i = 0; i < kStages - 1; ++i) issue_next();
     }
-    __syncthreads();
   };
 
-  const int q4 = p.r >> 2;                            // float4s per sketch row
-  int cur_seq = -1, qt_seq = -1, done_in_seq = 0, consumed = 0;
-  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-  bool acc_live = false;
-  const int cq = tid & 15, rg = tid >> 4;
-
-  // tail of one sequence (this CTA finished its last item): Steps 4-6 on the whole row
-  auto run_tail = [&](int seq) {
-    const SeqInfo si = seq_info(p.seqlens, seq, p.B);
-    const int bq = si.bq, hi = bq + 1;
+  // this CTA has finished `n` duties / chunks of sequence `seq`: publish; the CTA that completes a sequence
+  // runs its tail (after its own streaming work: the tail's row buffer aliases the ring)
+  auto publish = [&](int seq, int n) {
     __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+      const SeqInfo si = seq_info(s_len, seq, p.B);
+      const unsigned total = (unsigned)(si.duties() + si.total_chunks(walk));
+      const unsigned old = atomicAdd(p.ws_cnt + seq, (unsigned)n);
+      if (old + (unsigned)n == total) {               // every other CTA's partials and scores are visible after
+        __threadfence();                              // this fence; the tail reads them past a barrier, from L2
+        s_tailmask[seq >> 5] |= 1u << (seq & 31); s_flag = 1;
+      }
+    }
+  };
+
+  // ================= duties: Steps 2-4 for one column tile each ==========================================
+  constexpr int kGroups = kThreads / D;
+  const int q4 = p.r >> 2;                            // float4s per sketch row
+  const bool vec_ok = (p.r & 3) == 0 && q4 >= 1 && q4 <= 32 && (q4 & (q4 - 1)) == 0 && kTile * q4 <= kKU * kThreads &&
+                      (reinterpret_cast<uintptr_t>(p.ks) & 15u) == 0;
+  const int hx = tid % D, hg = tid / D;
+  int qt_seq = -1;
+  bool stream_started = false;
+  for (int dty = d_begin; dty < d_end; ++dty) {
+    const int seq = find_seq(s_dpref, dty), tile = dty - s_dpref[seq];
+    const SeqInfo si = seq_info(s_len, seq, p.B);
+    const int bq = si.bq, hi = bq + 1, col0 = tile * kTile;
+    const bool need_q = qt_seq != seq, need_k = tile == si.a;   // tile a owns the key-side update of Step 2
+    const float* ksb = p.ks + (int64_t)seq * mb * p.r;
+    const int part = vec_ok ? (tid & (q4 - 1)) : 0, per_pass = vec_ok ? kThreads / q4 : 1;
+    const int colq = vec_ok ? tid / q4 : 0;
+    // ---- all loads of the duty, before anything waits on memory: unconditional loads from clamped (always
+    // valid) addresses, raw values kept in registers -- a predicated load followed by its convert made every
+    // group of loads wait for the previous one (5 us instead of one memory latency)
+    TIn qraw[kHeadRegs], kraw[kHeadRegs];
+    float4 kv[kKU];
+    const TIn* qp = reinterpret_cast<const TIn*>(p.q) + (int64_t)seq * p.q_stride_seq + hx;
+    const TIn* kp = reinterpret_cast<const TIn*>(p.k) + (int64_t)seq * p.k_stride_seq + hx;
+#pragma unroll
+    for (int u = 0; u < kHeadRegs; ++u) {
+      const int h = hg + u * kGroups;
+      qraw[u] = qp[(int64_t)min(h, p.h_q - 1) * p.q_stride_head];
+      kraw[u] = kp[(int64_t)min(h, p.h_kv - 1) * p.k_stride_head];
+    }
+    const int cnt = (s_len[seq] - 1) % p.B;                        // tokens already in block b_curr
+    float* kb = p.kbar + ((int64_t)seq * mb + bq) * D;
+    const float kbar_old = kb[tid & (D - 1)];
+#pragma unroll
+    for (int u = 0; u < kKU; ++u) {
+      const int cj = u * per_pass + colq;
+      const int j = min(col0 + min(cj, kTile - 1), bq);                        // clamped: always a valid row
+      kv[u] = vec_ok ? *reinterpret_cast<const float4*>(ksb + (int64_t)j * p.r + part * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    if (dty == d_end - 1) { start_stream(); stream_started = true; }
+    // ---- head means, running key-block mean, sketches ----------------------------------------------------
+    if (need_q || need_k) {
+      float sq = 0.f, sk = 0.f;
+#pragma unroll
+      for (int u = 0; u < kHeadRegs; ++u) {
+        const int h = hg + u * kGroups;
+        if (h < p.h_q) sq += (float)qraw[u];
+        if (h < p.h_kv) sk += (float)kraw[u];
+      }
+      if (need_q) for (int h = hg + kHeadRegs * kGroups; h < p.h_q; h += kGroups) sq += (float)qp[(int64_t)h * p.q_stride_head];
+      if (need_k) for (int h = hg + kHeadRegs * kGroups; h < p.h_kv; h += kGroups) sk += (float)kp[(int64_t)h * p.k_stride_head];
+      if (need_q) {
+        s_hx[hg][hx] = sq;
+        __syncthreads();
+        if (tid < D) {
+          float a = 0.f;
+#pragma unroll
+          for (int g = 0; g < kGroups; ++g) a += s_hx[g][tid];
+          s_vec[tid] = a / (float)p.h_q;
+        }
+        __syncthreads();
+        swsk::sketch_tail<D>(s_vec, s_sign, s_cols, p.r, p.scale, s_qt);         // q~_t
+        qt_seq = seq;
+        __syncthreads();
+      }
+      if (need_k) {
+        s_hx[hg][hx] = sk;
+        __syncthreads();
+        if (tid < D) {
+          float a = 0.f;
+#pragma unroll
+          for (int g = 0; g < kGroups; ++g) a += s_hx[g][tid];
+          const float avg = a / (float)p.h_kv;
+          const float mn = (cnt == 0) ? avg : ((float)cnt * kbar_old + avg) / (float)(cnt + 1);
+          kb[tid] = mn;                                                          // PAPER.md:811-813
+          s_vec[tid] = mn;
+        }
+        __syncthreads();
+        swsk::sketch_tail<D>(s_vec, s_sign, s_cols, p.r, p.scale, s_kt, p.ks + ((int64_t)seq * mb + bq) * p.r);
+        __syncthreads();
+      }
+    }
+    // ---- raw scores of the tile's columns (Steps 3-4; column b_q from the fresh sketch) --------------------
+    float* sc = p.ws_scores + (int64_t)seq * p.mbp;
+    if (vec_ok) {
+      // q4 adjacent lanes share one column; partial dots meet in a fixed xor butterfly
+      const float4 qv = *reinterpret_cast<const float4*>(s_qt + part * 4);
+#pragma unroll
+      for (int u = 0; u < kKU; ++u) {
+        if (u * per_pass >= kTile) break;                                        // warp-uniform
+        const int cj = u * per_pass + colq, j = col0 + cj;
+        if (j == bq) kv[u] = *reinterpret_cast<const float4*>(s_kt + part * 4);
+        float a = fmaf(qv.w, kv[u].w, fmaf(qv.z, kv[u].z, fmaf(qv.y, kv[u].y, qv.x * kv[u].x)));
+        for (int o = q4 >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+        if (part == 0 && cj < kTile && j < hi) sc[j] = a * p.inv_sqrt_r;
+      }
+    } else {
+      for (int cj = warp; cj < kTile; cj += kThreads / 32) {
+        const int j = col0 + cj;
+        if (j < hi) {
+          const float* kr = (j == bq) ? s_kt : ksb + (int64_t)j * p.r;
+          float a = 0.f;
+          for (int c = lane; c < p.r; c += 32) a = fmaf(s_qt[c], kr[c], a);
+          a = swd::warp_sum(a);
+          if (lane == 0) sc[j] = a * p.inv_sqrt_r;
+        }
+      }
+    }
+    // duties of one sequence are published together
+    if (dty == d_end - 1 || find_seq(s_dpref, dty + 1) != seq) {
+      const int first = max(d_begin, s_dpref[seq]);
+      publish(seq, dty - first + 1);
+    }
+  }
+  if (!stream_started) start_stream();
+
+  // ================= chunks: Step 5, r_prev[m] W[m][j] over this CTA's range ===============================
+  int cur_seq = -1, done_in_seq = 0, consumed = 0;
+  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  const int cq = tid & 15, rg = tid >> 4;
+  const float* rprev_cur = s_rprev;
+  for (int it = 0; it < n_my; ++it) {
+    const SeqInfo& si = cc.si;
+    const int seq = cc.seq, tile = cc.tile, bq = si.bq;
+    if (seq != cur_seq) {
+      if (cur_seq >= 0) { publish(cur_seq, done_in_seq); done_in_seq = 0; }
+      cur_seq = seq;
+      const int slot2 = seq - seq_first;
+      if (slot2 < 2) {
+        rprev_cur = s_rprev + slot2 * rstride;        // requested up front
+      } else {                                        // a range over more than two (tiny) sequences: reload
+        __syncthreads();
+        const float* rp = p.r_prev + (int64_t)seq * mb;
+        for (int i = tid; i < mb; i += kThreads) s_rprev[i] = __ldg(rp + i);
+        rprev_cur = s_rprev;
+        __syncthreads();
+      }
+    }
+    const int m0 = (tile + cc.chunk) * kTile;
+    const int rows = min(kChunkRows, bq - m0);        // rows >= b_q are not part of the product
+    if (async) {
+      asm volatile("cp.async.wait_group %0;" ::"n"(kStages - 2) : "memory");   // chunk `consumed` (and r_prev) landed
+      __syncthreads();                                // ... for every thread; the previous chunk is fully consumed
+      issue_next();                                   // refill the stage the previous chunk occupied
+      const float* box = reinterpret_cast<const float*>(s_ring + (size_t)(consumed % kStages) * kChunkBytes);
+#pragma unroll
+      for (int u = 0; u < kChunkRows / kRowGroups; ++u) {
+        const int rr = rg + u * kRowGroups;
+        if (rr < rows) {
+          const float4 v = *reinterpret_cast<const float4*>(box + rr * kTile + cq * 4);
+          const float a = rprev_cur[m0 + rr];
+          acc.x = fmaf(a, v.x, acc.x);
+          acc.y = fmaf(a, v.y, acc.y);
+          acc.z = fmaf(a, v.z, acc.z);
+          acc.w = fmaf(a, v.w, acc.w);
+        }
+      }
+      ++consumed;
+    } else {
+      if (it == 0) __syncthreads();                   // s_rprev is complete
+      const float* Wm = p.W + (int64_t)seq * p.w_stride_seq;
+      const int c4 = tile * kTile + cq * 4;
+      for (int rr = rg; rr < rows; rr += kRowGroups) {
+        const float a = rprev_cur[m0 + rr];
+        const float* wr = Wm + (int64_t)(m0 + rr) * mb;
+        if (c4 + 0 < mb) acc.x = fmaf(a, __ldg(wr + c4 + 0), acc.x);
+        if (c4 + 1 < mb) acc.y = fmaf(a, __ldg(wr + c4 + 1), acc.y);
+        if (c4 + 2 < mb) acc.z = fmaf(a, __ldg(wr + c4 + 2), acc.z);
+        if (c4 + 3 < mb) acc.w = fmaf(a, __ldg(wr + c4 + 3), acc.w);
+      }
+    }
+    ++done_in_seq;
+    if (it == n_my - 1 || cc.chunk + 1 >= si.chunks(tile, walk)) {
+      // one partial per (tile, CTA): slot = rank of this CTA among the CTAs that share the tile
+      *reinterpret_cast<float4*>(s_part + rg * kTile + cq * 4) = acc;
+      __syncthreads();
+      if (tid < kTile) {
+        float v = 0.f;
+#pragma unroll
+        for (int g = 0; g < kRowGroups; ++g) v += s_part[g * kTile + tid];      // fixed order
+        const long long f0 = s_pref[seq] + si.chunks_before(tile, walk);
+        const int slot = me - cta_of(f0, T, G);
+        p.ws_part[(((int64_t)seq * p.tiles_max + tile) * p.slots + slot) * kTile + tid] = v;
+      }
+      __syncthreads();
+      acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    advance(cc);
+  }
+  if (cur_seq >= 0) publish(cur_seq, done_in_seq);
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  __syncthreads();
+  if (!s_flag) return;
+
+  // ================= tails: Steps 4-6 on the whole row of every sequence this CTA completed ================
+  for (int seq = 0; seq < p.batch; ++seq) {
+    if (!((s_tailmask[seq >> 5] >> (seq & 31)) & 1u)) continue;
+    const SeqInfo si = seq_info(s_len, seq, p.B);
+    const int bq = si.bq, hi = bq + 1;
+    const int tt = max(0, min(__ldg(p.tau + seq), p.tau_max));     // (requested ahead of the dependent loads below)
+    const float rq = walk ? __ldg(p.r_prev + (int64_t)seq * mb + bq) : 1.f;
+    // partials per column tile = CTAs that share the tile's chunks (cta_of is monotone: one division per tile)
+    for (int tl = tid; tl <= si.a; tl += kThreads) {
+      const int nch = si.chunks(tl, walk);
+      int ns = 0;
+      if (nch > 0) {
+        const long long f0 = s_pref[seq] + si.chunks_before(tl, walk);
+        ns = cta_of(f0 + nch - 1, T, G) - cta_of(f0, T, G) + 1;
+      }
+      s_nslot[tl] = (unsigned char)min(ns, 255);
+    }
     const float* sc = p.ws_scores + (int64_t)seq * p.mbp;
     float lmax = -INFINITY;
     for (int j = tid; j < hi; j += kThreads) { const float v = __ldcg(sc + j); s_row[j] = v; lmax = fmaxf(lmax, v); }
@@ -259,208 +493,73 @@ decode_select_kernel(const Params p) {
       float e = 0.f;
       for (int j = tid; j < hi; j += kThreads) e += expf(s_row[j] - m);
       inv_l = 1.f / block_sum(e, s_red);
+    } else {
+      __syncthreads();                                // s_nslot
     }
     // W_new = A^s; Alg. 2 Step 4 cache update: the new row becomes row b_q of the cached W,
     // zeros right of the diagonal.  Row b_q is never read while b_q is the current block.
+    // Step 5: r_out[j] = sum_{m < b_q} r_prev[m] W[m][j] + r_prev[b_q] w[j], the partial sums in slot order;
+    // 8 columns x 4 slots of loads are in flight per thread (a dependent load per slot cost 5 us here).
     float* wrow = p.W + (int64_t)seq * p.w_stride_seq + (int64_t)bq * mb;
-    const float rq = walk ? __ldg(p.r_prev + (int64_t)seq * mb + bq) : 1.f;
-    const int base_g = s_pref[seq];
     float lamax = 0.f;
-    for (int j = tid; j < mb; j += kThreads) {
-      float w = 0.f, v = 0.f;
-      if (j < hi) {
-        const float sj = s_row[j];
-        w = swd::powi(soft ? expf(sj - m) * inv_l : sj, p.s);
-        // Step 5: r_out[j] = sum_{m < b_q} r_prev[m] W[m][j] + r_prev[b_q] w[j]; the partial sums in slot order
-        const int tile = j / kTile, nch = si.chunks(tile, walk);
-        if (nch > 0) {
-          const long long f0 = base_g + si.items_before(tile, walk);
-          const int i0 = cta_of(f0, T, G), i1 = cta_of(f0 + nch - 1, T, G);
-          const float* pp = p.ws_part + (((int64_t)seq * p.tiles_max + tile) * p.slots) * kTile + (j & (kTile - 1));
-          for (int sl = 0; sl <= i1 - i0; ++sl) v += __ldcg(pp + sl * kTile);
-        }
-        v = fmaf(rq, w, v);
-        s_row[j] = v;
-        lamax = fmaxf(lamax, fabsf(v));
+    constexpr int kCols = 8, kSl = 4;
+    for (int j0 = 0; j0 < mb; j0 += kCols * kThreads) {
+      float v[kCols];
+      int ns[kCols], nsmax = 0;
+      const float* pp[kCols];
+#pragma unroll
+      for (int c = 0; c < kCols; ++c) {
+        const int j = j0 + c * kThreads + tid;
+        v[c] = 0.f;
+        ns[c] = (j < hi) ? (int)s_nslot[j / kTile] : 0;
+        nsmax = max(nsmax, ns[c]);
+        pp[c] = p.ws_part + (((int64_t)seq * p.tiles_max + min(j, mb - 1) / kTile) * p.slots) * kTile + (j & (kTile - 1));
       }
-      wrow[j] = w;
+      nsmax = __reduce_max_sync(0xffffffffu, nsmax);
+      for (int s0 = 0; s0 < nsmax; s0 += kSl) {
+        float x[kSl][kCols];
+#pragma unroll
+        for (int e = 0; e < kSl; ++e)
+#pragma unroll
+          for (int c = 0; c < kCols; ++c) x[e][c] = (s0 + e < ns[c]) ? __ldcg(pp[c] + (s0 + e) * kTile) : 0.f;
+#pragma unroll
+        for (int e = 0; e < kSl; ++e)
+#pragma unroll
+          for (int c = 0; c < kCols; ++c) v[c] += x[e][c];                     // slot order
+      }
+#pragma unroll
+      for (int c = 0; c < kCols; ++c) {
+        const int j = j0 + c * kThreads + tid;
+        if (j < mb) {
+          float w = 0.f;
+          if (j < hi) {
+            const float sj = s_row[j];
+            w = swd::powi(soft ? expf(sj - m) * inv_l : sj, p.s);
+            const float r = fmaf(rq, w, v[c]);
+            s_row[j] = r;
+            lamax = fmaxf(lamax, fabsf(r));
+          }
+          wrow[j] = w;
+        }
+      }
     }
-    const float amax = block_max(lamax, s_red);           // (its barriers also publish s_row)
+    const float amax = block_max(lamax, s_red);       // (its barriers also publish s_row)
     const bool rescale = (p.flags & SW_ROWNORM) && amax > 0.f;
     float* ro = p.r_out + (int64_t)seq * mb;
     for (int j = tid; j < mb; j += kThreads) {
       float v = 0.f;
-      if (j < hi) { v = rescale ? s_row[j] / amax : s_row[j]; s_row[j] = v; }
+      if (j < hi) { v = rescale ? s_row[j] / amax : s_row[j]; s_row[j] = v; }   // the selection reads r_out's values
       ro[j] = v;
     }
     __syncthreads();
     // Step 6: S = TopK(r[0..b_q), tau - |forced|) U {b_q} (U {0})
-    const int tt = max(0, min(__ldg(p.tau + seq), p.tau_max));
     swsel::RowJob J = swsel::make_job(hi, bq, true, p.flags & SW_FORCE_FIRST, tt);
     const float* row = s_row;
     swsel::select_row([row](int j) { return row[j]; }, J, p.idx + (int64_t)seq * p.tau_max, p.tau_max,
                       p.count + seq, scratch);
-    if (tid == 0) p.ws_cnt[seq] = 0;                      // leave the counter ready for the next call
+    if (tid == 0) p.ws_cnt[seq] = 0;                  // leave the counter ready for the next call
     __syncthreads();
-  };
-
-  // this CTA has finished `done_in_seq` items of sequence `seq`: publish, and take the tail if it was the last
-  auto finish_seq = [&](int seq) {
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) {
-      const unsigned total = (unsigned)(s_pref[seq + 1] - s_pref[seq]);
-      const unsigned old = atomicAdd(p.ws_cnt + seq, (unsigned)done_in_seq);
-      // the tail runs after this CTA's streaming work (its row buffer aliases the ring)
-      if (old + (unsigned)done_in_seq == total) { s_tailmask[seq >> 5] |= 1u << (seq & 31); s_last = 1; }
-    }
-    done_in_seq = 0;
-  };
-
-  for (int it = 0; it < n_my; ++it) {
-    const SeqInfo& si = cc.si;
-    const int seq = cc.seq, tile = cc.tile, bq = si.bq;
-    if (seq != cur_seq) {
-      if (cur_seq >= 0) finish_seq(cur_seq);
-      cur_seq = seq;
-      __syncthreads();
-      if (walk) {
-        const float* rp = p.r_prev + (int64_t)seq * mb;
-        for (int i = tid; i < p.mbp + kChunkRows; i += kThreads) s_rprev[i] = (i <= bq) ? __ldg(rp + i) : 0.f;
-      }
-    }
-    if (cc.chunk == 0) {
-      // ---- score duty of (seq, tile): Steps 2-4 for columns [64 tile, 64 tile + 64) ------------------------
-      if (qt_seq != seq) {
-        head_mean(p.q, p.q_stride_seq, p.q_stride_head, p.h_q, seq);
-        swsk::sketch_tail<D>(s_vec, s_sign, s_cols, p.r, p.scale, s_qt);       // q~_t
-        qt_seq = seq;
-        __syncthreads();
-      }
-      if (tile == si.a) {
-        // the tile that holds column b_q owns the key-side update of Step 2
-        const int cnt = (__ldg(p.seqlens + seq) - 1) % p.B;                    // tokens already in block b_curr
-        float kbar_old = 0.f;
-        float* kb = p.kbar + ((int64_t)seq * mb + bq) * D;
-        if (cnt != 0 && tid < D) kbar_old = kb[tid];
-        head_mean(p.k, p.k_stride_seq, p.k_stride_head, p.h_kv, seq);
-        if (tid < D) {
-          const float avg = s_vec[tid];
-          const float mn = (cnt == 0) ? avg : ((float)cnt * kbar_old + avg) / (float)(cnt + 1);
-          kb[tid] = mn;                                                        // PAPER.md:811-813
-          s_vec[tid] = mn;
-        }
-        __syncthreads();
-        swsk::sketch_tail<D>(s_vec, s_sign, s_cols, p.r, p.scale, s_kt, p.ks + ((int64_t)seq * mb + bq) * p.r);
-        __syncthreads();
-      }
-      const float* ksb = p.ks + (int64_t)seq * mb * p.r;
-      float* sc = p.ws_scores + (int64_t)seq * p.mbp;
-      const int hi = bq + 1, col0 = tile * kTile;
-      const bool vec_scores = (p.r & 3) == 0 && q4 <= 32 && (reinterpret_cast<uintptr_t>(ksb) & 15u) == 0;
-      if (vec_scores) {
-        // q4 adjacent lanes share one column; all loads of the tile are issued before the first use
-        const int part = tid & (q4 - 1), per_pass = kThreads / q4;
-        const float4 qv = *reinterpret_cast<const float4*>(s_qt + part * 4);
-        constexpr int kU = 8;
-        for (int c0 = 0; c0 < kTile; c0 += kU * per_pass) {
-          float4 kv[kU];
-#pragma unroll
-          for (int u = 0; u < kU; ++u) {
-            const int cj = c0 + u * per_pass + tid / q4, j = col0 + cj;
-            kv[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (cj < kTile && j < hi) {
-              const float* kp2 = (j == bq) ? s_kt : ksb + (int64_t)j * p.r;
-              kv[u] = *reinterpret_cast<const float4*>(kp2 + part * 4);
-            }
-          }
-#pragma unroll
-          for (int u = 0; u < kU; ++u) {
-            if (c0 + u * per_pass >= kTile) break;                              // warp-uniform
-            const int cj = c0 + u * per_pass + tid / q4, j = col0 + cj;
-            float a = fmaf(qv.w, kv[u].w, fmaf(qv.z, kv[u].z, fmaf(qv.y, kv[u].y, qv.x * kv[u].x)));
-            for (int o = q4 >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-            if (part == 0 && cj < kTile && j < hi) sc[j] = a * p.inv_sqrt_r;
-          }
-        }
-      } else {
-        for (int cj = warp; cj < kTile; cj += kThreads / 32) {
-          const int j = col0 + cj;
-          if (j < hi) {
-            const float* kp = (j == bq) ? s_kt : ksb + (int64_t)j * p.r;
-            float a = 0.f;
-            for (int c = lane; c < p.r; c += 32) a = fmaf(s_qt[c], kp[c], a);
-            a = swd::warp_sum(a);
-            if (lane == 0) sc[j] = a * p.inv_sqrt_r;
-          }
-        }
-      }
-    }
-    const int nch = si.chunks(tile, walk);
-    if (nch > 0) {
-      // ---- Step 5, one chunk: acc[j] += sum_m r_prev[m] W[m][j] over rows [m0, m0 + 64) ---------------------
-      const int m0 = (tile + cc.chunk) * kTile;
-      const int rows = min(kChunkRows, bq - m0);
-      if (async) {
-        asm volatile("cp.async.wait_group %0;" ::"n"(kStages - 2) : "memory");   // chunk `consumed` has landed
-        __syncthreads();                              // ... for every thread; the previous chunk is fully consumed
-        issue_next();                                 // refill the stage the previous chunk occupied
-        const float* box = reinterpret_cast<const float*>(s_ring + (size_t)(consumed % kStages) * kChunkBytes);
-#pragma unroll
-        for (int u = 0; u < kChunkRows / kRowGroups; ++u) {
-          const int rr = rg + u * kRowGroups;
-          if (rr < rows) {
-            const float4 v = *reinterpret_cast<const float4*>(box + rr * kTile + cq * 4);
-            const float a = s_rprev[m0 + rr];
-            acc.x = fmaf(a, v.x, acc.x);
-            acc.y = fmaf(a, v.y, acc.y);
-            acc.z = fmaf(a, v.z, acc.z);
-            acc.w = fmaf(a, v.w, acc.w);
-          }
-        }
-        ++consumed;
-      } else {
-        __syncthreads();                              // s_rprev is complete
-        const float* Wm = p.W + (int64_t)seq * p.w_stride_seq;
-        const int c4 = tile * kTile + cq * 4;
-        for (int rr = rg; rr < rows; rr += kRowGroups) {
-          const float a = s_rprev[m0 + rr];
-          const float* wr = Wm + (int64_t)(m0 + rr) * mb;
-          if (c4 + 0 < mb) acc.x = fmaf(a, __ldg(wr + c4 + 0), acc.x);
-          if (c4 + 1 < mb) acc.y = fmaf(a, __ldg(wr + c4 + 1), acc.y);
-          if (c4 + 2 < mb) acc.z = fmaf(a, __ldg(wr + c4 + 2), acc.z);
-          if (c4 + 3 < mb) acc.w = fmaf(a, __ldg(wr + c4 + 3), acc.w);
-        }
-      }
-      acc_live = true;
-    }
-    ++done_in_seq;
-    const bool tile_ends = (it == n_my - 1) || (cc.chunk + 1 >= si.items(tile, walk));
-    if (tile_ends && acc_live) {
-      // one partial per (tile, CTA): slot = rank of this CTA among the CTAs that share the tile
-      *reinterpret_cast<float4*>(s_part + rg * kTile + cq * 4) = acc;
-      __syncthreads();
-      if (tid < kTile) {
-        float v = 0.f;
-#pragma unroll
-        for (int g = 0; g < kRowGroups; ++g) v += s_part[g * kTile + tid];      // fixed order
-        const long long f0 = s_pref[seq] + si.items_before(tile, walk);
-        const int slot = (int)blockIdx.x - cta_of(f0, T, G);
-        p.ws_part[(((int64_t)seq * p.tiles_max + tile) * p.slots + slot) * kTile + tid] = v;
-      }
-      __syncthreads();
-      acc = make_float4(0.f, 0.f, 0.f, 0.f);
-      acc_live = false;
-    }
-    advance(cc);
   }
-  const int seq_first = locate(g_begin).seq;
-  finish_seq(cur_seq);
-  asm volatile("cp.async.wait_group 0;" ::: "memory");
-  __syncthreads();
-  if (s_last)
-    for (int sq = seq_first; sq <= cur_seq; ++sq)
-      if ((s_tailmask[sq >> 5] >> (sq & 31)) & 1u) run_tail(sq);
 }
 
 }  // namespace
@@ -469,8 +568,8 @@ namespace sw {
 
 static int ds_grid(int batch, int max_blocks) {
   const int a = (max_blocks - 1) / kTile;
-  const long long items = (long long)batch * ((long long)a * (a + 1) / 2 + a + 1);
-  return (int)std::min<long long>(items, 2LL * num_sms());
+  const long long work = (long long)batch * ((long long)a * (a + 1) / 2 + a + 1);   // >= chunks, >= duties
+  return (int)std::min<long long>(work, 2LL * num_sms());
 }
 
 size_t decode_select_ws_bytes(int batch, int max_blocks) {
@@ -482,6 +581,8 @@ size_t decode_select_ws_bytes(int batch, int max_blocks) {
 int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st) {
   if (a.batch == 0) return SW_OK;
   if (a.batch > kMaxBatch) return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: batch %d > %d", a.batch, kMaxBatch);
+  if (cdiv(a.max_blocks, kTile) > kMaxTiles)
+    return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: max_blocks %d too large", a.max_blocks);
   const size_t need = decode_select_ws_bytes(a.batch, a.max_blocks);
   if (a.ws == nullptr || a.ws_bytes < need)
     return fail(SW_ERR_WORKSPACE, "sw_decode_select: workspace %zu < %zu bytes", a.ws_bytes, need);
@@ -509,11 +610,12 @@ int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st) {
   else if (a.q.dtype == SW_F32 && d == 64) kern = decode_select_kernel<float, 64>;
   else return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: dtype %d / d %d", a.q.dtype, d);
 
-  // cp.async stream of the cached W needs 16-byte aligned row pieces; otherwise the plain-load path runs
-  p.use_async = a.r_prev != nullptr && aligned16(a.W_cache) && (a.max_blocks & 3) == 0 && (a.stride_seq & 3) == 0;
+  // cp.async stream of the cached W (and of r_prev) needs 16-byte aligned row pieces; otherwise plain loads
+  p.use_async = a.r_prev != nullptr && aligned16(a.W_cache) && aligned16(a.r_prev) && (a.max_blocks & 3) == 0 &&
+                (a.stride_seq & 3) == 0;
 
   const size_t ring = std::max((size_t)kStages * kChunkBytes, sizeof(float) * (size_t)p.mbp);
-  const size_t smem = sizeof(float) * ((size_t)p.mbp + kChunkRows + kRowGroups * kTile) + 128 + ring;
+  const size_t smem = sizeof(float) * (2 * ((size_t)p.mbp + kChunkRows) + kRowGroups * kTile) + 128 + ring;
   if (smem > 200 * 1024) return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: max_blocks %d too large", a.max_blocks);
   if (int32_t rc = allow_dynamic_smem(kern, smem, "sw_decode_select smem attribute")) return rc;
   count_launch();

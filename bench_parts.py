@@ -15,7 +15,7 @@ from synth import gen
 CFG_IDX = 1
 METRIC = "prefill_tokens_per_s_per_layer_at_20pct_density"
 UNIT = "tokens/s"
-KERNELS = ["sketch_q", "sketch_k", "block_scores", "walk", "select", "attn"]
+KERNELS = ["sketch_qk", "block_scores", "walk", "select", "attn"]
 ROOT = os.path.dirname(os.path.abspath(__file__))
 
 
@@ -63,21 +63,20 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
             Q, K, V = Qs[layer], Ks[layer], Vs[layer]
             ev = events[layer] if events is not None else None
             if ev is not None: ev[0].record(stream)
-            pkg.sw_sketch(L, Q, pipe.signs, pipe.cols, pipe.r, pipe.sketch_scale, pipe.qs, pipe.qbar)
+            pkg.sw_sketch_qk(L, Q, K, pipe.signs, pipe.cols, pipe.r, pipe.sketch_scale, pipe.qs, pipe.ks, pipe.qbar,
+                             pipe.kbar)
             if ev is not None: ev[1].record(stream)
-            pkg.sw_sketch(L, K, pipe.signs, pipe.cols, pipe.r, pipe.sketch_scale, pipe.ks, pipe.kbar)
-            if ev is not None: ev[2].record(stream)
             pkg.sw_block_scores(L, pipe.qs, pipe.ks, pipe.r, pipe.s, pipe.flags, pipe.W, None)
-            if ev is not None: ev[3].record(stream)
+            if ev is not None: ev[2].record(stream)
             nxt = 0 if pipe.cur < 0 else 1 - pipe.cur
             pkg.sw_walk_update(L, pipe.R_cur, pipe.W, pipe.s, pipe.flags, pipe.R[nxt], pipe.walk_ws)
             pipe.cur = nxt
-            if ev is not None: ev[4].record(stream)
+            if ev is not None: ev[3].record(stream)
             pkg.sw_select_topk(L, pipe.R[nxt], pipe.tau, pipe.tau_max, pipe.flags, pipe.idx, pipe.count)
-            if ev is not None: ev[5].record(stream)
+            if ev is not None: ev[4].record(stream)
             pkg.sw_sparse_attn_prefill(L, Q, K, V, pipe.idx, pipe.count, pipe.tau_max, pipe.softmax_scale,
                                        pipe.flags, outs[layer & 1], None, pipe.attn_ws)
-            if ev is not None: ev[6].record(stream)
+            if ev is not None: ev[5].record(stream)
 
     def barrier():
         if dist is not None:
@@ -87,7 +86,7 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
     for _ in range(args.warmup):
         step()
     barrier()
-    events = [[[torch.cuda.Event(enable_timing=True) for _ in range(7)] for _ in range(layers)]
+    events = [[[torch.cuda.Event(enable_timing=True) for _ in range(len(KERNELS) + 1)] for _ in range(layers)]
               for _ in range(args.steps)]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     if rank == 0:
@@ -116,10 +115,10 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
     attn_flops = 4.0 * cfg.B * cfg.B * cfg.d * cfg.h_q * pairs          # full tile counted for the diagonal
     achieved = attn_flops / (attn_ms * 1e-3) / 1e12
     peak = peaks.get("bf16_tflops_sustained", peaks.get("bf16_tflops"))
-    sel_ms = sum(kern_ms[k] for k in KERNELS[:5])
+    sel_ms = sum(kern_ms[k] for k in KERNELS[:-1])
     layer_ms = ms_step / layers
     sketch_bytes = n * (cfg.h_q + cfg.h_kv) * cfg.d * 2
-    sketch_gbs = sketch_bytes / ((kern_ms["sketch_q"] + kern_ms["sketch_k"]) * 1e-3) / 1e9
+    sketch_gbs = sketch_bytes / (kern_ms["sketch_qk"] * 1e-3) / 1e9
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

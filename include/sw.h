@@ -106,6 +106,29 @@ typedef struct {
 SW_API int32_t sw_sketch(const sw_layout* L, const sw_tensor* x, const int8_t* signs, const int32_t* cols,
                   int32_t r, float scale, float* sketch, float* mean, sw_stream_t stream);
 
+/* Q and K of one layer in ONE launch (bit-identical to two sw_sketch calls: the same kernel body, the query
+ * blocks first and the key blocks behind them in one grid).  q: [total_tokens, h_q, d], k: [total_tokens, h_kv, d],
+ * same dtype and d.  qs / ks: dev fp32 [total_blocks, r] (written).  qbar / kbar: dev fp32 [total_blocks, d] or
+ * NULL. */
+SW_API int32_t sw_sketch_qk(const sw_layout* L, const sw_tensor* q, const sw_tensor* k, const int8_t* signs,
+                     const int32_t* cols, int32_t r, float scale, float* qs, float* ks, float* qbar, float* kbar,
+                     sw_stream_t stream);
+
+/* Sketch fused upstream ("custom CUDA kernels for block aggregation").  The
+ * token-space sketch is a plain sum, so whatever kernel produces (or copies) Q / K can leave the per-block sums
+ * behind and the 10 240 bytes per token that sw_sketch re-reads disappear:
+ *   sums[i, x] = sum over the heads and the valid tokens of block i of x[token, head, x]     (Steps 1-3, unscaled)
+ * sw_sketch_from_pooled finishes Alg. 1 Steps 3-4 from such sums: divide by heads * (valid
+ * tokens of the block) (P12), sign flip, FWHT, column pick, scale -- the same arithmetic as sw_sketch after its
+ * pooling loop.  sums: dev fp32 [total_blocks, d]; heads: how many heads were summed; sketch / mean as sw_sketch.
+ * sw_copy_pool is one such producer: it copies x (bf16 or fp32, strided) into the packed bf16 tensor dst
+ * [total_tokens, heads, d] (a KV-cache append, or the bf16 cast pre-pass of P17) and writes sums as a
+ * by-product of the same pass. */
+SW_API int32_t sw_sketch_from_pooled(const sw_layout* L, const float* sums, int32_t heads, int32_t d,
+                              const int8_t* signs, const int32_t* cols, int32_t r, float scale, float* sketch,
+                              float* mean, sw_stream_t stream);
+SW_API int32_t sw_copy_pool(const sw_layout* L, const sw_tensor* x, void* dst, float* sums, sw_stream_t stream);
+
 /* Decode form, Alg. 2 Steps 2-3: one new token per sequence.
  * x: [batch, heads, d] (stride_tok = stride between sequences).  seqlens: dev int32[batch],
  * length INCLUDING the new token (t).  Block b_curr = (t-1)/B gets the running mean

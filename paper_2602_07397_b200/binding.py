@@ -27,7 +27,7 @@ SW_WALK_AUTO, SW_WALK_SIMT, SW_WALK_TCGEN05 = 0, 1, 2
 SW_OP_SKETCH, SW_OP_BLOCK_SCORES, SW_OP_WALK_UPDATE, SW_OP_SELECT_TOPK, SW_OP_ATTN_PREFILL, SW_OP_ATTN_DECODE = range(6)
 
 EXPORTS = [
-    "sw_sketch", "sw_sketch_append", "sw_block_scores", "sw_block_scores_row", "sw_walk_update",
+    "sw_sketch", "sw_sketch_qk", "sw_sketch_from_pooled", "sw_copy_pool", "sw_sketch_append", "sw_block_scores", "sw_block_scores_row", "sw_walk_update",
     "sw_walk_update_row", "sw_select_topk", "sw_select_topk_row", "sw_decode_select", "sw_sparse_attn_prefill",
     "sw_sparse_attn_decode", "sw_sparse_attn_decode_paged", "sw_workspace_bytes", "sw_decode_workspace_bytes", "sw_decode_select_workspace_bytes", "sw_decode_num_splits",
     "sw_set_prefill_kernel", "sw_get_prefill_kernel_used", "sw_set_walk_kernel", "sw_get_walk_kernel_used",
@@ -62,6 +62,9 @@ def _load() -> C.CDLL:
     LP, TP = C.POINTER(_Layout), C.POINTER(_Tensor)
     sig = {
         "sw_sketch": (i32, [LP, TP, vp, vp, i32, f32, vp, vp, vp]),
+        "sw_sketch_qk": (i32, [LP, TP, TP, vp, vp, i32, f32, vp, vp, vp, vp, vp]),
+        "sw_sketch_from_pooled": (i32, [LP, vp, i32, i32, vp, vp, i32, f32, vp, vp, vp]),
+        "sw_copy_pool": (i32, [LP, TP, vp, vp, vp]),
         "sw_sketch_append": (i32, [i32, i32, i32, TP, vp, vp, vp, i32, f32, vp, vp, vp, vp]),
         "sw_block_scores": (i32, [LP, vp, vp, i32, i32, u32, vp, vp, vp]),
         "sw_block_scores_row": (i32, [i32, i32, i32, vp, vp, vp, i32, i32, u32, vp, vp]),
@@ -203,6 +206,28 @@ def sw_sketch(L: Layout, x, signs, cols, r: int, scale: float, sketch, mean=None
     lay, xt = L.c(), _tensor(x)
     _check(_lib.sw_sketch(C.byref(lay), C.byref(xt), _ptr(signs), _ptr(cols), r, scale, _ptr(sketch),
                           _ptr(mean), _stream(stream)))
+
+
+def sw_sketch_qk(L: Layout, q, k, signs, cols, r: int, scale: float, qs, ks, qbar=None, kbar=None, stream=None) -> None:
+    lay, qt, kt = L.c(), _tensor(q), _tensor(k)
+    _check(_lib.sw_sketch_qk(C.byref(lay), C.byref(qt), C.byref(kt), _ptr(signs), _ptr(cols), r, scale, _ptr(qs),
+                             _ptr(ks), _ptr(qbar), _ptr(kbar), _stream(stream)))
+
+
+def sw_sketch_from_pooled(L: Layout, sums, heads: int, signs, cols, r: int, scale: float, sketch, mean=None,
+                          stream=None) -> None:
+    """sums: fp32 [total_blocks, d] = per-block sums over heads and valid tokens (left behind by a producer)."""
+    lay = L.c()
+    _check(_lib.sw_sketch_from_pooled(C.byref(lay), _ptr(sums), heads, sums.shape[-1], _ptr(signs), _ptr(cols), r,
+                                      scale, _ptr(sketch), _ptr(mean), _stream(stream)))
+
+
+def sw_copy_pool(L: Layout, x, dst, sums, stream=None) -> None:
+    """dst: bf16 [total_tokens, heads, d] contiguous copy of x; sums: fp32 [total_blocks, d] (written)."""
+    lay, xt = L.c(), _tensor(x)
+    if dst.dtype != torch.bfloat16 or not dst.is_contiguous() or dst.shape != x.shape:
+        raise SwError(SW_ERR_INVALID_ARG, "dst must be a contiguous bf16 tensor of x's shape")
+    _check(_lib.sw_copy_pool(C.byref(lay), C.byref(xt), _ptr(dst), _ptr(sums), _stream(stream)))
 
 
 def sw_sketch_append(batch, block, max_blocks, x, seqlens, signs, cols, r, scale, mean, sketch, tok_sketch,

@@ -122,6 +122,40 @@ SW_API int32_t sw_sketch(const sw_layout* L, const sw_tensor* x, const int8_t* s
   return launch_sketch(*L, *x, signs, cols, r, scale, sketch, mean, (cudaStream_t)stream);
 }
 
+SW_API int32_t sw_sketch_qk(const sw_layout* L, const sw_tensor* q, const sw_tensor* k, const int8_t* signs,
+                     const int32_t* cols, int32_t r, float scale, float* qs, float* ks, float* qbar, float* kbar,
+                     sw_stream_t stream) {
+  SW_TRY(validate_layout(L));
+  SW_TRY(validate_tensor(q, "q"));
+  SW_TRY(validate_tensor(k, "k"));
+  SW_REQUIRE(q->dtype == k->dtype && q->d == k->d, SW_ERR_UNSUPPORTED, "q / k dtype or head_dim differ");
+  SW_TRY(validate_sketch_params(q, cols, r));
+  SW_REQUIRE(qs != nullptr && ks != nullptr, SW_ERR_INVALID_ARG, "qs / ks is NULL");
+  SW_TRY(check_arch());
+  return launch_sketch_qk(*L, *q, *k, signs, cols, r, scale, qs, ks, qbar, kbar, (cudaStream_t)stream);
+}
+
+SW_API int32_t sw_copy_pool(const sw_layout* L, const sw_tensor* x, void* dst, float* sums, sw_stream_t stream) {
+  SW_TRY(validate_layout(L));
+  SW_TRY(validate_tensor(x, "x"));
+  SW_REQUIRE(dst != nullptr && sums != nullptr, SW_ERR_INVALID_ARG, "dst / sums is NULL");
+  SW_REQUIRE(aligned16(dst) && dst != x->ptr, SW_ERR_INVALID_ARG, "dst must be 16-byte aligned and not alias x");
+  SW_TRY(check_arch());
+  return launch_copy_pool(*L, *x, reinterpret_cast<__nv_bfloat16*>(dst), sums, (cudaStream_t)stream);
+}
+
+SW_API int32_t sw_sketch_from_pooled(const sw_layout* L, const float* sums, int32_t heads, int32_t d,
+                              const int8_t* signs, const int32_t* cols, int32_t r, float scale, float* sketch,
+                              float* mean, sw_stream_t stream) {
+  SW_TRY(validate_layout(L));
+  SW_REQUIRE(sums != nullptr && sketch != nullptr && cols != nullptr, SW_ERR_INVALID_ARG, "sums / sketch / cols is NULL");
+  SW_REQUIRE(d == 64 || d == 128, SW_ERR_UNSUPPORTED, "d = %d not in {64,128}", d);
+  SW_REQUIRE(heads >= 1, SW_ERR_INVALID_ARG, "heads = %d", heads);
+  SW_REQUIRE(is_pow2(r) && r <= d, SW_ERR_INVALID_ARG, "r = %d must be a power of two <= d = %d", r, d);
+  SW_TRY(check_arch());
+  return launch_sketch_from_pooled(*L, sums, heads, d, signs, cols, r, scale, sketch, mean, (cudaStream_t)stream);
+}
+
 SW_API int32_t sw_sketch_append(int32_t batch, int32_t block, int32_t max_blocks, const sw_tensor* x,
                          const int32_t* seqlens, const int8_t* signs, const int32_t* cols, int32_t r,
                          float scale, float* mean, float* sketch, float* tok_sketch, sw_stream_t stream) {

@@ -45,6 +45,13 @@ int32_t validate_tensor(const sw_tensor* t, const char* name);
 // ---- kernel launchers (one per translation unit) ---------------------------------------
 int32_t launch_sketch(const sw_layout& L, const sw_tensor& x, const int8_t* signs, const int32_t* cols,
                       int r, float scale, float* sketch, float* mean, cudaStream_t st);
+int32_t launch_sketch_qk(const sw_layout& L, const sw_tensor& q, const sw_tensor& k, const int8_t* signs,
+                         const int32_t* cols, int r, float scale, float* qs, float* ks, float* qbar, float* kbar,
+                         cudaStream_t st);
+int32_t launch_copy_pool(const sw_layout& L, const sw_tensor& x, __nv_bfloat16* dst, float* sums, cudaStream_t st);
+int32_t launch_sketch_from_pooled(const sw_layout& L, const float* sums, int heads, int d, const int8_t* signs,
+                                  const int32_t* cols, int r, float scale, float* sketch, float* mean,
+                                  cudaStream_t st);
 int32_t launch_sketch_append(int batch, int block, int max_blocks, const sw_tensor& x,
                              const int32_t* seqlens, const int8_t* signs, const int32_t* cols, int r,
                              float scale, float* mean, float* sketch, float* tok_sketch, cudaStream_t st);

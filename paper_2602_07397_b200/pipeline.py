@@ -62,8 +62,12 @@ class PrefillPipeline:
     def select(self, Q: torch.Tensor, K: torch.Tensor, stream=None) -> None:
         """Steps 1-7: sketch -> block scores -> walk -> top-tau (idx / count updated in place)."""
         L = self.L
-        sw.sw_sketch(L, Q, self.signs, self.cols, self.r, self.sketch_scale, self.qs, self.qbar, stream)
-        sw.sw_sketch(L, K, self.signs, self.cols, self.r, self.sketch_scale, self.ks, self.kbar, stream)
+        if Q.dtype == K.dtype:
+            sw.sw_sketch_qk(L, Q, K, self.signs, self.cols, self.r, self.sketch_scale, self.qs, self.ks, self.qbar,
+                            self.kbar, stream)
+        else:
+            sw.sw_sketch(L, Q, self.signs, self.cols, self.r, self.sketch_scale, self.qs, self.qbar, stream)
+            sw.sw_sketch(L, K, self.signs, self.cols, self.r, self.sketch_scale, self.ks, self.kbar, stream)
         sw.sw_block_scores(L, self.qs, self.ks, self.r, self.s, self.flags, self.W, self.A, stream)
         nxt = 0 if self.cur < 0 else 1 - self.cur
         sw.sw_walk_update(L, self.R_cur, self.W, self.s, self.flags, self.R[nxt], self.walk_ws, stream)

@@ -85,6 +85,81 @@ def test_sketch_strided_and_nosigns(sw):
     assert rowwise_close(sk.cpu().numpy(), ref)
 
 
+def _ref_sketch(xn, seqlens, B, H):
+    ref_mean, ref_sk, lo = [], [], 0
+    for n in seqlens:
+        m = O.block_mean(O.head_mean(xn[lo:lo + n]), B)
+        ref_mean.append(m); ref_sk.append(O.sketch(m, H)); lo += n
+    return np.concatenate(ref_mean), np.concatenate(ref_sk)
+
+
+@pytest.mark.parametrize("seqlens,h_q,h_kv,d,r,B,dtype", [
+    ((1024,), 1, 1, 64, 16, 64, torch.float32),                 # cfg 1
+    ((2048 + 19,), 32, 8, 128, 64, 64, torch.bfloat16),         # cfg 2 recipe, ragged tail (a 19-token block)
+    ((192, 700, 1024, 5), 32, 8, 128, 64, 64, torch.bfloat16),  # varlen; a 5-token sequence
+    ((1000,), 12, 3, 128, 32, 128, torch.bfloat16),             # B = 128
+    ((300,), 6, 6, 64, 64, 64, torch.bfloat16),                 # h_q = h_kv, d = 64
+])
+def test_sketch_qk_one_launch(sw, seqlens, h_q, h_kv, d, r, B, dtype):
+    """sw_sketch_qk (Q and K in one launch) against the oracle's head mean -> block mean -> SRHT (Alg. 1 Steps
+    1-4), and against two sw_sketch calls."""
+    torch.manual_seed(2)
+    T = sum(seqlens)
+    q = (torch.randn(T, h_q, d) + 0.3).to(dtype); k = (torch.randn(T, h_kv, d) - 0.2).to(dtype)
+    signs, cols, H = H_of(d, r)
+    L = sw.make_layout(seqlens, B)
+    nb = L.total_blocks
+    out = {n: torch.full((nb, w), float("nan"), device="cuda") for n, w in [("qs", r), ("ks", r), ("qbar", d), ("kbar", d)]}
+    launches0 = sw.sw_launch_count()
+    sw.sw_sketch_qk(L, q.cuda(), k.cuda(), dev(signs), dev(cols), r, 1 / math.sqrt(r), out["qs"], out["ks"], out["qbar"],
+                    out["kbar"])
+    assert sw.sw_launch_count() - launches0 == 1
+    for x, sk, mean, heads in [(q, "qs", "qbar", h_q), (k, "ks", "kbar", h_kv)]:
+        ref_mean, ref_sk = _ref_sketch(gen.to_numpy_f64(x), seqlens, B, H)
+        assert rowwise_close(out[mean].cpu().numpy(), ref_mean)
+        assert rowwise_close(out[sk].cpu().numpy(), ref_sk)
+        one = torch.empty(nb, r, device="cuda")
+        sw.sw_sketch(L, x.cuda(), dev(signs), dev(cols), r, 1 / math.sqrt(r), one, None)
+        assert rowwise_close(out[sk].cpu().numpy(), one.cpu().numpy().astype(np.float64), rel=1e-5)
+
+
+@pytest.mark.parametrize("seqlens,heads,d,r,B,dtype", [
+    ((2048 + 19,), 8, 128, 64, 64, torch.bfloat16),
+    ((192, 700, 5), 32, 128, 64, 64, torch.bfloat16),
+    ((1024,), 1, 64, 16, 64, torch.float32),                    # fp32 source: the bf16 cast pre-pass of P17
+])
+def test_sketch_from_pooled_sums_of_a_producer(sw, seqlens, heads, d, r, B, dtype):
+    """Sketch fused upstream (SURVEY 8(f) item 4): sw_copy_pool copies x and leaves the per-block sums behind;
+    sw_sketch_from_pooled turns them into the sketch sw_sketch computes by re-reading x.  Both against the oracle."""
+    torch.manual_seed(3)
+    T = sum(seqlens)
+    big = (torch.randn(T, heads + 1, d) + 0.25).to(dtype).cuda()
+    x = big[:, 1:]                                              # strided source
+    signs, cols, H = H_of(d, r)
+    L = sw.make_layout(seqlens, B)
+    nb = L.total_blocks
+    dst = torch.full((T, heads, d), float("nan"), dtype=torch.bfloat16, device="cuda")
+    sums = torch.full((nb, d), float("nan"), device="cuda")
+    sw.sw_copy_pool(L, x, dst, sums)
+    assert torch.equal(dst, x.to(torch.bfloat16))               # the copy (round-to-nearest cast for fp32)
+    xn = gen.to_numpy_f64(x)
+    lo, blk = 0, 0
+    for n in seqlens:                                           # sums = plain sums over heads and valid tokens
+        for i in range(O.num_blocks(n, B)):
+            ref = xn[lo + i * B: lo + min((i + 1) * B, n)].sum(axis=(0, 1))
+            assert np.abs(sums[blk].cpu().numpy() - ref).max() <= 1e-3 * max(np.abs(ref).max(), 1.0)
+            blk += 1
+        lo += n
+    sk = torch.full((nb, r), float("nan"), device="cuda"); mean = torch.full((nb, d), float("nan"), device="cuda")
+    sw.sw_sketch_from_pooled(L, sums, heads, dev(signs), dev(cols), r, 1 / math.sqrt(r), sk, mean)
+    ref_mean, ref_sk = _ref_sketch(xn, seqlens, B, H)
+    assert rowwise_close(mean.cpu().numpy(), ref_mean)
+    assert rowwise_close(sk.cpu().numpy(), ref_sk)
+    direct = torch.empty(nb, r, device="cuda")
+    sw.sw_sketch(L, x, dev(signs), dev(cols), r, 1 / math.sqrt(r), direct, None)
+    assert rowwise_close(sk.cpu().numpy(), direct.cpu().numpy().astype(np.float64), rel=1e-5)
+
+
 # ------------------------------------------------------------------------------ block scores
 FLAG_SETS = [O.DEFAULT_FLAGS, O.DEFAULT_FLAGS & ~O.SCORE_SOFTMAX, O.DEFAULT_FLAGS & ~O.CAUSAL,
              O.DEFAULT_FLAGS | O.POW_MATRIX, 0]

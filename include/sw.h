@@ -174,11 +174,12 @@ SW_API int32_t sw_block_scores_row(int32_t batch, int32_t block, int32_t max_blo
  *   SW_ROWNORM: each row of R_out is divided by its max-abs (P9)
  *   SW_CAUSAL: both operands are lower triangular; the strictly upper part of R_out is 0.
  * R_prev, W, R_out: dev fp32 packed (cu_sq).  R_out must not alias R_prev or W.
- * ws: dev scratch of sw_workspace_bytes(SW_OP_WALK_UPDATE, ...) bytes = one ping-pong matrix
+ * ws: dev scratch (128-byte aligned) of sw_workspace_bytes(SW_OP_WALK_UPDATE, ...) bytes = one ping-pong matrix
  * (batch * max_blocks^2 floats; required with SW_POW_MATRIX and s > 1, else SW_ERR_WORKSPACE) followed
- * by the hi/lo operand images of the tensor-core kernel (4 b^2 floats; only when batch = 1, b >= 256
- * and b % 4 == 0).  ws may be NULL or shorter otherwise: the fp32 SIMT kernel then runs (see
- * sw_set_walk_kernel).  Both kernels keep ~fp32 accuracy (the tcgen05 one by 3xTF32 splitting).
+ * by the hi/lo operand images of the tensor-core kernel (max_blocks >= 256; any batch: the sequences are
+ * stacked with one row pitch, ~4 (total_blocks + 128 (batch + 1)) max_blocks floats).  ws may be NULL or
+ * shorter otherwise: the fp32 SIMT kernel then runs (see sw_set_walk_kernel).  Both kernels keep ~fp32
+ * accuracy (the tcgen05 one by 3xTF32 splitting).
  * ------------------------------------------------------------------------------------- */
 SW_API int32_t sw_walk_update(const sw_layout* L, const float* R_prev, const float* W, int32_t s,
                        uint32_t flags, float* R_out, void* ws, size_t ws_bytes, sw_stream_t stream);
@@ -209,6 +210,22 @@ SW_API int32_t sw_walk_update_row(int32_t batch, int32_t block, int32_t max_bloc
  * ------------------------------------------------------------------------------------- */
 SW_API int32_t sw_select_topk(const sw_layout* L, const float* R, const int32_t* tau, int32_t tau_max,
                        uint32_t flags, int32_t* idx, int32_t* count, sw_stream_t stream);
+
+/* Prefill selection, fused -- Alg. 1 Steps 5-7: exactly the sequence
+ *   sw_block_scores(qs, ks -> W, A); sw_walk_update(R_prev, W -> R_out); sw_select_topk(R_out -> idx, count)
+ * with the same arguments and the same results up to fp32 summation order, in at most three launches
+ * (SURVEY 8(f) item 1): (1) score tiles, row softmax and power in one kernel that keeps a strip of rows on chip
+ * and, for the tensor-core walk, writes W directly as the hi / lo TF32 operand images next to the fp32 W (the
+ * images of R_prev come from extra CTAs of the same grid); (2) the walk GEMM (tcgen05 3xTF32 for
+ * max_blocks >= 512, any batch; fp32 SIMT below), which leaves the raw product in R_out; (3) the per-row
+ * max-abs rescale (P9) and the top-tau of the same row in one kernel, in place.  R_prev = NULL: R_out = W
+ * (P10) and launch (2) is skipped.  W: dev fp32 packed (written; what a decode cache keeps).  A: optional.
+ * ws: as sw_walk_update (sw_workspace_bytes(SW_OP_WALK_UPDATE)); without it the SIMT GEMM runs.  With
+ * SW_POW_MATRIX and s > 1 (s successive products) the three plain calls are issued instead. */
+SW_API int32_t sw_prefill_select(const sw_layout* L, const float* qs, const float* ks, int32_t r, int32_t s,
+                          uint32_t flags, const float* R_prev, float* R_out, float* W, float* A,
+                          const int32_t* tau, int32_t tau_max, int32_t* idx, int32_t* count, void* ws,
+                          size_t ws_bytes, sw_stream_t stream);
 
 /* Decode form, Alg. 2 Step 6: S = TopK(r[0..b_q), tau-1) U {b_q}, block 0
  * also forced with SW_FORCE_FIRST.  r: dev fp32 [batch, max_blocks].
@@ -310,10 +327,10 @@ SW_API int32_t sw_get_prefill_kernel_used(void);
 
 /* Kernel choice of sw_walk_update (process-wide; for tests and benchmarks -- both are CUDA kernels of
  * this library).
- *   SW_WALK_AUTO (default): the tcgen05 3xTF32 GEMM when batch = 1, b >= 512, b % 4 == 0 and the
- *                    workspace holds its operand images, else the fp32 SIMT GEMM.
+ *   SW_WALK_AUTO (default): the tcgen05 3xTF32 GEMM when max_blocks >= 512 and the workspace holds its
+ *                    operand images, else the fp32 SIMT GEMM.
  *   SW_WALK_SIMT: always the SIMT kernel.
- *   SW_WALK_TCGEN05: the tcgen05 kernel (b >= 256); SW_ERR_UNSUPPORTED / SW_ERR_WORKSPACE when the
+ *   SW_WALK_TCGEN05: the tcgen05 kernel (max_blocks >= 256); SW_ERR_UNSUPPORTED / SW_ERR_WORKSPACE when the
  *                    problem or the workspace does not fit it.
  * Returns the previous setting, or SW_ERR_INVALID_ARG.  sw_get_walk_kernel_used(): the kernel the last
  * sw_walk_update of this thread launched (SW_WALK_SIMT / SW_WALK_TCGEN05; 0 = none yet). */

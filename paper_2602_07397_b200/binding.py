@@ -28,7 +28,7 @@ SW_OP_SKETCH, SW_OP_BLOCK_SCORES, SW_OP_WALK_UPDATE, SW_OP_SELECT_TOPK, SW_OP_AT
 
 EXPORTS = [
     "sw_sketch", "sw_sketch_qk", "sw_sketch_from_pooled", "sw_copy_pool", "sw_sketch_append", "sw_block_scores", "sw_block_scores_row", "sw_walk_update",
-    "sw_walk_update_row", "sw_select_topk", "sw_select_topk_row", "sw_decode_select", "sw_sparse_attn_prefill",
+    "sw_walk_update_row", "sw_select_topk", "sw_select_topk_row", "sw_prefill_select", "sw_decode_select", "sw_sparse_attn_prefill",
     "sw_sparse_attn_decode", "sw_sparse_attn_decode_paged", "sw_workspace_bytes", "sw_decode_workspace_bytes", "sw_decode_select_workspace_bytes", "sw_decode_num_splits",
     "sw_set_prefill_kernel", "sw_get_prefill_kernel_used", "sw_set_walk_kernel", "sw_get_walk_kernel_used",
     "sw_last_error", "sw_version", "sw_launch_count",
@@ -71,6 +71,7 @@ def _load() -> C.CDLL:
         "sw_walk_update": (i32, [LP, vp, vp, i32, u32, vp, vp, sz, vp]),
         "sw_walk_update_row": (i32, [i32, i32, i32, vp, vp, i64, vp, vp, u32, vp, vp]),
         "sw_select_topk": (i32, [LP, vp, vp, i32, u32, vp, vp, vp]),
+        "sw_prefill_select": (i32, [LP, vp, vp, i32, i32, u32, vp, vp, vp, vp, vp, i32, vp, vp, vp, sz, vp]),
         "sw_select_topk_row": (i32, [i32, i32, i32, vp, vp, vp, i32, u32, vp, vp, vp]),
         "sw_decode_select": (i32, [i32, i32, i32, TP, TP, vp, vp, vp, i32, f32, i32, u32, vp, vp, vp, i64, vp, vp,
                                    vp, i32, vp, vp, vp, sz, vp]),
@@ -263,6 +264,14 @@ def sw_select_topk(L: Layout, R, tau, tau_max, flags, idx, count, stream=None) -
     lay = L.c()
     _check(_lib.sw_select_topk(C.byref(lay), _ptr(R), _ptr(tau), tau_max, flags, _ptr(idx), _ptr(count),
                                _stream(stream)))
+
+
+def sw_prefill_select(L: Layout, qs, ks, r, s, flags, R_prev, R_out, W, A, tau, tau_max, idx, count, ws=None,
+                      stream=None) -> None:
+    lay = L.c()
+    _check(_lib.sw_prefill_select(C.byref(lay), _ptr(qs), _ptr(ks), r, s, flags, _ptr(R_prev), _ptr(R_out), _ptr(W),
+                                  _ptr(A), _ptr(tau), tau_max, _ptr(idx), _ptr(count), _ptr(ws),
+                                  0 if ws is None else ws.numel() * ws.element_size(), _stream(stream)))
 
 
 def sw_select_topk_row(batch, block, max_blocks, r, seqlens, tau, tau_max, flags, idx, count, stream=None) -> None:

@@ -236,6 +236,50 @@ SW_API int32_t sw_select_topk(const sw_layout* L, const float* R, const int32_t*
   return launch_select(*L, R, tau, tau_max, flags, idx, count, (cudaStream_t)stream);
 }
 
+SW_API int32_t sw_prefill_select(const sw_layout* L, const float* qs, const float* ks, int32_t r, int32_t s,
+                          uint32_t flags, const float* R_prev, float* R_out, float* W, float* A,
+                          const int32_t* tau, int32_t tau_max, int32_t* idx, int32_t* count, void* ws,
+                          size_t ws_bytes, sw_stream_t stream) {
+  SW_TRY(validate_layout(L));
+  SW_REQUIRE(qs && ks && R_out && W && tau && idx && count, SW_ERR_INVALID_ARG, "NULL argument");
+  SW_REQUIRE(R_out != R_prev && R_out != W, SW_ERR_INVALID_ARG, "R_out must not alias its inputs");
+  SW_REQUIRE(r >= 1 && r <= 128, SW_ERR_INVALID_ARG, "r = %d out of [1,128]", r);
+  SW_REQUIRE(s >= 1 && tau_max >= 1, SW_ERR_INVALID_ARG, "s = %d / tau_max = %d", s, tau_max);
+  const size_t pp_bytes = walk_pp_bytes(*L);
+  const bool products = (flags & SW_POW_MATRIX) && s > 1;
+  if (products)
+    SW_REQUIRE(ws != nullptr && ws_bytes >= pp_bytes, SW_ERR_WORKSPACE, "sw_prefill_select: workspace %zu < %zu bytes",
+               ws_bytes, pp_bytes);
+  SW_TRY(check_arch());
+  cudaStream_t st = (cudaStream_t)stream;
+  if (L->total_blocks == 0) return SW_OK;
+  if (products || !scores_fused_supported(*L, r)) {
+    // s successive products (P4 matrix reading) or a sketch the fused score kernel does not take: the plain chain
+    SW_TRY(launch_block_scores(*L, qs, ks, r, s, flags, W, A, st));
+    SW_TRY(launch_walk(*L, R_prev, W, s, flags, R_out, ws, ws_bytes, st));
+    return launch_select(*L, R_out, tau, tau_max, flags, idx, count, st);
+  }
+  const int causal = (flags & SW_CAUSAL) ? 1 : 0;
+  int32_t which = SW_WALK_SIMT;
+  if (R_prev != nullptr) {
+    const bool have_ws = ws != nullptr && (reinterpret_cast<uintptr_t>(ws) & 127u) == 0 && ws_bytes > pp_bytes;
+    which = choose_walk_kernel(*L, have_ws ? ws_bytes - pp_bytes : 0);
+    if (which < 0) return which;
+  }
+  WalkImages im = {};
+  const bool tc = which == SW_WALK_TCGEN05;
+  if (tc) im = walk_images(*L, reinterpret_cast<uint8_t*>(ws) + pp_bytes);
+  note_walk_kernel(which);
+  // launch 1: W = A^s (+ R^0 = W^0 for the first layer, + the operand images of W and R_prev for the GEMM)
+  SW_TRY(launch_scores_fused(*L, qs, ks, r, s, flags, W, A, R_prev ? nullptr : R_out, tc ? &im : nullptr, R_prev, st));
+  // launch 2: the raw product R_prev W
+  if (R_prev != nullptr)
+    SW_TRY(tc ? launch_walk_tc(*L, im, R_out, causal, /*zero_upper=*/false, st)
+              : launch_walk_simt(*L, R_prev, W, R_out, causal, st));
+  // launch 3: row rescale (P9) + top-tau, in place
+  return launch_rescale_select(*L, R_out, tau, tau_max, flags, idx, count, st);
+}
+
 SW_API int32_t sw_select_topk_row(int32_t batch, int32_t block, int32_t max_blocks, const float* r,
                            const int32_t* seqlens, const int32_t* tau, int32_t tau_max, uint32_t flags,
                            int32_t* idx, int32_t* count, sw_stream_t stream) {
@@ -284,7 +328,7 @@ SW_API size_t sw_workspace_bytes(int32_t op, const sw_layout* L, int32_t h_q, in
                           int32_t tau_max, int32_t dtype) {
   switch (op) {
     case SW_OP_WALK_UPDATE:
-      return L ? (size_t)L->batch * L->max_blocks * L->max_blocks * sizeof(float) + walk_tc_ws_bytes(*L) : 0;
+      return L ? walk_pp_bytes(*L) + walk_tc_ws_bytes(*L) : 0;
     case SW_OP_ATTN_PREFILL:
       if (!L || dtype != SW_F32) return 0;
       return cast_bytes(L->total_tokens, h_q, d) + 2 * cast_bytes(L->total_tokens, h_kv, d);

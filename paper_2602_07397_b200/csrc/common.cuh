@@ -62,10 +62,35 @@ int32_t launch_block_scores_row(int batch, int block, int max_blocks, const floa
                                 cudaStream_t st);
 int32_t launch_walk(const sw_layout& L, const float* R_prev, const float* W, int s, uint32_t flags,
                     float* R_out, void* ws, size_t ws_bytes, cudaStream_t st);
+// workspace of sw_walk_update = [ping-pong matrix of the matrix-power reading | operand images of the tcgen05 GEMM]
+static inline size_t walk_pp_bytes(const sw_layout& L) {
+  return ((size_t)L.batch * L.max_blocks * L.max_blocks * sizeof(float) + 255) & ~(size_t)255;
+}
 bool walk_tc_supported(const sw_layout& L);
 size_t walk_tc_ws_bytes(const sw_layout& L);
-int32_t launch_walk_tc(int b, const float* A, const float* Bm, float* dst, float* ws4, bool split_R, bool split_W,
-                       int causal, cudaStream_t st);
+struct WalkImages {               // hi / lo TF32 operand images of the tensor-core walk GEMM (walk_images.cuh)
+  float *r_hi, *r_lo, *w_hi, *w_lo;
+  int pitch, rows;
+};
+WalkImages walk_images(const sw_layout& L, void* ws_images);
+int32_t launch_split_tf32(const sw_layout& L, const float* R, const float* W, const WalkImages& im, int causal,
+                          cudaStream_t st);
+int32_t launch_walk_tc(const sw_layout& L, const WalkImages& im, float* dst, int causal, bool zero_upper,
+                       cudaStream_t st);
+int32_t launch_walk_simt(const sw_layout& L, const float* R_prev, const float* W, float* dst, int causal,
+                         cudaStream_t st);
+// fused selection chain (scores.cu / select.cu): scores + softmax + power (+ operand images) in one launch,
+// row rescale + top-tau in one launch
+int32_t launch_scores_fused(const sw_layout& L, const float* qs, const float* ks, int r, int s, uint32_t flags,
+                            float* W, float* A, float* W2, const WalkImages* im, const float* R_prev,
+                            cudaStream_t st);
+bool scores_fused_supported(const sw_layout& L, int r);
+int32_t launch_rescale_select(const sw_layout& L, float* R, const int32_t* tau, int tau_max, uint32_t flags,
+                              int32_t* idx, int32_t* count, cudaStream_t st);
+int32_t choose_walk_kernel(const sw_layout& L, size_t images_bytes);
+void note_walk_kernel(int32_t which);
+int32_t launch_copy_rows(const sw_layout& L, const float* src, float* dst, cudaStream_t st);
+int32_t launch_row_rescale(const sw_layout& L, float* R, cudaStream_t st);
 int32_t set_walk_kernel(int32_t which);
 int32_t walk_kernel_used();
 int32_t launch_walk_row(int batch, int block, int max_blocks, const float* r_prev, float* W_cache,

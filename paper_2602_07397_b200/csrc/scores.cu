@@ -6,6 +6,7 @@
 // row-sweeping CTAs of the first version, 56 -> ~8 us); (2) score_rows_kernel - one warp per row reads
 // its row twice from L2 (max / sum-exp, then normalise) and writes A and W = A^s in place.
 #include "common.cuh"
+#include "walk_images.cuh"
 
 namespace {
 
@@ -171,6 +172,162 @@ score_rows_kernel(int s, uint32_t flags, const int32_t* __restrict__ cu_blocks, 
   }
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Fused form: scores, row softmax, power and -- for the tensor-core walk -- the hi / lo
+// TF32 operand images of W in ONE launch, with the images of R_prev written by extra CTAs of the same grid.
+// One CTA per strip of kFRows = 8 query rows: the strip's raw scores stay in shared memory ([8][b] floats)
+// while the key sketches stream through a cp.async double buffer in 64-column tiles (float4 shared-memory reads,
+// row stride r + 4 floats: conflict free), then warp w turns row w into A, W = A^s and the image rows.  W is
+// written once and never re-read by this step; split_tf32_kernel and its pass over W and R are gone.
+constexpr int kFRows = 8;
+constexpr int kFCols = 64;
+
+struct FusedParams {
+  const float *qs, *ks;
+  int r, s;
+  uint32_t flags;
+  const int32_t* cu_blocks;
+  const int64_t* cu_sq;
+  float *W, *A, *W2;                 // packed outputs (A, W2 may be NULL; W2 = a second copy of W: R^0 = W^0)
+  float *whi, *wlo;                  // operand images of W, or NULL
+  const float* R_prev;               // packed; split into rhi / rlo by the CTAs behind the strips, or NULL
+  float *rhi, *rlo;
+  int pitch, n_strips, lds;          // lds: row stride of the score strip in shared memory (floats)
+  float inv_sqrt_r;
+};
+
+__global__ void __launch_bounds__(kThreads)
+score_fused_kernel(const FusedParams p) {
+  extern __shared__ __align__(16) float smem[];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int seq = blockIdx.z;
+  const int blk0 = __ldg(p.cu_blocks + seq);
+  const int b = __ldg(p.cu_blocks + seq + 1) - blk0;
+  const bool causal = p.flags & SW_CAUSAL, soft = p.flags & SW_SCORE_SOFTMAX, matpow = p.flags & SW_POW_MATRIX;
+  const bool images = p.whi != nullptr;
+  const int rows_all = images ? swimg::pad_rows(b) : b;       // image rows include the zero padding
+  const int rbase = images ? swimg::row_base(p.cu_blocks, seq) : 0;
+
+  if ((int)blockIdx.x >= p.n_strips) {
+    // ---- operand images of R_prev: one warp per row ------------------------------------------------------
+    const int i = ((int)blockIdx.x - p.n_strips) * kFRows + warp;
+    if (i < rows_all)
+      swimg::split_row(p.R_prev + __ldg(p.cu_sq + seq) + (int64_t)i * b, i, b, p.pitch, causal,
+                       p.rhi + (int64_t)(rbase + i) * p.pitch, p.rlo + (int64_t)(rbase + i) * p.pitch, lane, 32);
+    return;
+  }
+  const int i0 = blockIdx.x * kFRows;
+  if (i0 >= rows_all) return;
+  const int r = p.r, r4 = r >> 2, ldk = r + 4;
+  float* s_q = smem;                                          // [kFRows][r]
+  float* s_k = s_q + kFRows * r;                              // [2][kFCols][r + 4]
+  float* s_S = s_k + 2 * kFCols * ldk;                        // [kFRows][lds]
+  const int nrows = max(0, min(kFRows, b - i0));
+
+  if (nrows > 0) {
+    const int hi_col = causal ? min(b, i0 + kFRows) : b;      // columns some row of the strip can see
+    const int nct = (hi_col + kFCols - 1) / kFCols;
+    auto load_k = [&](int ct, int buf) {
+      float* dst = s_k + buf * kFCols * ldk;
+      for (int i = tid; i < kFCols * r4; i += kThreads) {
+        const int kk = i / r4, c = (i - kk * r4) * 4;
+        const int j = ct * kFCols + kk;
+        const float* src = p.ks + (int64_t)(blk0 + min(j, b - 1)) * r + c;
+        const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst + kk * ldk + c);
+        const int sz = (j < b) ? 16 : 0;                      // rows past the sequence: zero fill
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(sz) : "memory");
+      }
+      asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    load_k(0, 0);
+    for (int i = tid; i < kFRows * r4; i += kThreads) {
+      const int rr = i / r4, c = (i - rr * r4) * 4;
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (rr < nrows) v = *reinterpret_cast<const float4*>(p.qs + (int64_t)(blk0 + i0 + rr) * r + c);
+      *reinterpret_cast<float4*>(s_q + rr * r + c) = v;
+    }
+    const int col = tid & (kFCols - 1), rg = tid / kFCols;    // rows 2 rg, 2 rg + 1 of the strip
+    for (int ct = 0; ct < nct; ++ct) {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      __syncthreads();                                        // tile ct landed; tile ct - 1 fully consumed
+      if (ct + 1 < nct) load_k(ct + 1, (ct + 1) & 1);
+      const float* kp = s_k + (ct & 1) * kFCols * ldk + col * ldk;
+      const float* q0 = s_q + (2 * rg) * r;
+      const float* q1 = q0 + r;
+      float a0 = 0.f, a1 = 0.f;
+      for (int c = 0; c < r; c += 4) {
+        const float4 kv = *reinterpret_cast<const float4*>(kp + c);
+        const float4 x0 = *reinterpret_cast<const float4*>(q0 + c);
+        const float4 x1 = *reinterpret_cast<const float4*>(q1 + c);
+        a0 = fmaf(x0.x, kv.x, a0); a0 = fmaf(x0.y, kv.y, a0); a0 = fmaf(x0.z, kv.z, a0); a0 = fmaf(x0.w, kv.w, a0);
+        a1 = fmaf(x1.x, kv.x, a1); a1 = fmaf(x1.y, kv.y, a1); a1 = fmaf(x1.z, kv.z, a1); a1 = fmaf(x1.w, kv.w, a1);
+      }
+      s_S[(2 * rg) * p.lds + ct * kFCols + col] = a0 * p.inv_sqrt_r;
+      s_S[(2 * rg + 1) * p.lds + ct * kFCols + col] = a1 * p.inv_sqrt_r;
+    }
+    __syncthreads();
+  }
+
+  // ---- row phase: warp w owns row i0 + w -------------------------------------------------------------------
+  const int i = i0 + warp;
+  if (i >= rows_all) return;
+  float* ihi = images ? p.whi + (int64_t)(rbase + i) * p.pitch : nullptr;
+  float* ilo = images ? p.wlo + (int64_t)(rbase + i) * p.pitch : nullptr;
+  const int icols = images ? swimg::row_cols(i, p.pitch, causal) : 0;
+  if (i >= b) {                                               // padding row of the images
+    for (int j = lane * 4; j < icols; j += 128) {
+      *reinterpret_cast<float4*>(ihi + j) = make_float4(0.f, 0.f, 0.f, 0.f);
+      *reinterpret_cast<float4*>(ilo + j) = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    return;
+  }
+  const float* srow = s_S + warp * p.lds;
+  const int hi = causal ? i + 1 : b;                          // unmasked columns [0, hi)
+  float m = 0.f, inv_l = 1.f;
+  if (soft) {
+    float mx = -INFINITY;
+    for (int j = lane; j < hi; j += 32) mx = fmaxf(mx, srow[j]);
+    m = swd::warp_max(mx);
+    float e = 0.f;
+    for (int j = lane; j < hi; j += 32) e += expf(srow[j] - m);
+    inv_l = 1.f / swd::warp_sum(e);
+  }
+  const int64_t off = __ldg(p.cu_sq + seq) + (int64_t)i * b;
+  float* wrow = p.W + off;
+  float* arow = p.A ? p.A + off : nullptr;
+  float* w2row = p.W2 ? p.W2 + off : nullptr;
+  const bool vec = (b & 3) == 0 && (reinterpret_cast<uintptr_t>(wrow) & 15u) == 0 &&
+                   (arow == nullptr || (reinterpret_cast<uintptr_t>(arow) & 15u) == 0) &&
+                   (w2row == nullptr || (reinterpret_cast<uintptr_t>(w2row) & 15u) == 0);
+  const int jend = max((b + 3) & ~3, icols);
+  for (int j = lane * 4; j < jend; j += 128) {
+    float a[4], w[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      a[e] = 0.f;
+      if (j + e < hi) a[e] = soft ? expf(srow[j + e] - m) * inv_l : srow[j + e];
+      w[e] = matpow ? a[e] : swd::powi(a[e], p.s);            // powi(0, s) = 0 for s >= 1: masked entries stay 0
+    }
+    if (j < b) {
+      if (vec) {
+        if (arow) *reinterpret_cast<float4*>(arow + j) = make_float4(a[0], a[1], a[2], a[3]);
+        *reinterpret_cast<float4*>(wrow + j) = make_float4(w[0], w[1], w[2], w[3]);
+        if (w2row) *reinterpret_cast<float4*>(w2row + j) = make_float4(w[0], w[1], w[2], w[3]);
+      } else {
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+          if (j + e < b) { if (arow) arow[j + e] = a[e]; wrow[j + e] = w[e]; if (w2row) w2row[j + e] = w[e]; }
+      }
+    }
+    if (j < icols) {
+      float4 h, l;
+      swimg::split4(make_float4(w[0], w[1], w[2], w[3]), h, l);
+      *reinterpret_cast<float4*>(ihi + j) = h;
+      *reinterpret_cast<float4*>(ilo + j) = l;
+    }
+  }
+}
+
 // Decode row (Alg. 2 Steps 3-4): one CTA per sequence.
 __global__ void __launch_bounds__(256)
 block_scores_row_kernel(const float* __restrict__ q_tok, const float* __restrict__ ks,
@@ -236,6 +393,7 @@ static size_t scores_smem_bytes() {
 int32_t launch_block_scores(const sw_layout& L, const float* qs, const float* ks, int r, int s,
                             uint32_t flags, float* W, float* A, cudaStream_t st) {
   if (L.total_blocks == 0) return SW_OK;
+  if (scores_fused_supported(L, r)) return launch_scores_fused(L, qs, ks, r, s, flags, W, A, nullptr, nullptr, nullptr, st);
   const size_t smem = scores_smem_bytes();
   if (int32_t rc = allow_dynamic_smem(score_tile_kernel, smem, "sw_block_scores smem attribute")) return rc;
   dim3 grid(cdiv(L.max_blocks, kCols), cdiv(L.max_blocks, kRows), L.batch);
@@ -244,6 +402,38 @@ int32_t launch_block_scores(const sw_layout& L, const float* qs, const float* ks
   score_rows_kernel<<<cdiv(L.total_blocks, kThreads / 32), kThreads, 0, st>>>(s, flags, L.cu_blocks, L.cu_sq, L.batch,
                                                                              W, A);
   return check_launch("sw_block_scores");
+}
+
+static size_t fused_smem_bytes(int max_blocks, int r, int* lds_out) {
+  const int lds = ((max_blocks + kFCols - 1) / kFCols) * kFCols + 4;   // whole 64-column tiles are written
+  if (lds_out) *lds_out = lds;
+  return sizeof(float) * ((size_t)kFRows * r + 2 * (size_t)kFCols * (r + 4) + (size_t)kFRows * lds);
+}
+
+bool scores_fused_supported(const sw_layout& L, int r) {
+  return r >= 4 && (r & 3) == 0 && r <= kRMax && fused_smem_bytes(L.max_blocks, r, nullptr) <= 200 * 1024;
+}
+
+// W (and A) of sw_block_scores, plus -- when im != NULL -- the operand images of W and, when R_prev != NULL too,
+// those of R_prev, in one launch.
+int32_t launch_scores_fused(const sw_layout& L, const float* qs, const float* ks, int r, int s, uint32_t flags,
+                            float* W, float* A, float* W2, const WalkImages* im, const float* R_prev,
+                            cudaStream_t st) {
+  if (L.total_blocks == 0) return SW_OK;
+  FusedParams p;
+  p.qs = qs; p.ks = ks; p.r = r; p.s = s; p.flags = flags; p.cu_blocks = L.cu_blocks; p.cu_sq = L.cu_sq;
+  p.W = W; p.A = A; p.W2 = W2;
+  p.whi = im ? im->w_hi : nullptr; p.wlo = im ? im->w_lo : nullptr;
+  p.R_prev = im ? R_prev : nullptr; p.rhi = im ? im->r_hi : nullptr; p.rlo = im ? im->r_lo : nullptr;
+  p.pitch = im ? im->pitch : 0;
+  p.n_strips = cdiv(im ? swimg::pad_rows(L.max_blocks) : L.max_blocks, kFRows);
+  p.inv_sqrt_r = 1.0f / sqrtf((float)r);
+  const size_t smem = fused_smem_bytes(L.max_blocks, r, &p.lds);
+  if (int32_t rc = allow_dynamic_smem(score_fused_kernel, smem, "sw_block_scores(fused) smem attribute")) return rc;
+  dim3 grid(p.n_strips * (p.R_prev ? 2 : 1), 1, L.batch);
+  count_launch();
+  score_fused_kernel<<<grid, kThreads, smem, st>>>(p);
+  return check_launch("sw_block_scores(fused)");
 }
 
 int32_t launch_block_scores_row(int batch, int block, int max_blocks, const float* q_tok, const float* ks,

@@ -3,6 +3,8 @@
 // fp32 SIMT GEMM (true fp32 FMA: selection parity needs ~1e-5 relative accuracy) that exploits
 // the block-causal structure: R_prev and W are lower triangular, so output tile (ti, tj) is zero
 // for tj > ti and its reduction runs over k-tiles tj..ti only (about 1/3 of the dense 2 b^3).
+#include <atomic>
+
 #include "common.cuh"
 
 namespace {
@@ -198,54 +200,82 @@ vec_rescale_kernel(float* __restrict__ r, int max_blocks) {
 
 namespace sw {
 
-static int32_t g_walk_kernel = SW_WALK_AUTO;
+static std::atomic<int32_t> g_walk_kernel{SW_WALK_AUTO};      // process-wide test / benchmark switch
 static thread_local int32_t g_walk_used = 0;
-constexpr int kWalkTcMinBlocks = 512;      // SW_WALK_AUTO: tensor-core path from this b on
+constexpr int kWalkTcMinBlocks = 512;      // SW_WALK_AUTO: tensor-core path from this max_blocks on
 
-int32_t set_walk_kernel(int32_t which) { const int32_t prev = g_walk_kernel; g_walk_kernel = which; return prev; }
+int32_t set_walk_kernel(int32_t which) { return g_walk_kernel.exchange(which); }
 int32_t walk_kernel_used() { return g_walk_used; }
+void note_walk_kernel(int32_t which) { g_walk_used = which; }
+
+// SW_WALK_SIMT / SW_WALK_TCGEN05 for this problem and workspace (images_bytes = bytes available for the operand
+// images), or a negative status when SW_WALK_TCGEN05 was forced and does not fit.
+int32_t choose_walk_kernel(const sw_layout& L, size_t images_bytes) {
+  const int32_t want = g_walk_kernel.load();
+  const size_t tc_bytes = walk_tc_ws_bytes(L);
+  const bool fits = tc_bytes > 0 && images_bytes >= tc_bytes;
+  if (want == SW_WALK_TCGEN05 && !fits)
+    return fail(tc_bytes == 0 ? SW_ERR_UNSUPPORTED : SW_ERR_WORKSPACE,
+                "sw_walk_update: SW_WALK_TCGEN05 needs max_blocks >= 256 and %zu bytes of workspace for the operand images",
+                tc_bytes);
+  if (want == SW_WALK_SIMT || !fits) return SW_WALK_SIMT;
+  return (want == SW_WALK_TCGEN05 || L.max_blocks >= kWalkTcMinBlocks) ? SW_WALK_TCGEN05 : SW_WALK_SIMT;
+}
+
+int32_t launch_walk_simt(const sw_layout& L, const float* R_prev, const float* W, float* dst, int causal,
+                         cudaStream_t st) {
+  dim3 grid(cdiv(L.max_blocks, TN), cdiv(L.max_blocks, TM), L.batch);
+  count_launch();
+  walk_gemm_kernel<<<grid, kThreads, 0, st>>>(R_prev, W, dst, L.cu_blocks, L.cu_sq, causal);
+  return check_launch("sw_walk_update");
+}
+
+int32_t launch_copy_rows(const sw_layout& L, const float* src, float* dst, cudaStream_t st) {
+  count_launch();
+  row_rescale_kernel<<<L.total_blocks, 128, 0, st>>>(src, dst, L.cu_blocks, L.cu_sq, L.batch, 0);
+  return check_launch("sw_walk_update");
+}
+
+int32_t launch_row_rescale(const sw_layout& L, float* R, cudaStream_t st) {
+  count_launch();
+  row_rescale_kernel<<<L.total_blocks, 128, 0, st>>>(R, R, L.cu_blocks, L.cu_sq, L.batch, 1);
+  return check_launch("sw_walk_update");
+}
 
 int32_t launch_walk(const sw_layout& L, const float* R_prev, const float* W, int s, uint32_t flags,
                     float* R_out, void* ws, size_t ws_bytes, cudaStream_t st) {
   if (L.total_blocks == 0) return SW_OK;
   const int causal = (flags & SW_CAUSAL) ? 1 : 0;
-  const int rownorm = (flags & SW_ROWNORM) ? 1 : 0;
   const int nprod = (flags & SW_POW_MATRIX) ? s : 1;
   // workspace = [ping-pong matrix (batch * max_blocks^2 floats) | hi/lo images of the tcgen05 path]
-  const size_t pp_bytes = (size_t)L.batch * L.max_blocks * L.max_blocks * sizeof(float);
-  const size_t tc_bytes = walk_tc_ws_bytes(L);
-  bool use_tc = false;
-  if (g_walk_kernel != SW_WALK_SIMT && tc_bytes > 0 && ws != nullptr && ws_bytes >= pp_bytes + tc_bytes)
-    use_tc = (g_walk_kernel == SW_WALK_TCGEN05) || L.total_blocks >= kWalkTcMinBlocks;
-  if (g_walk_kernel == SW_WALK_TCGEN05 && !use_tc)
-    return fail(tc_bytes == 0 ? SW_ERR_UNSUPPORTED : SW_ERR_WORKSPACE,
-                "sw_walk_update: SW_WALK_TCGEN05 needs batch = 1, b >= 256, b %% 4 == 0 and %zu bytes of workspace",
-                pp_bytes + tc_bytes);
-  float* ws4 = use_tc ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(ws) + pp_bytes) : nullptr;
-  g_walk_used = use_tc ? SW_WALK_TCGEN05 : SW_WALK_SIMT;
-  dim3 grid(cdiv(L.max_blocks, TN), cdiv(L.max_blocks, TM), L.batch);
+  const size_t pp_bytes = walk_pp_bytes(L);
+  const bool have_ws = ws != nullptr && (reinterpret_cast<uintptr_t>(ws) & 127u) == 0 && ws_bytes > pp_bytes;
+  const int32_t which = choose_walk_kernel(L, have_ws ? ws_bytes - pp_bytes : 0);
+  if (which < 0) return which;
+  const bool use_tc = which == SW_WALK_TCGEN05;
+  WalkImages im = {};
+  if (use_tc) im = walk_images(L, reinterpret_cast<uint8_t*>(ws) + pp_bytes);
+  g_walk_used = which;
   const float* cur = R_prev;
   bool w_split = false;
   for (int k = 1; k <= nprod; ++k) {
     // the last product must land in R_out; alternate with the workspace before that
     float* dst = ((nprod - k) % 2 == 0) ? R_out : reinterpret_cast<float*>(ws);
+    int32_t rc;
     if (cur == nullptr) {                   // identity * W = W
-      count_launch();
-      row_rescale_kernel<<<L.total_blocks, 128, 0, st>>>(W, dst, L.cu_blocks, L.cu_sq, L.batch, 0);
+      rc = launch_copy_rows(L, W, dst, st);
     } else if (use_tc) {
-      const int32_t rc = launch_walk_tc(L.total_blocks, cur, W, dst, ws4, true, !w_split, causal, st);
-      if (rc != SW_OK) return rc;
+      rc = launch_split_tf32(L, cur, w_split ? nullptr : W, im, causal, st);
+      if (rc == SW_OK) rc = launch_walk_tc(L, im, dst, causal, /*zero_upper=*/true, st);
       w_split = true;
     } else {
-      count_launch();
-      walk_gemm_kernel<<<grid, kThreads, 0, st>>>(cur, W, dst, L.cu_blocks, L.cu_sq, causal);
+      rc = launch_walk_simt(L, cur, W, dst, causal, st);
     }
+    if (rc != SW_OK) return rc;
     cur = dst;
   }
-  if (rownorm) count_launch();
-  if (rownorm)
-    row_rescale_kernel<<<L.total_blocks, 128, 0, st>>>(R_out, R_out, L.cu_blocks, L.cu_sq, L.batch, 1);
-  return check_launch("sw_walk_update");
+  if (flags & SW_ROWNORM) return launch_row_rescale(L, R_out, st);
+  return SW_OK;
 }
 
 int32_t launch_walk_row(int batch, int block, int max_blocks, const float* r_prev, float* W_cache,

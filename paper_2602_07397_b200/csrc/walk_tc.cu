@@ -5,13 +5,16 @@
 // (2^-11) does not give, so each fp32 operand is split  x = hi + lo,  hi = x with the low 13 mantissa
 // bits cleared (exactly a TF32 number), lo = x - hi (exact in fp32, |lo| < 2^-10 |x|), and the product is
 //     R W  ~=  R_hi W_hi + R_hi W_lo + R_lo W_hi          (3xTF32; dropped term <= 2^-20 relative)
-// accumulated in fp32 in TMEM.  The split is a pre-pass (split_tf32_kernel) into the caller's workspace:
-// converting inside the GEMM would double the shared-memory traffic of a kernel that is already bound by
-// the tensor core's operand reads (SS MMA at M = N = 128 reads 128 B/clk).
+// accumulated in fp32 in TMEM.  The hi / lo images live in the caller's workspace (walk_images.cuh: all
+// sequences of a batch stacked with one row pitch, zero padded, so that ONE tensor map per operand serves a
+// varlen batch); they are written by split_tf32_kernel here, or directly by the fused score kernel
+// (scores.cu).  Converting inside the GEMM would double the shared-memory traffic of a kernel that is already
+// bound by the tensor core's operand reads (SS MMA at M = N = 128 reads 128 B/clk).
 //
-// GEMM: one CTA per 128x128 output tile (ti, tj).  With SW_CAUSAL both operands are lower triangular,
-// so tiles with tj > ti are zero-filled and the reduction of tile (ti, tj) runs over k in
-// [128 tj, 128 (ti+1)) only; tiles are issued longest first.  K step = 32 fp32 (128-byte rows):
+// GEMM: one CTA per 128x128 output tile (sequence, ti, tj).  With SW_CAUSAL both operands are lower
+// triangular, so the reduction of tile (ti, tj) runs over k in [128 tj, 128 (ti+1)) only and tiles with
+// tj > ti are zero (written only when asked: the fused selection path fills them itself); tiles are issued
+// longest first.  K step = 32 fp32 (128-byte rows):
 //   A = R_hi / R_lo [128 x 32]  K-major,  SWIZZLE_128B        (one TMA box each)
 //   B = W_hi / W_lo [32 x 128]  MN-major, SWIZZLE_128B_ATOM_32B (four 32x32 TMA boxes each; 32-bit
 //       MN-major operands need the 32-byte-atom swizzle, see sm100.cuh)
@@ -22,6 +25,7 @@
 // Warps: 0 = TMA producer, 1 = MMA issuer, 2-5 = epilogue (TMEM -> registers -> global, causal mask).
 #include "common.cuh"
 #include "sm100.cuh"
+#include "walk_images.cuh"
 
 namespace {
 
@@ -35,28 +39,22 @@ constexpr int kThreads = 192;
 constexpr int kAcc = 4;                              // TMEM accumulators (k-step ks adds into ks % 4)
 constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/;
 
-// x = hi + lo with hi a TF32 number (low 13 mantissa bits zero) and lo = x - hi exact.
+// x = hi + lo with hi a TF32 number (low 13 mantissa bits zero) and lo = x - hi exact.  Packed per-sequence
+// matrices (cu_sq) -> stacked, pitched, zero-padded images.  grid = (padded rows, 2 = R / W, batch).
 __global__ void __launch_bounds__(256)
 split_tf32_kernel(const float* __restrict__ R, const float* __restrict__ W, float* __restrict__ Rhi,
-                  float* __restrict__ Rlo, float* __restrict__ Whi, float* __restrict__ Wlo, int b, int causal) {
-  const int i = blockIdx.x;
+                  float* __restrict__ Rlo, float* __restrict__ Whi, float* __restrict__ Wlo,
+                  const int32_t* __restrict__ cu_blocks, const int64_t* __restrict__ cu_sq, int pitch, int causal) {
+  const int i = blockIdx.x, seq = blockIdx.z;
   const float* src = blockIdx.y ? W : R;
   float* hi = blockIdx.y ? Whi : Rhi;
   float* lo = blockIdx.y ? Wlo : Rlo;
   if (src == nullptr) return;
-  // the GEMM reads whole 128-wide diagonal tiles, so cover the row up to the end of its diagonal tile
-  const int lim = causal ? min(b, (i / BM + 1) * BM) : b;
-  const int64_t off = (int64_t)i * b;
-  for (int j = threadIdx.x * 4; j < lim; j += 256 * 4) {
-    const float4 x = *reinterpret_cast<const float4*>(src + off + j);
-    float4 h, l;
-    h.x = __uint_as_float(__float_as_uint(x.x) & 0xffffe000u); l.x = x.x - h.x;
-    h.y = __uint_as_float(__float_as_uint(x.y) & 0xffffe000u); l.y = x.y - h.y;
-    h.z = __uint_as_float(__float_as_uint(x.z) & 0xffffe000u); l.z = x.z - h.z;
-    h.w = __uint_as_float(__float_as_uint(x.w) & 0xffffe000u); l.w = x.w - h.w;
-    *reinterpret_cast<float4*>(hi + off + j) = h;
-    *reinterpret_cast<float4*>(lo + off + j) = l;
-  }
+  const int b = __ldg(cu_blocks + seq + 1) - __ldg(cu_blocks + seq);
+  if (i >= swimg::pad_rows(b)) return;
+  const int64_t irow = (int64_t)(swimg::row_base(cu_blocks, seq) + i) * pitch;
+  swimg::split_row(src + __ldg(cu_sq + seq) + (int64_t)i * b, i, b, pitch, causal, hi + irow, lo + irow,
+                   threadIdx.x, 256);
 }
 
 // kind::tf32, fp32 accumulate: [4,6) D fmt = 1 (f32), [7,10) A fmt = 2 (tf32), [10,13) B fmt = 2,
@@ -79,8 +77,10 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* m, 
 }
 
 struct Params {
-  float* out;
-  int b, nt, causal, n_work;      // nt = tiles per side, n_work = tiles that run the GEMM
+  float* out;                     // packed per-sequence matrices (cu_sq)
+  const int32_t* cu_blocks;
+  const int64_t* cu_sq;
+  int causal, zero_upper;         // zero_upper: also write the strictly upper tiles (as zeros)
 };
 
 __global__ void __launch_bounds__(kThreads, 1)
@@ -88,7 +88,12 @@ walk_tc_kernel(const __grid_constant__ CUtensorMap map_rhi, const __grid_constan
                const __grid_constant__ CUtensorMap map_whi, const __grid_constant__ CUtensorMap map_wlo,
                const Params p) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int b = p.b, nt = p.nt;
+  const int seq = blockIdx.y;
+  const int b = __ldg(p.cu_blocks + seq + 1) - __ldg(p.cu_blocks + seq);
+  const int nt = (b + BM - 1) / BM;
+  const int n_work = p.causal ? nt * (nt + 1) / 2 : nt * nt;
+  float* out = p.out + __ldg(p.cu_sq + seq);
+  const int rbase = swimg::row_base(p.cu_blocks, seq);
 
   // ---- tile of this CTA: GEMM tiles longest first (by ti - tj), then the zero tiles -------------
   int ti, tj;
@@ -96,13 +101,15 @@ walk_tc_kernel(const __grid_constant__ CUtensorMap map_rhi, const __grid_constan
   {
     int w = blockIdx.x;
     if (!p.causal) {
+      if (w >= n_work) return;
       ti = w / nt; tj = w - ti * nt;
-    } else if (w < p.n_work) {
+    } else if (w < n_work) {
       int dgap = nt - 1;                     // tiles with ti - tj = dgap: nt - dgap of them
       while (w >= nt - dgap) { w -= nt - dgap; --dgap; }
       tj = w; ti = tj + dgap;
     } else {
-      w -= p.n_work;                         // strictly upper tiles, row-major
+      w -= n_work;                           // strictly upper tiles, row-major
+      if (!p.zero_upper || w >= nt * (nt - 1) / 2) return;
       zero_tile = true;
       ti = 0;
       while (w >= nt - 1 - ti) { w -= nt - 1 - ti; ++ti; }
@@ -110,10 +117,18 @@ walk_tc_kernel(const __grid_constant__ CUtensorMap map_rhi, const __grid_constan
     }
   }
   const int row0 = ti * BM, col0 = tj * BN;
+  const bool vec_out = (b & 3) == 0 && (reinterpret_cast<uintptr_t>(out) & 15u) == 0;
   if (zero_tile) {
     for (int e = threadIdx.x; e < BM * (BN / 4); e += kThreads) {
       const int r = row0 + e / (BN / 4), c = col0 + (e % (BN / 4)) * 4;
-      if (r < b && c < b) *reinterpret_cast<float4*>(p.out + (int64_t)r * b + c) = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (r < b) {
+        if (vec_out) {
+          if (c < b) *reinterpret_cast<float4*>(out + (int64_t)r * b + c) = make_float4(0.f, 0.f, 0.f, 0.f);
+        } else {
+          for (int f = 0; f < 4; ++f)
+            if (c + f < b) out[(int64_t)r * b + c + f] = 0.f;
+        }
+      }
     }
     return;
   }
@@ -154,12 +169,12 @@ walk_tc_kernel(const __grid_constant__ CUtensorMap map_rhi, const __grid_constan
         const uint32_t dst = sTiles + st * kStageBytes;
         const int k = k_begin + ks * BK;
         mbar_arrive_expect_tx(FULL(st), kStageBytes);
-        tma_load_2d(dst, &map_rhi, FULL(st), k, row0);
-        tma_load_2d(dst + kTileBytes, &map_rlo, FULL(st), k, row0);
+        tma_load_2d(dst, &map_rhi, FULL(st), k, rbase + row0);
+        tma_load_2d(dst + kTileBytes, &map_rlo, FULL(st), k, rbase + row0);
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
-          tma_load_2d(dst + 2 * kTileBytes + c * 4096, &map_whi, FULL(st), col0 + c * 32, k);
-          tma_load_2d(dst + 3 * kTileBytes + c * 4096, &map_wlo, FULL(st), col0 + c * 32, k);
+          tma_load_2d(dst + 2 * kTileBytes + c * 4096, &map_whi, FULL(st), col0 + c * 32, rbase + k);
+          tma_load_2d(dst + 3 * kTileBytes + c * 4096, &map_wlo, FULL(st), col0 + c * 32, rbase + k);
         }
       }
     }
@@ -208,17 +223,22 @@ walk_tc_kernel(const __grid_constant__ CUtensorMap map_rhi, const __grid_constan
         for (int e = 0; e < 32; ++e) v[e] = __float_as_uint(__uint_as_float(v[e]) + __uint_as_float(w[e]));
       }
       if (r < b) {
-        float* dst = p.out + (int64_t)r * b + col0 + ch * 32;
+        float* dst = out + (int64_t)r * b + col0 + ch * 32;
 #pragma unroll
         for (int e = 0; e < 32; e += 4) {
           const int c = col0 + ch * 32 + e;
-          if (c < b) {                                   // b % 4 == 0: a float4 is inside or outside
-            float4 o;
-            o.x = (p.causal && c + 0 > r) ? 0.f : __uint_as_float(v[e + 0]);
-            o.y = (p.causal && c + 1 > r) ? 0.f : __uint_as_float(v[e + 1]);
-            o.z = (p.causal && c + 2 > r) ? 0.f : __uint_as_float(v[e + 2]);
-            o.w = (p.causal && c + 3 > r) ? 0.f : __uint_as_float(v[e + 3]);
-            *reinterpret_cast<float4*>(dst + e) = o;
+          float4 o;
+          o.x = (p.causal && c + 0 > r) ? 0.f : __uint_as_float(v[e + 0]);
+          o.y = (p.causal && c + 1 > r) ? 0.f : __uint_as_float(v[e + 1]);
+          o.z = (p.causal && c + 2 > r) ? 0.f : __uint_as_float(v[e + 2]);
+          o.w = (p.causal && c + 3 > r) ? 0.f : __uint_as_float(v[e + 3]);
+          if (vec_out) {
+            if (c < b) *reinterpret_cast<float4*>(dst + e) = o;     // b % 4 == 0: a float4 is inside or outside
+          } else {
+            if (c + 0 < b) dst[e + 0] = o.x;
+            if (c + 1 < b) dst[e + 1] = o.y;
+            if (c + 2 < b) dst[e + 2] = o.z;
+            if (c + 3 < b) dst[e + 3] = o.w;
           }
         }
       }
@@ -229,12 +249,12 @@ walk_tc_kernel(const __grid_constant__ CUtensorMap map_rhi, const __grid_constan
   if (warp == 2) tmem_dealloc<kAcc * BN>(tm);
 }
 
-// [rows, cols] fp32 row-major -> 2-D map (cols, rows), box = (32 cols = 128 B, box_rows), 128-byte swizzle
-bool make_map_f32(CUtensorMap* map, const float* base, int rows, int cols, int box_rows, bool atom32) {
+// stacked images [rows, pitch] fp32 -> 2-D map (pitch, rows), box = (32 cols = 128 B, box_rows), 128-byte swizzle
+bool make_map_f32(CUtensorMap* map, const float* base, int rows, int pitch, int box_rows, bool atom32) {
   sm100host::EncodeTiledFn fn = sm100host::encode_fn();
   if (!fn) return false;
-  cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
-  cuuint64_t strides[1] = {(cuuint64_t)cols * 4};
+  cuuint64_t dims[2] = {(cuuint64_t)pitch, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)pitch * 4};
   cuuint32_t box[2] = {32, (cuuint32_t)box_rows};
   cuuint32_t estr[2] = {1, 1};
   return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
@@ -247,36 +267,49 @@ bool make_map_f32(CUtensorMap* map, const float* base, int rows, int cols, int b
 namespace sw {
 
 bool walk_tc_supported(const sw_layout& L) {
-  return L.batch == 1 && L.max_blocks == L.total_blocks && L.total_blocks >= 256 && L.total_blocks % 4 == 0 &&
-         sm100host::encode_fn() != nullptr;
+  return L.batch >= 1 && L.max_blocks >= 256 && sm100host::encode_fn() != nullptr;
+}
+
+WalkImages walk_images(const sw_layout& L, void* ws_images) {
+  WalkImages im;
+  im.pitch = swimg::pitch_of(L.max_blocks);
+  im.rows = swimg::rows_bound(L.total_blocks, L.batch);
+  const size_t n = (size_t)im.rows * im.pitch;
+  float* f = reinterpret_cast<float*>(ws_images);
+  im.r_hi = f; im.r_lo = f + n; im.w_hi = f + 2 * n; im.w_lo = f + 3 * n;
+  return im;
 }
 
 size_t walk_tc_ws_bytes(const sw_layout& L) {
-  return walk_tc_supported(L) ? (size_t)4 * L.total_blocks * L.total_blocks * sizeof(float) : 0;
+  if (!walk_tc_supported(L)) return 0;
+  return (size_t)4 * swimg::rows_bound(L.total_blocks, L.batch) * swimg::pitch_of(L.max_blocks) * sizeof(float);
 }
 
-// One product dst = A * Bm on the tensor cores.  split_R / split_W: which operands still need their hi/lo
-// images written into ws4 = [R_hi | R_lo | W_hi | W_lo] (b*b floats each).
-int32_t launch_walk_tc(int b, const float* A, const float* Bm, float* dst, float* ws4, bool split_R, bool split_W,
-                       int causal, cudaStream_t st) {
-  const size_t bb = (size_t)b * b;
-  float *Rhi = ws4, *Rlo = ws4 + bb, *Whi = ws4 + 2 * bb, *Wlo = ws4 + 3 * bb;
-  if (split_R || split_W) {
-    dim3 grid(b, 2);
-    count_launch();
-    split_tf32_kernel<<<grid, 256, 0, st>>>(split_R ? A : nullptr, split_W ? Bm : nullptr, Rhi, Rlo, Whi, Wlo, b,
-                                            causal);
-  }
+int32_t launch_split_tf32(const sw_layout& L, const float* R, const float* W, const WalkImages& im, int causal,
+                          cudaStream_t st) {
+  dim3 grid(swimg::pad_rows(L.max_blocks), 2, L.batch);
+  count_launch();
+  split_tf32_kernel<<<grid, 256, 0, st>>>(R, W, im.r_hi, im.r_lo, im.w_hi, im.w_lo, L.cu_blocks, L.cu_sq, im.pitch,
+                                          causal);
+  return check_launch("sw_walk_update(split)");
+}
+
+// One product dst = R * W per sequence on the tensor cores, operands = the hi / lo images in `im`.
+int32_t launch_walk_tc(const sw_layout& L, const WalkImages& im, float* dst, int causal, bool zero_upper,
+                       cudaStream_t st) {
   CUtensorMap mrh, mrl, mwh, mwl;
-  const bool ok = make_map_f32(&mrh, Rhi, b, b, BM, false) && make_map_f32(&mrl, Rlo, b, b, BM, false) &&
-                  make_map_f32(&mwh, Whi, b, b, BK, true) && make_map_f32(&mwl, Wlo, b, b, BK, true);
+  const bool ok = make_map_f32(&mrh, im.r_hi, im.rows, im.pitch, BM, false) &&
+                  make_map_f32(&mrl, im.r_lo, im.rows, im.pitch, BM, false) &&
+                  make_map_f32(&mwh, im.w_hi, im.rows, im.pitch, BK, true) &&
+                  make_map_f32(&mwl, im.w_lo, im.rows, im.pitch, BK, true);
   if (!ok) return fail(SW_ERR_CUDA, "sw_walk_update: cuTensorMapEncodeTiled failed");
   if (int32_t rc = allow_dynamic_smem(walk_tc_kernel, kSmemBytes, "sw_walk_update(tcgen05) smem attribute")) return rc;
   Params p;
-  p.out = dst; p.b = b; p.nt = cdiv(b, BM); p.causal = causal;
-  p.n_work = causal ? p.nt * (p.nt + 1) / 2 : p.nt * p.nt;
+  p.out = dst; p.cu_blocks = L.cu_blocks; p.cu_sq = L.cu_sq; p.causal = causal; p.zero_upper = zero_upper ? 1 : 0;
+  const int nt = cdiv(L.max_blocks, BM);
+  const int tiles = (causal && !zero_upper) ? nt * (nt + 1) / 2 : nt * nt;
   count_launch();
-  walk_tc_kernel<<<p.nt * p.nt, kThreads, kSmemBytes, st>>>(mrh, mrl, mwh, mwl, p);
+  walk_tc_kernel<<<dim3(tiles, L.batch), kThreads, kSmemBytes, st>>>(mrh, mrl, mwh, mwl, p);
   return check_launch("sw_walk_update(tcgen05)");
 }
 

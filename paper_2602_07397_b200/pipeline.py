@@ -59,9 +59,18 @@ class PrefillPipeline:
     def R_cur(self) -> Optional[torch.Tensor]:
         return None if self.cur < 0 else self.R[self.cur]
 
-    def select(self, Q: torch.Tensor, K: torch.Tensor, stream=None) -> None:
-        """Steps 1-7: sketch -> block scores -> walk -> top-tau (idx / count updated in place)."""
+    def select(self, Q: torch.Tensor, K: torch.Tensor, stream=None, fused: bool = True) -> None:
+        """Steps 1-7: sketch -> block scores -> walk -> top-tau (idx / count updated in place).
+        ``fused`` = sw_sketch_qk + sw_prefill_select (four launches); otherwise the plain calls."""
         L = self.L
+        if fused and Q.dtype == K.dtype:
+            sw.sw_sketch_qk(L, Q, K, self.signs, self.cols, self.r, self.sketch_scale, self.qs, self.ks, self.qbar,
+                            self.kbar, stream)
+            nxt = 0 if self.cur < 0 else 1 - self.cur
+            sw.sw_prefill_select(L, self.qs, self.ks, self.r, self.s, self.flags, self.R_cur, self.R[nxt], self.W,
+                                 self.A, self.tau, self.tau_max, self.idx, self.count, self.walk_ws, stream)
+            self.cur = nxt
+            return
         if Q.dtype == K.dtype:
             sw.sw_sketch_qk(L, Q, K, self.signs, self.cols, self.r, self.sketch_scale, self.qs, self.ks, self.qbar,
                             self.kbar, stream)
@@ -82,8 +91,8 @@ class PrefillPipeline:
                                   self.flags, out, lse, self.attn_ws, stream)
         return out
 
-    def layer(self, Q, K, V, out=None, stream=None) -> torch.Tensor:
-        self.select(Q, K, stream)
+    def layer(self, Q, K, V, out=None, stream=None, fused: bool = True) -> torch.Tensor:
+        self.select(Q, K, stream, fused)
         return self.attend(Q, K, V, out, None, stream)
 
 

@@ -272,7 +272,7 @@ def test_walk_tcgen05_needs_workspace_and_shape(sw):
     B = 64
     prev = sw.sw_set_walk_kernel(sw.SW_WALK_TCGEN05)
     try:
-        for blocks, ws_ok in (((512,), False), ((100,), True), ((256, 256), True)):
+        for blocks, ws_ok in (((512,), False), ((100,), True), ((100, 255), True)):
             L = sw.make_layout([b * B for b in blocks], B)
             x = torch.zeros(L.total_sq, device="cuda")
             out = torch.zeros(L.total_sq, device="cuda")
@@ -283,6 +283,103 @@ def test_walk_tcgen05_needs_workspace_and_shape(sw):
             assert e.value.code == (sw.SW_ERR_UNSUPPORTED if ws_ok else sw.SW_ERR_WORKSPACE)
     finally:
         sw.sw_set_walk_kernel(prev)
+
+
+@pytest.mark.parametrize("blocks", [(256, 301, 512), (130, 600), (257,)])
+@pytest.mark.parametrize("flags", [O.DEFAULT_FLAGS, O.DEFAULT_FLAGS & ~O.CAUSAL])
+def test_walk_update_tcgen05_varlen_batch(sw, blocks, flags):
+    """The tensor-core walk on a packed varlen batch (one stacked operand image per operand), sizes that are no
+    multiple of the 128-row tiles or of 4, against the oracle's fp64 product of the fp32 operands."""
+    rng = np.random.RandomState(sum(blocks))
+    B, s = 64, 2
+    L = sw.make_layout([b * B for b in blocks], B)
+    As = [O.power(O.masked_softmax(rng.randn(b, b) * 2, flags), s, flags).astype(np.float32) for b in blocks]
+    Rs = [O.masked_softmax(rng.randn(b, b) * 2, flags).astype(np.float32) for b in blocks]
+    Wd = dev(np.concatenate([a.ravel() for a in As])); Rp = dev(np.concatenate([r.ravel() for r in Rs]))
+    ws = torch.full((sw.sw_workspace_bytes(sw.SW_OP_WALK_UPDATE, L),), 0xFF, dtype=torch.uint8, device="cuda")   # NaN bits
+    prev = sw.sw_set_walk_kernel(sw.SW_WALK_TCGEN05)
+    try:
+        out = torch.full((L.total_sq,), float("nan"), device="cuda")
+        sw.sw_walk_update(L, Rp, Wd, s, flags, out, ws)
+        torch.cuda.synchronize()
+        assert sw.sw_get_walk_kernel_used() == sw.SW_WALK_TCGEN05
+    finally:
+        sw.sw_set_walk_kernel(prev)
+    on = out.cpu().numpy(); off = 0
+    for k, b in enumerate(blocks):
+        ref = Rs[k].astype(np.float64) @ As[k].astype(np.float64)
+        if flags & O.ROWNORM:
+            ref = O.row_rescale(ref)
+        got = on[off:off + b * b].reshape(b, b)
+        assert np.isfinite(got).all()
+        scale = np.abs(ref).max(axis=-1, keepdims=True)
+        assert (np.abs(got - ref) / scale).max() <= 1e-5
+        off += b * b
+
+
+@pytest.mark.parametrize("blocks,r", [((16,), 16), ((100,), 64), ((37, 130, 64), 64), ((512,), 64), ((300, 700), 32),
+                                      ((1030,), 64), ((50,), 2)])
+@pytest.mark.parametrize("flags,s", [(O.DEFAULT_FLAGS, 2), (O.DEFAULT_FLAGS & ~O.SCORE_SOFTMAX, 3),
+                                     (O.DEFAULT_FLAGS | O.POW_MATRIX, 2), (O.DEFAULT_FLAGS & ~O.ROWNORM, 1),
+                                     (O.DEFAULT_FLAGS & ~O.CAUSAL, 2), (O.DEFAULT_FLAGS, 8)])
+def test_prefill_select_fused_chain(sw, blocks, r, flags, s):
+    """sw_prefill_select (scores + softmax + power + operand images | walk GEMM | rescale + top-tau: at most three
+    launches) against the oracle's Alg. 1 Steps 5-7, three layers with R carried, and against the three plain calls
+    on the same inputs.  Sizes cover the SIMT and the tensor-core walk, varlen batches, b % 4 != 0 and r = 2 (which
+    the fused score kernel does not take: the plain chain runs)."""
+    B, layers = 64, 3
+    L = sw.make_layout([b * B for b in blocks], B)
+    taus = [O.tau_from_density(0.2, b) for b in blocks]
+    tau_max = max(taus)
+    tau_d = dev(np.asarray(taus, np.int32))
+    ws = torch.full((max(sw.sw_workspace_bytes(sw.SW_OP_WALK_UPDATE, L), 16),), 0xFF, dtype=torch.uint8, device="cuda")
+    nb = L.total_blocks
+    R_gpu = [torch.full((L.total_sq,), float("nan"), device="cuda") for _ in range(2)]
+    R_pl = [torch.full((L.total_sq,), float("nan"), device="cuda") for _ in range(2)]
+    R_ref = [None] * len(blocks)
+    cur = -1
+    for layer in range(layers):
+        rng = np.random.RandomState(1000 * layer + nb)
+        qs = (rng.randn(nb, r) * 1.2).astype(np.float32); ks = (rng.randn(nb, r) * 1.2).astype(np.float32)
+        W = torch.full((L.total_sq,), float("nan"), device="cuda"); A = torch.full_like(W, float("nan"))
+        idx = torch.full((nb, tau_max), -7, dtype=torch.int32, device="cuda"); cnt = torch.full((nb,), -7, dtype=torch.int32, device="cuda")
+        nxt = 0 if cur < 0 else 1 - cur
+        n0 = sw.sw_launch_count()
+        sw.sw_prefill_select(L, dev(qs), dev(ks), r, s, flags, None if cur < 0 else R_gpu[cur], R_gpu[nxt], W, A, tau_d,
+                             tau_max, idx, cnt, ws)
+        launches = sw.sw_launch_count() - n0
+        if r >= 4 and not ((flags & O.POW_MATRIX) and s > 1):
+            assert launches == (2 if cur < 0 else 3), launches
+        # the three plain calls on the same inputs
+        W2 = torch.empty_like(W); idx2 = torch.empty_like(idx); cnt2 = torch.empty_like(cnt)
+        sw.sw_block_scores(L, dev(qs), dev(ks), r, s, flags, W2, None)
+        sw.sw_walk_update(L, None if cur < 0 else R_pl[cur], W2, s, flags, R_pl[nxt], ws)
+        sw.sw_select_topk(L, R_pl[nxt], tau_d, tau_max, flags, idx2, cnt2)
+        torch.cuda.synchronize()
+        cur = nxt
+        Wn, An, Rn, Rp = W.cpu().numpy(), A.cpu().numpy(), R_gpu[cur].cpu().numpy(), R_pl[cur].cpu().numpy()
+        idx_g, cnt_g = idx.cpu().numpy(), cnt.cpu().numpy()
+        assert np.array_equal(cnt_g, cnt2.cpu().numpy())
+        lo = off = 0
+        for k, b in enumerate(blocks):
+            S = O.block_scores(qs[lo:lo + b].astype(np.float64), ks[lo:lo + b].astype(np.float64))
+            A_ref = O.masked_softmax(S, flags)
+            W_ref = A_ref if (flags & O.POW_MATRIX) else O.power(A_ref, s, flags)
+            R_ref[k] = O.walk_update(R_ref[k], A_ref, s, flags)
+            sl = slice(off, off + b * b)
+            assert rowwise_close(An[sl].reshape(b, b), A_ref)
+            assert rowwise_close(Wn[sl].reshape(b, b), W_ref)
+            assert rowwise_close(Rn[sl].reshape(b, b), R_ref[k])
+            assert rowwise_close(Rn[sl].reshape(b, b), Rp[sl].reshape(b, b).astype(np.float64), rel=1e-4)
+            if flags & O.CAUSAL:
+                assert not np.triu(Rn[sl].reshape(b, b), 1).any()
+            idx_ref, cnt_ref = O.select_topk(R_ref[k], taus[k], flags)
+            assert np.array_equal(cnt_g[lo:lo + b], cnt_ref)
+            for i in range(b):
+                forced = ({i} if flags & O.FORCE_LAST else set()) | ({0} if flags & O.FORCE_FIRST else set())
+                assert near_tie_only(idx_g[lo + i, :cnt_ref[i]], idx_ref[i, :cnt_ref[i]], R_ref[k][i], forced), (layer, k, i)
+                assert (idx_g[lo + i, cnt_ref[i]:] == -1).all()
+            lo += b; off += b * b
 
 
 def test_walk_s1_identity_is_block_scores(sw):

@@ -15,7 +15,7 @@ from synth import gen
 CFG_IDX = 1
 METRIC = "prefill_tokens_per_s_per_layer_at_20pct_density"
 UNIT = "tokens/s"
-KERNELS = ["sketch_qk", "block_scores", "walk", "select", "attn"]
+KERNELS = ["sketch_qk", "prefill_select", "attn"]
 ROOT = os.path.dirname(os.path.abspath(__file__))
 
 
@@ -66,17 +66,14 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
             pkg.sw_sketch_qk(L, Q, K, pipe.signs, pipe.cols, pipe.r, pipe.sketch_scale, pipe.qs, pipe.ks, pipe.qbar,
                              pipe.kbar)
             if ev is not None: ev[1].record(stream)
-            pkg.sw_block_scores(L, pipe.qs, pipe.ks, pipe.r, pipe.s, pipe.flags, pipe.W, None)
-            if ev is not None: ev[2].record(stream)
             nxt = 0 if pipe.cur < 0 else 1 - pipe.cur
-            pkg.sw_walk_update(L, pipe.R_cur, pipe.W, pipe.s, pipe.flags, pipe.R[nxt], pipe.walk_ws)
+            pkg.sw_prefill_select(L, pipe.qs, pipe.ks, pipe.r, pipe.s, pipe.flags, pipe.R_cur, pipe.R[nxt], pipe.W, None,
+                                  pipe.tau, pipe.tau_max, pipe.idx, pipe.count, pipe.walk_ws)
             pipe.cur = nxt
-            if ev is not None: ev[3].record(stream)
-            pkg.sw_select_topk(L, pipe.R[nxt], pipe.tau, pipe.tau_max, pipe.flags, pipe.idx, pipe.count)
-            if ev is not None: ev[4].record(stream)
+            if ev is not None: ev[2].record(stream)
             pkg.sw_sparse_attn_prefill(L, Q, K, V, pipe.idx, pipe.count, pipe.tau_max, pipe.softmax_scale,
                                        pipe.flags, outs[layer & 1], None, pipe.attn_ws)
-            if ev is not None: ev[5].record(stream)
+            if ev is not None: ev[3].record(stream)
 
     def barrier():
         if dist is not None:

@@ -181,6 +181,7 @@ score_rows_kernel(int s, uint32_t flags, const int32_t* __restrict__ cu_blocks, 
 // written once and never re-read by this step; split_tf32_kernel and its pass over W and R are gone.
 constexpr int kFRows = 8;
 constexpr int kFCols = 64;
+constexpr int kFStages = 4;           // ring of key-sketch tiles (cp.async)
 
 struct FusedParams {
   const float *qs, *ks;
@@ -220,26 +221,28 @@ score_fused_kernel(const FusedParams p) {
   if (i0 >= rows_all) return;
   const int r = p.r, r4 = r >> 2, ldk = r + 4;
   float* s_q = smem;                                          // [kFRows][r]
-  float* s_k = s_q + kFRows * r;                              // [2][kFCols][r + 4]
-  float* s_S = s_k + 2 * kFCols * ldk;                        // [kFRows][lds]
+  float* s_k = s_q + kFRows * r;                              // [kFStages][kFCols][r + 4]
+  float* s_S = s_k + kFStages * kFCols * ldk;                        // [kFRows][lds]
   const int nrows = max(0, min(kFRows, b - i0));
 
   if (nrows > 0) {
     const int hi_col = causal ? min(b, i0 + kFRows) : b;      // columns some row of the strip can see
     const int nct = (hi_col + kFCols - 1) / kFCols;
-    auto load_k = [&](int ct, int buf) {
-      float* dst = s_k + buf * kFCols * ldk;
-      for (int i = tid; i < kFCols * r4; i += kThreads) {
-        const int kk = i / r4, c = (i - kk * r4) * 4;
-        const int j = ct * kFCols + kk;
-        const float* src = p.ks + (int64_t)(blk0 + min(j, b - 1)) * r + c;
-        const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst + kk * ldk + c);
-        const int sz = (j < b) ? 16 : 0;                      // rows past the sequence: zero fill
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(sz) : "memory");
+    auto load_k = [&](int ct) {                               // tile ct -> ring slot ct % kFStages (or an empty group)
+      if (ct < nct) {
+        float* dst = s_k + (ct % kFStages) * kFCols * ldk;
+        for (int i = tid; i < kFCols * r4; i += kThreads) {
+          const int kk = i / r4, c = (i - kk * r4) * 4;
+          const int j = ct * kFCols + kk;
+          const float* src = p.ks + (int64_t)(blk0 + min(j, b - 1)) * r + c;
+          const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst + kk * ldk + c);
+          const int sz = (j < b) ? 16 : 0;                    // rows past the sequence: zero fill
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(sz) : "memory");
+        }
       }
       asm volatile("cp.async.commit_group;" ::: "memory");
     };
-    load_k(0, 0);
+    for (int ct = 0; ct < kFStages - 1; ++ct) load_k(ct);     // kFStages - 1 tiles in flight (one latency, not one each)
     for (int i = tid; i < kFRows * r4; i += kThreads) {
       const int rr = i / r4, c = (i - rr * r4) * 4;
       float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -248,10 +251,10 @@ score_fused_kernel(const FusedParams p) {
     }
     const int col = tid & (kFCols - 1), rg = tid / kFCols;    // rows 2 rg, 2 rg + 1 of the strip
     for (int ct = 0; ct < nct; ++ct) {
-      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      asm volatile("cp.async.wait_group %0;" ::"n"(kFStages - 2) : "memory");
       __syncthreads();                                        // tile ct landed; tile ct - 1 fully consumed
-      if (ct + 1 < nct) load_k(ct + 1, (ct + 1) & 1);
-      const float* kp = s_k + (ct & 1) * kFCols * ldk + col * ldk;
+      load_k(ct + kFStages - 1);
+      const float* kp = s_k + (ct % kFStages) * kFCols * ldk + col * ldk;
       const float* q0 = s_q + (2 * rg) * r;
       const float* q1 = q0 + r;
       float a0 = 0.f, a1 = 0.f;
@@ -265,6 +268,7 @@ score_fused_kernel(const FusedParams p) {
       s_S[(2 * rg) * p.lds + ct * kFCols + col] = a0 * p.inv_sqrt_r;
       s_S[(2 * rg + 1) * p.lds + ct * kFCols + col] = a1 * p.inv_sqrt_r;
     }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
   }
 
@@ -407,7 +411,7 @@ int32_t launch_block_scores(const sw_layout& L, const float* qs, const float* ks
 static size_t fused_smem_bytes(int max_blocks, int r, int* lds_out) {
   const int lds = ((max_blocks + kFCols - 1) / kFCols) * kFCols + 4;   // whole 64-column tiles are written
   if (lds_out) *lds_out = lds;
-  return sizeof(float) * ((size_t)kFRows * r + 2 * (size_t)kFCols * (r + 4) + (size_t)kFRows * lds);
+  return sizeof(float) * ((size_t)kFRows * r + (size_t)kFStages * kFCols * (r + 4) + (size_t)kFRows * lds);
 }
 
 bool scores_fused_supported(const sw_layout& L, int r) {

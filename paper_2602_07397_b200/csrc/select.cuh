@@ -116,7 +116,8 @@ __device__ void radix_threshold(Load load, const RowJob& J, Scratch& S, uint32_t
 // keys of its contiguous index range [lo, hi) in registers, so the four passes and the compaction touch
 // memory only for the histogram.  cmask: bit e set = index lo + e is a non-forced candidate.
 constexpr int kRegKeys = 8;
-__device__ __forceinline__ void radix_threshold_regs(const uint32_t (&key)[kRegKeys], uint32_t cmask, const RowJob& J,
+template <int K>
+__device__ __forceinline__ void radix_threshold_regs(const uint32_t (&key)[K], uint32_t cmask, const RowJob& J,
                                                      Scratch& S, uint32_t& thr, int& n_gt_out) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   uint32_t prefix = 0;
@@ -127,10 +128,10 @@ __device__ __forceinline__ void radix_threshold_regs(const uint32_t (&key)[kRegK
     S.hist[tid] = 0;
     __syncthreads();
     const uint32_t mask_hi = (pass == 0) ? 0u : (0xffffffffu << (shift + 8));
-    uint32_t bin[kRegKeys];
+    uint32_t bin[K];
     bool same = true;
 #pragma unroll
-    for (int e = 0; e < kRegKeys; ++e) {
+    for (int e = 0; e < K; ++e) {
       const bool in = ((cmask >> e) & 1u) && (key[e] & mask_hi) == prefix;
       bin[e] = in ? ((key[e] >> shift) & 0xffu) : 256u;
       same = same && bin[e] == bin[0];
@@ -139,10 +140,10 @@ __device__ __forceinline__ void radix_threshold_regs(const uint32_t (&key)[kRegK
     // fall into one bin -- the degenerate row of equal scores -- would serialise, so it sends a single add
     const uint32_t b0 = __shfl_sync(0xffffffffu, bin[0], 0);
     if (__all_sync(0xffffffffu, same && bin[0] == b0)) {
-      if (lane == 0 && b0 < 256u) atomicAdd(&S.hist[b0], 32u * kRegKeys);
+      if (lane == 0 && b0 < 256u) atomicAdd(&S.hist[b0], 32u * K);
     } else {
 #pragma unroll
-      for (int e = 0; e < kRegKeys; ++e)
+      for (int e = 0; e < K; ++e)
         if (bin[e] < 256u) atomicAdd(&S.hist[bin[e]], 1u);
     }
     __syncthreads();
@@ -167,6 +168,63 @@ __device__ __forceinline__ void radix_threshold_regs(const uint32_t (&key)[kRegK
   n_gt_out = n_gt;
 }
 
+// Register path: every thread keeps the K keys of its contiguous index range [lo, hi) in registers (rows of at most
+// K * kThreads candidates).  K is chosen by the row length (2, 4 or 8): the passes cost K bin computations and
+// atomics per thread whatever the row length, and a short row (b = 512: 2 keys per thread) was issue-bound at K = 8.
+template <int K, typename Load>
+__device__ __forceinline__ void select_row_regs(Load load, const RowJob& J, int32_t* __restrict__ out, int tau_max,
+                                              int32_t* __restrict__ count_out, Scratch& S, bool take_all, int lo, int hi) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  uint32_t thr = 0;
+  int n_gt = 0;
+  uint32_t key[K];
+  uint32_t cmask = 0, fmask = 0;
+#pragma unroll
+  for (int e = 0; e < K; ++e) {
+    const int j = lo + e;
+    key[e] = 0;
+    if (j < hi) {
+      if (is_forced(J, j)) fmask |= 1u << e;
+      else { cmask |= 1u << e; key[e] = order_key(load(j)); }
+    }
+  }
+  if (!take_all && J.need > 0) radix_threshold_regs(key, cmask, J, S, thr, n_gt);
+  const int eq_quota = J.need - n_gt;
+  uint32_t cert = fmask, eqm = 0;                   // bit e: index lo + e is certainly in / equals the threshold
+#pragma unroll
+  for (int e = 0; e < K; ++e) {
+    if ((cmask >> e) & 1u) {
+      if (take_all) cert |= 1u << e;
+      else if (J.need > 0) {
+        if (key[e] > thr) cert |= 1u << e;
+        else if (key[e] == thr) eqm |= 1u << e;
+      }
+    }
+  }
+  unsigned long long v = ((unsigned long long)__popc(eqm) << 32) | (unsigned)__popc(cert), incl = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned long long u = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += u;
+  }
+  if (lane == 31) S.warp_scan[warp] = incl;
+  __syncthreads();
+  unsigned long long base = 0;
+  for (int w = 0; w < warp; ++w) base += S.warp_scan[w];
+  const unsigned long long excl = base + incl - v;
+  int c_before = (int)(excl & 0xffffffffu), e_before = (int)(excl >> 32);
+#pragma unroll
+  for (int e = 0; e < K; ++e) {
+    const bool c = (cert >> e) & 1u, q = (eqm >> e) & 1u;
+    const int pos = c_before + min(e_before, eq_quota);
+    if ((c || (q && e_before < eq_quota)) && pos < tau_max) out[pos] = lo + e;
+    c_before += c; e_before += q;
+  }
+  for (int p = J.budget + tid; p < tau_max; p += kThreads) out[p] = -1;
+  if (tid == 0) *count_out = J.budget;
+  __syncthreads();                          // scratch may be reused by the caller
+}
+
 // load(j): score of candidate j (global or shared memory).  out: tau_max ints (ascending, -1 padded).
 template <typename Load>
 __device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out, int tau_max,
@@ -179,55 +237,9 @@ __device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out
   // ordered compaction: thread t owns indices [t*per, (t+1)*per)
   const int per = (J.n_cand + kThreads - 1) / kThreads;
   const int lo = min(tid * per, J.n_cand), hi = min(lo + per, J.n_cand);
-  if (per <= kRegKeys) {
-    uint32_t key[kRegKeys];
-    uint32_t cmask = 0, fmask = 0;
-#pragma unroll
-    for (int e = 0; e < kRegKeys; ++e) {
-      const int j = lo + e;
-      key[e] = 0;
-      if (j < hi) {
-        if (is_forced(J, j)) fmask |= 1u << e;
-        else { cmask |= 1u << e; key[e] = order_key(load(j)); }
-      }
-    }
-    if (!take_all && J.need > 0) radix_threshold_regs(key, cmask, J, S, thr, n_gt);
-    const int eq_quota = J.need - n_gt;
-    uint32_t cert = fmask, eqm = 0;                   // bit e: index lo + e is certainly in / equals the threshold
-#pragma unroll
-    for (int e = 0; e < kRegKeys; ++e) {
-      if ((cmask >> e) & 1u) {
-        if (take_all) cert |= 1u << e;
-        else if (J.need > 0) {
-          if (key[e] > thr) cert |= 1u << e;
-          else if (key[e] == thr) eqm |= 1u << e;
-        }
-      }
-    }
-    unsigned long long v = ((unsigned long long)__popc(eqm) << 32) | (unsigned)__popc(cert), incl = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const unsigned long long u = __shfl_up_sync(0xffffffffu, incl, o);
-      if (lane >= o) incl += u;
-    }
-    if (lane == 31) S.warp_scan[warp] = incl;
-    __syncthreads();
-    unsigned long long base = 0;
-    for (int w = 0; w < warp; ++w) base += S.warp_scan[w];
-    const unsigned long long excl = base + incl - v;
-    int c_before = (int)(excl & 0xffffffffu), e_before = (int)(excl >> 32);
-#pragma unroll
-    for (int e = 0; e < kRegKeys; ++e) {
-      const bool c = (cert >> e) & 1u, q = (eqm >> e) & 1u;
-      const int pos = c_before + min(e_before, eq_quota);
-      if ((c || (q && e_before < eq_quota)) && pos < tau_max) out[pos] = lo + e;
-      c_before += c; e_before += q;
-    }
-    for (int p = J.budget + tid; p < tau_max; p += kThreads) out[p] = -1;
-    if (tid == 0) *count_out = J.budget;
-    __syncthreads();                          // scratch may be reused by the caller
-    return;
-  }
+  if (per <= 2) { select_row_regs<2>(load, J, out, tau_max, count_out, S, take_all, lo, hi); return; }
+  if (per <= 4) { select_row_regs<4>(load, J, out, tau_max, count_out, S, take_all, lo, hi); return; }
+  if (per <= kRegKeys) { select_row_regs<kRegKeys>(load, J, out, tau_max, count_out, S, take_all, lo, hi); return; }
   if (!take_all && J.need > 0) radix_threshold(load, J, S, thr, n_gt);
   const int eq_quota = J.need - n_gt;       // equal-key candidates to take, lowest index first
 

@@ -48,10 +48,12 @@ def test_launch_counter_counts_kernels(sw):
     qs = torch.randn(L.total_blocks, r, device="cuda"); ks = torch.randn(L.total_blocks, r, device="cuda")
     W = torch.empty(L.total_sq, device="cuda"); R = torch.empty(L.total_sq, device="cuda")
     n0 = sw.sw_launch_count()
-    sw.sw_block_scores(L, qs, ks, r, 2, sw.SW_DEFAULT_FLAGS, W, None)          # tile kernel + row kernel
-    assert sw.sw_launch_count() - n0 == 2
+    sw.sw_block_scores(L, qs, ks, r, 2, sw.SW_DEFAULT_FLAGS, W, None)          # one fused launch
+    assert sw.sw_launch_count() - n0 == 1
     sw.sw_walk_update(L, None, W, 2, sw.SW_DEFAULT_FLAGS, R, None)             # R^0 = W^0 copy + rescale
-    assert sw.sw_launch_count() - n0 == 4
+    assert sw.sw_launch_count() - n0 == 3
+    sw.sw_block_scores(L, qs[:, :2].contiguous(), ks[:, :2].contiguous(), 2, 2, sw.SW_DEFAULT_FLAGS, W, None)
+    assert sw.sw_launch_count() - n0 == 5                                      # r = 2: tile kernel + row kernel
     torch.cuda.synchronize()
 
 

@@ -234,21 +234,21 @@ SW_API int32_t sw_select_topk_row(int32_t batch, int32_t block, int32_t max_bloc
                            const int32_t* seqlens, const int32_t* tau, int32_t tau_max,
                            uint32_t flags, int32_t* idx, int32_t* count, sw_stream_t stream);
 
-/* Decode selection, fused -- Alg. 2 Steps 2-6 in ONE launch: exactly the sequence
+/* Decode selection, fused -- Alg. 2 Steps 2-6 in two launches: exactly the sequence
  *   sw_sketch_append(k_new -> kbar, ks); sw_sketch_append(q -> q~_t); sw_block_scores_row;
  *   sw_walk_update_row (with SW_ROWNORM: r_out / max|r_out|, P9); sw_select_topk_row
  * with the same arguments and the same results up to fp32 summation order (the selected indices are
- * bit-exact given the same r_out).  One thread-block cluster per sequence; the cached W is read once.
+ * bit-exact given the same r_out).  The cached W is read once, by the whole grid whatever the batch.
  * q: [batch, h_q, d], k_new: [batch, h_kv, d] (bf16 or fp32, same dtype).  kbar [batch, max_blocks, d]
  * and ks [batch, max_blocks, r] are updated in place for block b_curr, and the new row of W is stored
  * as row b_q of W_cache (as sw_walk_update_row does), so consecutive decode steps -- across block
  * boundaries too -- need no other cache maintenance than appending K/V.  r_prev (NULL = e_{b_q}),
  * r_out: dev fp32 [batch, max_blocks].  Needs !SW_POW_MATRIX and SW_CAUSAL (see sw_block_scores_row).
  * ws: dev scratch of sw_decode_select_workspace_bytes(batch, max_blocks) bytes (SW_ERR_WORKSPACE if smaller):
- * the raw score row, the partial sums of the W stream and one completion counter per sequence.  The
- * counters (the first 512 + 4 * batch bytes) must be ZERO when the call starts -- zero the buffer once after
- * allocating it -- and every completed call leaves them zero again, so one buffer serves all layers and
- * steps issued on the same stream (calls that share a workspace must not overlap).  batch <= 1024. */
+ * the raw score row and the partial sums of the W stream, handed from the first kernel to the second (no state is
+ * kept between calls; calls that share a workspace must not overlap).  batch <= 512.  Two launches: the
+ * streaming kernel (duties + cached-W stream over the whole grid) and, as its programmatic dependent, the
+ * per-sequence tail (softmax, W_new, rescale, select). */
 SW_API int32_t sw_decode_select(int32_t batch, int32_t block, int32_t max_blocks, const sw_tensor* q,
                          const sw_tensor* k_new, const int32_t* seqlens, const int8_t* signs,
                          const int32_t* cols, int32_t r, float scale, int32_t s, uint32_t flags,

@@ -281,7 +281,7 @@ def sw_select_topk_row(batch, block, max_blocks, r, seqlens, tau, tau_max, flags
 
 def sw_decode_select(batch, block, max_blocks, q, k_new, seqlens, signs, cols, r, scale, s, flags, kbar, ks,
                      W_cache, stride_seq, r_prev, r_out, tau, tau_max, idx, count, ws, stream=None) -> None:
-    """ws: uint8 tensor of sw_decode_select_workspace_bytes(batch, max_blocks) bytes, zero-filled once by the caller."""
+    """ws: uint8 tensor of sw_decode_select_workspace_bytes(batch, max_blocks) bytes."""
     qt, kt = _tensor(q), _tensor(k_new)
     _check(_lib.sw_decode_select(batch, block, max_blocks, C.byref(qt), C.byref(kt), _ptr(seqlens), _ptr(signs),
                                  _ptr(cols), r, scale, s, flags, _ptr(kbar), _ptr(ks), _ptr(W_cache), stride_seq,

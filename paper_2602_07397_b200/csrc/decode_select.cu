@@ -1,7 +1,7 @@
-// sw_decode_select: Alg. 2 Steps 2-6 for one new token per sequence, fused into
-// ONE kernel: running key-block mean + sketches (Steps 2-3), the new row of W (Steps 3-4), the
-// row-vector walk r^k = r^{k-1} W'^k (Step 5), the max-abs rescale (P9) and the
-// top-tau selection (Step 6).  HBM-bound on the cached W (4 b^2/2 bytes per sequence).
+// sw_decode_select: Alg. 2 Steps 2-6 for one new token per sequence: running key-block
+// mean + sketches (Steps 2-3), the new row of W (Steps 3-4), the row-vector walk r^k = r^{k-1} W'^k (Step 5,
+// SURVEY 8(a) row a6), the max-abs rescale (P9) and the top-tau selection (Step 6).  HBM-bound on the cached W
+// (4 b^2/2 bytes per sequence).  Two kernels; this file holds the first: everything that touches HBM-sized data.
 //
 // The whole grid (two CTAs per SM) works on the batch, whatever its size.  Two kinds of work are dealt out:
 //  * chunks: 64 rows x 64 columns of the block-causal part of the cached W (rows [64 c, b_q) of column tile
@@ -14,99 +14,24 @@
 // A CTA runs its duties first.  Every load they need (head values, key-sketch rows, the old mean) and the
 // r_prev rows of the stream are requested BEFORE the first chunks of the W stream: on an SM that keeps
 // ~160 KB of the stream in flight a load issued behind it waits ~3 us (queue depth / per-SM bandwidth).
-// Nothing waits on another CTA: every CTA counts what it has finished per sequence with one atomic, and
-// the CTA that completes a sequence runs its tail -- softmax statistics of the score row, W_new = A^s,
-// r = sum of partials + r_prev[b_q] W_new, rescale, radix select (select.cuh) -- on a row of at most
-// max_blocks floats in shared memory.  The counters live in the caller's workspace and are left at zero by
-// every completed call.  The new row of W is stored as row b_q of the cache (Alg. 2 Step 4).
+// The second kernel (decode_tail.cu, one CTA of 1024 threads per sequence, launched as a programmatic dependent
+// so that it becomes resident while the last CTAs of this one drain) turns the raw score row and the partial
+// sums into W_new = A^s, r, the rescaled r_out and the block list.  An earlier version ran that tail on the last
+// CTA to finish a sequence (one launch, a completion counter in the workspace): 256 threads made the radix
+// select and the row passes a 12 us serial chain (two warps per scheduler: every pass is bound by the dependent
+// issue latency), a quarter of a decode layer; 1024 threads do it in a fraction of that.
 // DESIGN.md sec. 6.2 has the measurements behind these choices.
 #include <algorithm>
 
 #include "common.cuh"
-#include "select.cuh"
+#include "decode_select.cuh"
 #include "sketch_common.cuh"
 #include "sm100.cuh"
 
 namespace {
 
-constexpr int kThreads = 256;
-constexpr int kTile = 64;            // columns per tile
-constexpr int kRowGroups = 16;       // row lanes of the vector-matrix product
-constexpr int kChunkRows = 64;
-constexpr int kStages = 4;            // 4 x 16 KB ring + two r_prev rows + the prefix tables: two CTAs per SM
-constexpr int kChunkBytes = kChunkRows * kTile * 4;
-constexpr int kPieces = kChunkBytes / 16 / kThreads;     // 16-byte cp.async pieces per thread per chunk
-constexpr int kMaxBatch = 512;       // sequence lengths and per-sequence work counts live in shared memory
-constexpr int kMaxTiles = 255;       // column tiles per sequence (max_blocks <= 16320)
-constexpr int kHeadRegs = 16;        // head values a thread holds while the loads of a duty are in flight
-constexpr int kKU = 4;               // key-sketch float4s per thread and duty (64 columns x r <= 64)
+using namespace swds;
 
-struct Params {
-  const void* q;  int64_t q_stride_seq, q_stride_head;  int h_q;
-  const void* k;  int64_t k_stride_seq, k_stride_head;  int h_kv;
-  const int32_t* seqlens;
-  const int8_t* signs;  const int32_t* cols;  int r;  float scale;  float inv_sqrt_r;
-  int s;  uint32_t flags;
-  float* kbar;  float* ks;
-  float* W;  int64_t w_stride_seq;
-  const float* r_prev;  float* r_out;
-  const int32_t* tau;  int tau_max;
-  int32_t* idx;  int32_t* count;
-  int batch, B, max_blocks;
-  int use_async;                     // W streamed by cp.async (needs 16-byte aligned rows), else plain loads
-  // workspace
-  unsigned int* ws_cnt;              // [batch] duties + chunks finished per sequence (zero between calls)
-  float* ws_scores;                  // [batch][mbp] raw scores of the new row
-  float* ws_part;                    // [batch][tiles_max][slots][64] partial walk sums
-  int mbp, tiles_max, slots;
-};
-
-// Work bookkeeping of one sequence.  b_q = 64 a + e; column tile c < a has rows [64 c, b_q): a - c + (e > 0)
-// chunks; tile a (the one that holds b_q) has (e > 0) chunks.  a + 1 duties.  No chunks without a walk
-// (r_prev = NULL).
-struct SeqInfo {
-  int bq, a, eps;
-  __device__ __forceinline__ int chunks(int tile, bool walk) const { return walk ? (tile < a ? a - tile + eps : eps) : 0; }
-  __device__ __forceinline__ int chunks_before(int tile, bool walk) const {        // tile <= a
-    return walk ? tile * a - tile * (tile - 1) / 2 + tile * eps : 0;
-  }
-  __device__ __forceinline__ int total_chunks(bool walk) const { return walk ? a * (a + 1) / 2 + a * eps + eps : 0; }
-  __device__ __forceinline__ int duties() const { return a + 1; }
-};
-__device__ __forceinline__ SeqInfo seq_info(const int32_t* seqlens, int seq, int B) {
-  SeqInfo s;
-  const int t = seqlens[seq];                          // (a shared-memory copy after the first pass)
-  s.bq = (t - 1) / B;                                  // block of the new token = b_curr
-  s.a = s.bq / kTile;
-  s.eps = (s.bq % kTile) != 0;
-  return s;
-}
-// CTA that owns item g when T items are dealt to G CTAs as [i T / G, (i+1) T / G)
-__device__ __forceinline__ int cta_of(long long g, int T, int G) {
-  const long long num = (g + 1) * G - 1;
-  return (num < (1ll << 31)) ? (int)((unsigned)num / (unsigned)T) : (int)(num / T);
-}
-
-__device__ __forceinline__ float block_max(float v, float* s_red) {
-  v = swd::warp_max(v);
-  __syncthreads();
-  if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
-  __syncthreads();
-  float m = s_red[0];
-#pragma unroll
-  for (int w = 1; w < kThreads / 32; ++w) m = fmaxf(m, s_red[w]);
-  return m;
-}
-__device__ __forceinline__ float block_sum(float v, float* s_red) {
-  v = swd::warp_sum(v);
-  __syncthreads();
-  if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
-  __syncthreads();
-  float m = 0.f;
-#pragma unroll
-  for (int w = 0; w < kThreads / 32; ++w) m += s_red[w];
-  return m;
-}
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
@@ -115,11 +40,12 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <typename TIn, int D>
 __global__ void __launch_bounds__(kThreads, 2)
 decode_select_kernel(const Params p) {
+  // the tail kernel is launched as a programmatic dependent: let it become resident as SMs drain
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int G = (int)gridDim.x, me = (int)blockIdx.x;
   const bool walk = p.r_prev != nullptr;
   const bool async = walk && p.use_async;
-  const bool soft = p.flags & SW_SCORE_SOFTMAX;
   const int mb = p.max_blocks;
   const int rstride = p.mbp + kChunkRows;
 
@@ -128,19 +54,13 @@ decode_select_kernel(const Params p) {
   float* s_part = s_rprev + 2 * rstride;                               // [kRowGroups][64]
   uint8_t* s_ring = reinterpret_cast<uint8_t*>(
       (reinterpret_cast<uintptr_t>(s_part + kRowGroups * kTile) + 127) & ~(uintptr_t)127);   // [kStages][16 KB]
-  float* s_row = reinterpret_cast<float*>(s_ring);                     // [mbp] tail only (the ring is idle then)
   __shared__ __align__(16) float s_vec[D], s_qt[128], s_kt[128], s_sign[D];
   __shared__ float s_hx[kThreads / D][D];
   __shared__ int32_t s_cols[128];
-  __shared__ float s_red[kThreads / 32];
   __shared__ int s_pref[kMaxBatch + 1];                                // exclusive prefix of chunks per sequence
   __shared__ int s_dpref[kMaxBatch + 1];                               // exclusive prefix of duties per sequence
   __shared__ int s_len[kMaxBatch];                                     // sequence lengths (read once from HBM)
   __shared__ int s_scan[2][kThreads / 32];
-  __shared__ int s_flag;                                               // this CTA completed some sequence
-  __shared__ unsigned s_tailmask[kMaxBatch / 32];                      // sequences whose tail this CTA runs
-  __shared__ unsigned char s_nslot[kMaxTiles + 1];                     // tail: partials per column tile
-  __shared__ swsel::Scratch scratch;
 
   // ---- chunk and duty counts of all sequences: exclusive prefixes in shared memory -------------------
   {
@@ -165,8 +85,6 @@ decode_select_kernel(const Params p) {
     }
     if (lane == 31) { s_scan[0][warp] = ic; s_scan[1][warp] = id; }
     if (tid < D) s_sign[tid] = p.signs ? (float)p.signs[tid] : 1.f;
-    if (tid < kMaxBatch / 32) s_tailmask[tid] = 0u;
-    if (tid == 0) s_flag = 0;
     if (tid < p.r && tid < 128) s_cols[tid] = p.cols[tid];
     __syncthreads();
     int bc = 0, bd = 0;
@@ -181,7 +99,10 @@ decode_select_kernel(const Params p) {
     __syncthreads();
   }
   const int T = s_pref[p.batch], ND = s_dpref[p.batch];
-  const int g_begin = (int)((long long)me * T / G), g_end = (int)((long long)(me + 1) * T / G);
+  // chunks are dealt to the first Gc = min(G, T) CTAs, so that every one of them has at least one: the partial
+  // slots of a tile (one per CTA that shares it) are then contiguous
+  const int Gc = max(1, min(G, T));
+  const int g_begin = me < Gc ? (int)((long long)me * T / Gc) : T, g_end = me < Gc ? (int)((long long)(me + 1) * T / Gc) : T;
   const int d_begin = (int)((long long)me * ND / G), d_end = (int)((long long)(me + 1) * ND / G);
   const int n_my = g_end - g_begin;
   if (n_my == 0 && d_begin == d_end) return;
@@ -255,22 +176,6 @@ decode_select_kernel(const Params p) {
     if (async) {
       cp_async_commit();
       for (int i = 0; i < kStages - 1; ++i) issue_next();
-    }
-  };
-
-  // this CTA has finished `n` duties / chunks of sequence `seq`: publish; the CTA that completes a sequence
-  // runs its tail (after its own streaming work: the tail's row buffer aliases the ring)
-  auto publish = [&](int seq, int n) {
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) {
-      const SeqInfo si = seq_info(s_len, seq, p.B);
-      const unsigned total = (unsigned)(si.duties() + si.total_chunks(walk));
-      const unsigned old = atomicAdd(p.ws_cnt + seq, (unsigned)n);
-      if (old + (unsigned)n == total) {               // every other CTA's partials and scores are visible after
-        __threadfence();                              // this fence; the tail reads them past a barrier, from L2
-        s_tailmask[seq >> 5] |= 1u << (seq & 31); s_flag = 1;
-      }
     }
   };
 
@@ -381,16 +286,11 @@ decode_select_kernel(const Params p) {
         }
       }
     }
-    // duties of one sequence are published together
-    if (dty == d_end - 1 || find_seq(s_dpref, dty + 1) != seq) {
-      const int first = max(d_begin, s_dpref[seq]);
-      publish(seq, dty - first + 1);
-    }
   }
   if (!stream_started) start_stream();
 
   // ================= chunks: Step 5, r_prev[m] W[m][j] over this CTA's range ===============================
-  int cur_seq = -1, done_in_seq = 0, consumed = 0;
+  int cur_seq = -1, consumed = 0;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   const int cq = tid & 15, rg = tid >> 4;
   const float* rprev_cur = s_rprev;
@@ -398,7 +298,6 @@ decode_select_kernel(const Params p) {
     const SeqInfo& si = cc.si;
     const int seq = cc.seq, tile = cc.tile, bq = si.bq;
     if (seq != cur_seq) {
-      if (cur_seq >= 0) { publish(cur_seq, done_in_seq); done_in_seq = 0; }
       cur_seq = seq;
       const int slot2 = seq - seq_first;
       if (slot2 < 2) {
@@ -444,7 +343,6 @@ decode_select_kernel(const Params p) {
         if (c4 + 3 < mb) acc.w = fmaf(a, __ldg(wr + c4 + 3), acc.w);
       }
     }
-    ++done_in_seq;
     if (it == n_my - 1 || cc.chunk + 1 >= si.chunks(tile, walk)) {
       // one partial per (tile, CTA): slot = rank of this CTA among the CTAs that share the tile
       *reinterpret_cast<float4*>(s_part + rg * kTile + cq * 4) = acc;
@@ -454,7 +352,7 @@ decode_select_kernel(const Params p) {
 #pragma unroll
         for (int g = 0; g < kRowGroups; ++g) v += s_part[g * kTile + tid];      // fixed order
         const long long f0 = s_pref[seq] + si.chunks_before(tile, walk);
-        const int slot = me - cta_of(f0, T, G);
+        const int slot = me - cta_of(f0, T, Gc);
         p.ws_part[(((int64_t)seq * p.tiles_max + tile) * p.slots + slot) * kTile + tid] = v;
       }
       __syncthreads();
@@ -462,104 +360,7 @@ decode_select_kernel(const Params p) {
     }
     advance(cc);
   }
-  if (cur_seq >= 0) publish(cur_seq, done_in_seq);
   asm volatile("cp.async.wait_group 0;" ::: "memory");
-  __syncthreads();
-  if (!s_flag) return;
-
-  // ================= tails: Steps 4-6 on the whole row of every sequence this CTA completed ================
-  for (int seq = 0; seq < p.batch; ++seq) {
-    if (!((s_tailmask[seq >> 5] >> (seq & 31)) & 1u)) continue;
-    const SeqInfo si = seq_info(s_len, seq, p.B);
-    const int bq = si.bq, hi = bq + 1;
-    const int tt = max(0, min(__ldg(p.tau + seq), p.tau_max));     // (requested ahead of the dependent loads below)
-    const float rq = walk ? __ldg(p.r_prev + (int64_t)seq * mb + bq) : 1.f;
-    // partials per column tile = CTAs that share the tile's chunks (cta_of is monotone: one division per tile)
-    for (int tl = tid; tl <= si.a; tl += kThreads) {
-      const int nch = si.chunks(tl, walk);
-      int ns = 0;
-      if (nch > 0) {
-        const long long f0 = s_pref[seq] + si.chunks_before(tl, walk);
-        ns = cta_of(f0 + nch - 1, T, G) - cta_of(f0, T, G) + 1;
-      }
-      s_nslot[tl] = (unsigned char)min(ns, 255);
-    }
-    const float* sc = p.ws_scores + (int64_t)seq * p.mbp;
-    float lmax = -INFINITY;
-    for (int j = tid; j < hi; j += kThreads) { const float v = __ldcg(sc + j); s_row[j] = v; lmax = fmaxf(lmax, v); }
-    float m = 0.f, inv_l = 1.f;
-    if (soft) {
-      m = block_max(lmax, s_red);
-      float e = 0.f;
-      for (int j = tid; j < hi; j += kThreads) e += expf(s_row[j] - m);
-      inv_l = 1.f / block_sum(e, s_red);
-    } else {
-      __syncthreads();                                // s_nslot
-    }
-    // W_new = A^s; Alg. 2 Step 4 cache update: the new row becomes row b_q of the cached W,
-    // zeros right of the diagonal.  Row b_q is never read while b_q is the current block.
-    // Step 5: r_out[j] = sum_{m < b_q} r_prev[m] W[m][j] + r_prev[b_q] w[j], the partial sums in slot order;
-    // 8 columns x 4 slots of loads are in flight per thread (a dependent load per slot cost 5 us here).
-    float* wrow = p.W + (int64_t)seq * p.w_stride_seq + (int64_t)bq * mb;
-    float lamax = 0.f;
-    constexpr int kCols = 8, kSl = 4;
-    for (int j0 = 0; j0 < mb; j0 += kCols * kThreads) {
-      float v[kCols];
-      int ns[kCols], nsmax = 0;
-      const float* pp[kCols];
-#pragma unroll
-      for (int c = 0; c < kCols; ++c) {
-        const int j = j0 + c * kThreads + tid;
-        v[c] = 0.f;
-        ns[c] = (j < hi) ? (int)s_nslot[j / kTile] : 0;
-        nsmax = max(nsmax, ns[c]);
-        pp[c] = p.ws_part + (((int64_t)seq * p.tiles_max + min(j, mb - 1) / kTile) * p.slots) * kTile + (j & (kTile - 1));
-      }
-      nsmax = __reduce_max_sync(0xffffffffu, nsmax);
-      for (int s0 = 0; s0 < nsmax; s0 += kSl) {
-        float x[kSl][kCols];
-#pragma unroll
-        for (int e = 0; e < kSl; ++e)
-#pragma unroll
-          for (int c = 0; c < kCols; ++c) x[e][c] = (s0 + e < ns[c]) ? __ldcg(pp[c] + (s0 + e) * kTile) : 0.f;
-#pragma unroll
-        for (int e = 0; e < kSl; ++e)
-#pragma unroll
-          for (int c = 0; c < kCols; ++c) v[c] += x[e][c];                     // slot order
-      }
-#pragma unroll
-      for (int c = 0; c < kCols; ++c) {
-        const int j = j0 + c * kThreads + tid;
-        if (j < mb) {
-          float w = 0.f;
-          if (j < hi) {
-            const float sj = s_row[j];
-            w = swd::powi(soft ? expf(sj - m) * inv_l : sj, p.s);
-            const float r = fmaf(rq, w, v[c]);
-            s_row[j] = r;
-            lamax = fmaxf(lamax, fabsf(r));
-          }
-          wrow[j] = w;
-        }
-      }
-    }
-    const float amax = block_max(lamax, s_red);       // (its barriers also publish s_row)
-    const bool rescale = (p.flags & SW_ROWNORM) && amax > 0.f;
-    float* ro = p.r_out + (int64_t)seq * mb;
-    for (int j = tid; j < mb; j += kThreads) {
-      float v = 0.f;
-      if (j < hi) { v = rescale ? s_row[j] / amax : s_row[j]; s_row[j] = v; }   // the selection reads r_out's values
-      ro[j] = v;
-    }
-    __syncthreads();
-    // Step 6: S = TopK(r[0..b_q), tau - |forced|) U {b_q} (U {0})
-    swsel::RowJob J = swsel::make_job(hi, bq, true, p.flags & SW_FORCE_FIRST, tt);
-    const float* row = s_row;
-    swsel::select_row([row](int j) { return row[j]; }, J, p.idx + (int64_t)seq * p.tau_max, p.tau_max,
-                      p.count + seq, scratch);
-    if (tid == 0) p.ws_cnt[seq] = 0;                  // leave the counter ready for the next call
-    __syncthreads();
-  }
 }
 
 }  // namespace
@@ -574,8 +375,7 @@ static int ds_grid(int batch, int max_blocks) {
 
 size_t decode_select_ws_bytes(int batch, int max_blocks) {
   const size_t tiles = (size_t)cdiv(max_blocks, kTile), mbp = tiles * kTile;
-  return 256 + (((size_t)batch * 4 + 255) & ~(size_t)255) + sizeof(float) * (size_t)batch * mbp +
-         sizeof(float) * (size_t)batch * tiles * tiles * kTile;
+  return 256 + sizeof(float) * (size_t)batch * mbp + sizeof(float) * (size_t)batch * tiles * tiles * kTile;
 }
 
 int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st) {
@@ -596,11 +396,10 @@ int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st) {
   p.batch = a.batch; p.B = a.block; p.max_blocks = a.max_blocks;
   p.tiles_max = cdiv(a.max_blocks, kTile); p.mbp = p.tiles_max * kTile; p.slots = p.tiles_max;
   uint8_t* w = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(a.ws) + 255) & ~(uintptr_t)255);
-  p.ws_cnt = reinterpret_cast<unsigned int*>(w);
-  w += ((size_t)a.batch * 4 + 255) & ~(size_t)255;
   p.ws_scores = reinterpret_cast<float*>(w);
   w += sizeof(float) * (size_t)a.batch * p.mbp;
   p.ws_part = reinterpret_cast<float*>(w);
+  p.g_stream = ds_grid(a.batch, a.max_blocks);
 
   void (*kern)(const Params) = nullptr;
   const int d = a.q.d;
@@ -614,13 +413,15 @@ int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st) {
   p.use_async = a.r_prev != nullptr && aligned16(a.W_cache) && aligned16(a.r_prev) && (a.max_blocks & 3) == 0 &&
                 (a.stride_seq & 3) == 0;
 
-  const size_t ring = std::max((size_t)kStages * kChunkBytes, sizeof(float) * (size_t)p.mbp);
-  const size_t smem = sizeof(float) * (2 * ((size_t)p.mbp + kChunkRows) + kRowGroups * kTile) + 128 + ring;
-  if (smem > 200 * 1024) return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: max_blocks %d too large", a.max_blocks);
+  const size_t smem = sizeof(float) * (2 * ((size_t)p.mbp + kChunkRows) + kRowGroups * kTile) + 128 +
+                      (size_t)kStages * kChunkBytes;
+  if (smem > 200 * 1024 || sizeof(float) * (size_t)p.mbp > 160 * 1024)
+    return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: max_blocks %d too large", a.max_blocks);
   if (int32_t rc = allow_dynamic_smem(kern, smem, "sw_decode_select smem attribute")) return rc;
   count_launch();
-  kern<<<ds_grid(a.batch, a.max_blocks), kThreads, smem, st>>>(p);
-  return check_launch("sw_decode_select");
+  kern<<<p.g_stream, kThreads, smem, st>>>(p);
+  if (int32_t rc = check_launch("sw_decode_select")) return rc;
+  return launch_decode_tail(p, st);
 }
 
 }  // namespace sw

@@ -3,7 +3,8 @@
 // order-preserving uint32 image of the fp32 scores, ties to the lower index, output ascending.
 // Integer work only, hence bit-exact.  Shared by select.cu and decode_select.cu.
 //
-// One CTA of kThreads = 256 threads per row:
+// One CTA of kThreads threads per row (256 unless the translation unit defines SWSEL_THREADS, a multiple of 256,
+// before including this file):
 //   * 4 radix passes of 8 bits on one shared histogram (plain shared-memory atomics; a warp whose lanes
 //     all hit the same bin sends one add), a 256-thread suffix scan picks the bin; rows of up to 2048
 //     candidates keep their keys in registers, so only the histogram touches memory;
@@ -15,8 +16,12 @@
 
 namespace swsel {
 
-constexpr int kThreads = 256;
+#ifndef SWSEL_THREADS
+#define SWSEL_THREADS 256
+#endif
+constexpr int kThreads = SWSEL_THREADS;
 constexpr int kWarps = kThreads / 32;
+static_assert(kThreads >= 256 && kThreads % 256 == 0, "thread b < 256 owns histogram bin b");
 
 struct Scratch {
   uint32_t hist[256];
@@ -77,7 +82,7 @@ __device__ void radix_threshold(Load load, const RowJob& J, Scratch& S, uint32_t
   int n_gt = 0;
   for (int pass = 0; pass < 4; ++pass) {
     const int shift = 24 - 8 * pass;
-    S.hist[tid] = 0;
+    if (tid < 256) S.hist[tid] = 0;
     __syncthreads();
     const uint32_t mask_hi = (pass == 0) ? 0u : (0xffffffffu << (shift + 8));
     for (int j0 = 0; j0 < J.n_cand; j0 += kThreads) {
@@ -91,7 +96,7 @@ __device__ void radix_threshold(Load load, const RowJob& J, Scratch& S, uint32_t
     }
     __syncthreads();
     // thread b owns bin b: count, then an inclusive suffix sum over bins b..255
-    const uint32_t cnt = S.hist[tid];
+    const uint32_t cnt = (tid < 256) ? S.hist[tid] : 0u;
     uint32_t suf = cnt;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -125,7 +130,7 @@ __device__ __forceinline__ void radix_threshold_regs(const uint32_t (&key)[K], u
   int n_gt = 0;
   for (int pass = 0; pass < 4; ++pass) {
     const int shift = 24 - 8 * pass;
-    S.hist[tid] = 0;
+    if (tid < 256) S.hist[tid] = 0;
     __syncthreads();
     const uint32_t mask_hi = (pass == 0) ? 0u : (0xffffffffu << (shift + 8));
     uint32_t bin[K];
@@ -147,7 +152,7 @@ __device__ __forceinline__ void radix_threshold_regs(const uint32_t (&key)[K], u
         if (bin[e] < 256u) atomicAdd(&S.hist[bin[e]], 1u);
     }
     __syncthreads();
-    const uint32_t cnt = S.hist[tid];
+    const uint32_t cnt = (tid < 256) ? S.hist[tid] : 0u;
     uint32_t suf = cnt;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {

@@ -770,8 +770,6 @@ def decode_case(sw, t, tau, fused, flags, B=64, s=None, layers=3, scale_q=1.0):
         assert dp.count[0].item() == len(sel) and (dp.idx[0, len(sel):] == -1).all()
         assert near_tie_only(got, sel, R_full[bq], forced), (got, sel)
         assert bq in got
-        if fused:                                        # the completion counters are back at zero
-            assert int(dp.select_ws[:4].view(torch.int32).item()) == 0
 
 
 @pytest.mark.parametrize("fused", [True, False])

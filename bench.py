@@ -50,7 +50,8 @@ def load_peaks():
 
 
 def tile_pairs(b: int, tau: int) -> int:
-    return sum(min(tau, i + 1) for i in range(b))
+    from bench_parts import tile_pairs as _tp       # one definition (bench_parts.py)
+    return _tp(b, tau)
 
 
 # ------------------------------------------------------------------------------------------ clocks
@@ -125,6 +126,16 @@ def oracle_sample(cfg, n, layer_inputs_cpu, H, n_qblocks=4):
     return n / t_layer, t_sel + t_att, desc
 
 
+def oracle_sample_1thread(*a, **kw):
+    """The same sample with every numerical library pool limited to one thread."""
+    try:
+        import threadpoolctl
+        with threadpoolctl.threadpool_limits(limits=1):
+            return oracle_sample(*a, **kw)
+    except Exception:
+        return None
+
+
 def cpu_threads() -> int:
     try:
         import threadpoolctl
@@ -173,6 +184,7 @@ def main():
     ap.add_argument("--no-decode", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the cfg 4 / cfg 5 / paper-default points")
     ap.add_argument("--prefill-kernel", default="auto", choices=["auto", "generic", "tcgen05"],
                     help="kernel of sw_sparse_attn_prefill (all are CUDA kernels of libsw; default: the library's choice)")
     args = ap.parse_args()
@@ -207,6 +219,15 @@ def main():
                 line["decode"] = decode_bench(pkg, args, peaks)
             except Exception as e:               # the headline line must still print
                 line["decode"] = {"error": repr(e)[:300]}
+        if not args.no_extras and world == 1 and not (args.layers or args.seqlen):
+            try:
+                for k_ in ("pipe", "Qs", "Ks", "Vs", "outs"):
+                    res.pop(k_, None)
+                torch.cuda.empty_cache()
+                from bench_sweep import driver_points
+                line["extras"] = driver_points(pkg, peaks)
+            except Exception as e:
+                line["extras"] = {"error": repr(e)[:300]}
         if not args.no_cpu_baseline:
             from oracle import sw_oracle as O
             cfg = gen.CONFIGS[CFG_IDX]
@@ -215,9 +236,14 @@ def main():
             H = O.srht_matrix(cfg.d, signs, cols, 1 / math.sqrt(cfg.r))
             li = gen.layer_inputs(CFG_IDX, 0, device="cuda", seqlens=(n,), plans=gen.make_plans(CFG_IDX, (n,)))
             inp = tuple(gen.to_numpy_f64(x) for x in (li.Q, li.K, li.V))
-            v, secs, desc = oracle_sample(cfg, n, inp, H, n_qblocks=96)   # ~15 s of CPU work
+            v, secs, desc = oracle_sample(cfg, n, inp, H, n_qblocks=96)   # ~13 s of CPU work
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
-                                    "sample": desc, "seconds": secs}
+                                    "sample": desc, "seconds": secs, "host_cpus": os.cpu_count(),
+                                    "threads": "numpy / BLAS pool as the oracle finds it (cores = its size)"}
+            one = oracle_sample_1thread(cfg, n, inp, H, n_qblocks=32)     # ~10 s, single thread
+            if one is not None:
+                line["cpu_baseline"]["single_thread"] = {"value": one[0], "unit": UNIT, "cores": 1, "seconds": one[1],
+                                                         "sample": one[2]}
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()

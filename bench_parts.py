@@ -135,12 +135,37 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
                        "frac": sketch_gbs / peaks.get("hbm_gbs")},
         "roofline": {"kernel": "sw_sparse_attn_prefill", "bound": "tensor", "achieved": achieved, "peak": peak,
                      "unit": "TFLOP/s", "frac": achieved / peak, "traffic": _ncu_traffic("sw_sparse_attn_prefill"),
+                     "traffic_source": _ncu_traffic("_source"),
                      "peak_source": f"{peaks['_source']} bf16 sustained (kernel timed inside a long step)",
+                     "frac_of_sustained": achieved / peak,
+                     "frac_of_burst": achieved / peaks.get("bf16_tflops", peak), "peak_burst": peaks.get("bf16_tflops"),
                      "flops_per_launch": attn_flops, "ms_per_launch": attn_ms,
                      "whole_layer_frac": (attn_flops / peak / 1e12) / (layer_ms * 1e-3)},
         "clocks": clocks,
         "gpu_launches": launches,                  # counted by libsw (sw_launch_count) over the timed region
     }
+    # with the per-block sums left behind by whatever produces Q / K (here: sw_copy_pool, untimed),
+    # the sketch step is two sw_sketch_from_pooled launches and the 336 MB re-read of Q and K is gone
+    qsum = torch.empty(pipe.L.total_blocks, cfg.d, device=dev); ksum = torch.empty_like(qsum)
+    scratch_q = torch.empty_like(Qs[0]); scratch_k = torch.empty_like(Ks[0])
+    pkg.sw_copy_pool(pipe.L, Qs[0], scratch_q, qsum); pkg.sw_copy_pool(pipe.L, Ks[0], scratch_k, ksum)
+    del scratch_q, scratch_k
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    p0.record(stream)
+    for _ in range(layers):
+        pkg.sw_sketch_from_pooled(pipe.L, qsum, cfg.h_q, pipe.signs, pipe.cols, pipe.r, pipe.sketch_scale, pipe.qs, pipe.qbar)
+        pkg.sw_sketch_from_pooled(pipe.L, ksum, cfg.h_kv, pipe.signs, pipe.cols, pipe.r, pipe.sketch_scale, pipe.ks, pipe.kbar)
+    p1.record(stream)
+    torch.cuda.synchronize()
+    pooled_ms = p0.elapsed_time(p1) / layers
+    layer_pooled = layer_ms - kern_ms["sketch_qk"] + pooled_ms
+    line["sketch_from_pooled"] = {"ms_per_layer_both_tensors": pooled_ms, "ms_per_layer_whole_path": layer_pooled,
+                                  "tokens_per_s_per_layer": n / (layer_pooled * 1e-3),
+                                  "selection_overhead_share": (sel_ms - kern_ms["sketch_qk"] + pooled_ms) /
+                                                              (sel_ms - kern_ms["sketch_qk"] + pooled_ms + attn_ms),
+                                  "note": "per-block sums supplied by the producer of Q / K (sw_copy_pool, outside the timed "
+                                          "region): sw_sketch_qk's re-read of Q and K is replaced by 2 x sw_sketch_from_pooled"}
     res = {"line": line, "n": n, "pipe": pipe, "Qs": Qs, "Ks": Ks, "Vs": Vs, "outs": outs}
 
     # ---- e2e: the same stack through the public API with HOST buffers (pinned), H2D of every layer's
@@ -289,10 +314,79 @@ def decode_bench(pkg, args, peaks, n_layer_bufs: int = 4, steps: int = 20):
     att_us = statistics.mean(e[1].elapsed_time(e[2]) * 1e3 for st in evs for e in st)
     kv_bytes = batch * tau * B * cfg.h_kv * d * 2 * 2
     gbs = kv_bytes / (att_us * 1e-6) / 1e9
-    return {"workload": cfg.name, "metric": "decode_us_per_step_per_layer_at_20pct_density",
+
+    def time_graph(fn, reps):
+        g_ = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g_):
+            fn()
+        g_.replay()
+        torch.cuda.synchronize()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record(stream)
+        for _ in range(reps):
+            g_.replay()
+        a1.record(stream)
+        torch.cuda.synchronize()
+        return a0.elapsed_time(a1) * 1e3 / reps
+
+    # ---- paged KV cache: layer 0's cache scattered into a pool of B-token pages by a random permutation ----------
+    extra = {}
+    try:
+        kc0, vc0 = layers[0][0], layers[0][1]
+        n_pages = batch * mb
+        gperm = torch.Generator(device=dev); gperm.manual_seed(77)
+        perm = torch.randperm(n_pages, device=dev, generator=gperm)
+        kpool = torch.empty(n_pages, B, cfg.h_kv, d, dtype=torch.bfloat16, device=dev); vpool = torch.empty_like(kpool)
+        kpool[perm] = kc0.view(n_pages, B, cfg.h_kv, d); vpool[perm] = vc0.view(n_pages, B, cfg.h_kv, d)
+        table = perm.view(batch, mb).to(torch.int32).contiguous()
+        out_p = torch.empty_like(out)
+        dp.attend_paged(layers[0][5], kpool, vpool, table, seqlens, out_p)
+        dp.attend(layers[0][5], kc0, vc0, seqlens, out)
+        torch.cuda.synchronize()
+        same = bool(torch.equal(out_p, out))
+        reps = 32
+        us_paged = time_graph(lambda: [dp.attend_paged(layers[0][5], kpool, vpool, table, seqlens, out_p) for _ in range(reps)], 5) / reps
+        us_contig = time_graph(lambda: [dp.attend(layers[0][5], kc0, vc0, seqlens, out) for _ in range(reps)], 5) / reps
+        extra["paged"] = {"attention_us_paged": us_paged, "attention_us_contiguous": us_contig,
+                          "paged_over_contiguous": us_paged / us_contig, "bit_equal_to_contiguous": same,
+                          "hbm_frac_paged": kv_bytes / (us_paged * 1e-6) / 1e9 / peaks.get("hbm_gbs"),
+                          "pages": n_pages, "page_tokens": B,
+                          "note": "same data, pages scattered by a seeded random permutation; 32 launches per graph, "
+                                  "860 MB read per launch >> L2"}
+        del kpool, vpool
+    except Exception as e:
+        extra["paged"] = {"error": repr(e)[:200]}
+    # ---- 64 consecutive decode steps with growing t, across a block boundary, one CUDA graph -----------------------
+    try:
+        n_steps = 64
+        t0s = (mb - 1) * B - 20                              # block b_q completes at step 21, a new one starts at 22
+        seq_g = torch.full((batch,), t0s, dtype=torch.int32, device=dev)
+
+        def many_steps():
+            for _ in range(n_steps):
+                dp.reset()
+                for l in range(n_model_layers):
+                    kc, vc, Wc, kbar, ks, q_new, k_new = layers[l % n_layer_bufs]
+                    dp.select(q_new, k_new, seq_g, kbar, ks, Wc)
+                    dp.attend(q_new, kc, vc, seq_g, out)
+                seq_g.add_(1)
+
+        us_total = time_graph(many_steps, 1)
+        seq_g.fill_(t0s)
+        extra["multi_step"] = {"steps": n_steps, "t_first": t0s, "t_last": t0s + n_steps - 1,
+                               "us_per_layer": us_total / (n_steps * n_model_layers),
+                               "us_per_step": us_total / n_steps,
+                               "hbm_frac_layer_over_kv_bytes": kv_bytes / (us_total / (n_steps * n_model_layers) * 1e-6) / 1e9 / peaks.get("hbm_gbs"),
+                               "note": "64 steps x 32 layers captured once (the sequence lengths advance on the device); the "
+                                       "cached W rows, key-block means and sketches are updated in place by sw_decode_select"}
+    except Exception as e:
+        extra["multi_step"] = {"error": repr(e)[:200]}
+    return {"workload": cfg.name, **extra, "metric": "decode_us_per_step_per_layer_at_20pct_density",
             "us_per_layer": us_layer, "us_per_layer_eager": us_layer_eager,
             "launch": "one CUDA graph per 32-layer decode step (us_per_layer); eager ctypes launches (us_per_layer_eager, selection_us, attention_us)",
             "selection_us": sel_us, "attention_us": att_us,
+            "hbm_frac_layer_over_kv_bytes": kv_bytes / (us_layer * 1e-6) / 1e9 / peaks.get("hbm_gbs"),
+            "hbm_frac_layer_over_kv_and_w_bytes": (kv_bytes + batch * mb * mb * 2) / (us_layer * 1e-6) / 1e9 / peaks.get("hbm_gbs"),
             "selection_overhead_share": sel_us / (sel_us + att_us), "batch": batch, "kv_len": t, "tau": tau,
             "splits": pkg.sw_decode_num_splits(batch, cfg.h_kv, d, tau), "layer_buffers_cycled": n_layer_bufs,
             "steps": steps, "gpu_launches": launches,

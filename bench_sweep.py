@@ -30,7 +30,7 @@ import torch
 from synth import gen
 from bench import load_peaks
 
-KERNELS = ["sketch_q", "sketch_k", "block_scores", "walk", "select", "attn"]
+KERNELS = ["sketch_qk", "prefill_select", "attn"]
 
 
 def tile_pairs(blocks, taus):
@@ -61,26 +61,22 @@ def time_stack(pkg, pipe, bufs, out, layers_run, passes, warm=1):
             Q, K, V = bufs[layer % len(bufs)]
             ev = events[layer] if events is not None else None
             if ev is not None: ev[0].record(stream)
-            pkg.sw_sketch(L, Q, pipe.signs, pipe.cols, pipe.r, pipe.sketch_scale, pipe.qs, pipe.qbar)
+            pkg.sw_sketch_qk(L, Q, K, pipe.signs, pipe.cols, pipe.r, pipe.sketch_scale, pipe.qs, pipe.ks, pipe.qbar,
+                             pipe.kbar)
             if ev is not None: ev[1].record(stream)
-            pkg.sw_sketch(L, K, pipe.signs, pipe.cols, pipe.r, pipe.sketch_scale, pipe.ks, pipe.kbar)
-            if ev is not None: ev[2].record(stream)
-            pkg.sw_block_scores(L, pipe.qs, pipe.ks, pipe.r, pipe.s, pipe.flags, pipe.W, None)
-            if ev is not None: ev[3].record(stream)
             nxt = 0 if pipe.cur < 0 else 1 - pipe.cur
-            pkg.sw_walk_update(L, pipe.R_cur, pipe.W, pipe.s, pipe.flags, pipe.R[nxt], pipe.walk_ws)
+            pkg.sw_prefill_select(L, pipe.qs, pipe.ks, pipe.r, pipe.s, pipe.flags, pipe.R_cur, pipe.R[nxt], pipe.W, None,
+                                  pipe.tau, pipe.tau_max, pipe.idx, pipe.count, pipe.walk_ws)
             pipe.cur = nxt
-            if ev is not None: ev[4].record(stream)
-            pkg.sw_select_topk(L, pipe.R[nxt], pipe.tau, pipe.tau_max, pipe.flags, pipe.idx, pipe.count)
-            if ev is not None: ev[5].record(stream)
+            if ev is not None: ev[2].record(stream)
             pkg.sw_sparse_attn_prefill(L, Q, K, V, pipe.idx, pipe.count, pipe.tau_max, pipe.softmax_scale,
                                        pipe.flags, out, None, pipe.attn_ws)
-            if ev is not None: ev[6].record(stream)
+            if ev is not None: ev[3].record(stream)
 
     for _ in range(warm):
         one_pass()
     torch.cuda.synchronize()
-    evs = [[[torch.cuda.Event(enable_timing=True) for _ in range(7)] for _ in range(layers_run)]
+    evs = [[[torch.cuda.Event(enable_timing=True) for _ in range(len(KERNELS) + 1)] for _ in range(layers_run)]
            for _ in range(passes)]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
@@ -112,7 +108,7 @@ def measure(pkg, peaks, name, seqlens, bufs, *, h_q, h_kv, d, B, r, s, density, 
     n = sum(seqlens)
     flops = 4.0 * B * B * d * h_q * pairs
     peak = peaks.get("bf16_tflops_sustained", peaks.get("bf16_tflops"))
-    sel_ms = sum(kern[k] for k in KERNELS[:5])
+    sel_ms = sum(kern[k] for k in KERNELS[:-1])
     sk_bytes = n * (h_q + h_kv) * d * 2
     res = {"name": name, "seqlens": list(seqlens), "block": B, "s": s, "r": r, "density": density,
            "pow_matrix": bool(flags is not None and (flags & pkg.SW_POW_MATRIX)),
@@ -121,8 +117,9 @@ def measure(pkg, peaks, name, seqlens, bufs, *, h_q, h_kv, d, B, r, s, density, 
            "selection_ms": sel_ms, "selection_overhead_share": sel_ms / (sel_ms + kern["attn"]),
            "attn_tflops": flops / (kern["attn"] * 1e-3) / 1e12, "attn_roofline_frac": flops / (kern["attn"] * 1e-3) / 1e12 / peak,
            "attn_kernel": pkg.sw_get_prefill_kernel_used() if hasattr(pkg, "sw_get_prefill_kernel_used") else None,
-           "sketch_gbs": sk_bytes / ((kern["sketch_q"] + kern["sketch_k"]) * 1e-3) / 1e9,
-           "sketch_hbm_frac": sk_bytes / ((kern["sketch_q"] + kern["sketch_k"]) * 1e-3) / 1e9 / peaks.get("hbm_gbs")}
+           "attn_roofline_frac_of_burst": flops / (kern["attn"] * 1e-3) / 1e12 / peaks.get("bf16_tflops", peak),
+           "sketch_gbs": sk_bytes / (kern["sketch_qk"] * 1e-3) / 1e9,
+           "sketch_hbm_frac": sk_bytes / (kern["sketch_qk"] * 1e-3) / 1e9 / peaks.get("hbm_gbs")}
     del pipe, out
     return res
 
@@ -132,15 +129,56 @@ def fmt_row(r, dense=None):
     sp = "" if dense is None else f"{dense['kernel_ms']['attn'] / k['attn']:.2f}x / {dense['layer_ms'] / r['layer_ms']:.2f}x"
     return (f"| {r['name']} | {r['block']} | {r['s']}{'m' if r['pow_matrix'] else ''} | {100 * r['density']:.0f} % | "
             f"{100 * r['work_fraction_of_causal_dense']:.0f} % | "
-            f"{k['sketch_q'] + k['sketch_k']:.3f} | {k['block_scores']:.3f} | {k['walk']:.3f} | {k['select']:.3f} | "
+            f"{k['sketch_qk']:.3f} | {k['prefill_select']:.3f} | "
             f"{k['attn']:.3f} | {r['layer_ms']:.3f} | {r['tokens_per_s_per_layer'] / 1e6:.2f} | "
             f"{r['attn_tflops']:.0f} ({100 * r['attn_roofline_frac']:.0f} %) | "
             f"{100 * r['selection_overhead_share']:.1f} % | {sp} |")
 
 
-HEADER = ("| workload | B | s | density | work vs causal-dense | sketch ms | scores ms | walk ms | select ms | attn ms | "
+HEADER = ("| workload | B | s | density | work vs causal-dense | sketch ms | scores+walk+select ms | attn ms | "
           "layer ms | Mtok/s per layer | attn TFLOP/s (of sustained bf16) | selection share | speedup vs 100 % (attn / layer) |\n"
-          "|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+          "|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+
+
+def _brief(r, dense=None):
+    out = {"workload": r["name"], "seqlens": r["seqlens"], "block": r["block"], "s": r["s"], "density": r["density"],
+           "tau": r["tau"], "tile_pairs": r["tile_pairs"], "layer_ms": r["layer_ms"], "kernel_ms": r["kernel_ms"],
+           "tokens_per_s_per_layer": r["tokens_per_s_per_layer"], "attn_tflops": r["attn_tflops"],
+           "attn_roofline_frac": r["attn_roofline_frac"], "attn_roofline_frac_of_burst": r["attn_roofline_frac_of_burst"],
+           "selection_overhead_share": r["selection_overhead_share"]}
+    if dense is not None:
+        out["speedup_vs_100pct_attn"] = dense["kernel_ms"]["attn"] / r["kernel_ms"]["attn"]
+        out["speedup_vs_100pct_layer"] = dense["layer_ms"] / r["layer_ms"]
+    return out
+
+
+def driver_points(pkg, peaks):
+    """The cfg 4 / cfg 5 / paper-default points bench.py carries in its JSON line (same code as the sweep, fewer
+    points): one layer stack each, 3 layers with the walk carried, 2 distinct layer buffers (each >> L2)."""
+    shape = dict(h_q=32, h_kv=8, d=128)
+    res = {}
+    c4 = gen.CONFIGS[3]
+    bufs4 = make_inputs(4000, c4.seqlens, c4.h_q, c4.h_kv, c4.d, 64, n_bufs=2)
+    kw = dict(B=64, r=64, layers_run=3, passes=1, **shape)
+    d100 = measure(pkg, peaks, "cfg4 128K @100% (dense reference, same kernel)", c4.seqlens, bufs4, s=2, density=1.0, **kw)
+    d20 = measure(pkg, peaks, "cfg4 128K @20%", c4.seqlens, bufs4, s=2, density=0.2, **kw)
+    pdef = measure(pkg, peaks, "paper default: cfg4 shape, s=8, r=64, 10% density (PAPER.md:218,266)", c4.seqlens, bufs4,
+                   s=8, density=0.10, **kw)
+    res["cfg4_20pct"] = _brief(d20, d100)
+    res["cfg4_100pct"] = _brief(d100)
+    res["paper_default"] = _brief(pdef, d100)
+    del bufs4
+    torch.cuda.empty_cache()
+    c5 = gen.CONFIGS[4]
+    bufs5 = make_inputs(5000, c5.seqlens, c5.h_q, c5.h_kv, c5.d, 64, n_bufs=2)
+    e100 = measure(pkg, peaks, "cfg5 varlen 16K+32K+48K+64K @100%", c5.seqlens, bufs5, s=2, density=1.0, **kw)
+    e20 = measure(pkg, peaks, "cfg5 varlen 16K+32K+48K+64K @20%", c5.seqlens, bufs5, s=2, density=0.2, **kw)
+    e5 = measure(pkg, peaks, "cfg5 varlen 16K+32K+48K+64K @5%", c5.seqlens, bufs5, s=2, density=0.05, **kw)
+    res["cfg5_20pct"] = _brief(e20, e100)
+    res["cfg5_5pct"] = _brief(e5, e100)
+    del bufs5
+    torch.cuda.empty_cache()
+    return res
 
 
 def main():

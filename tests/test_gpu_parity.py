@@ -902,21 +902,21 @@ def check_overlap(idx_gpu, cnt_gpu, sel, R_ref):
     return inter / tot
 
 
-@pytest.mark.parametrize("cfg_idx,seqlens,layers", [(0, None, 2), (1, (2048 + 19,), 4), (4, (192, 700, 1024), 3)])
-def test_end_to_end_prefill_stack(sw, cfg_idx, seqlens, layers):
-    """Whole hot path, several layers with the walk carried across them; cfg 1 in full, cfg 2 / cfg 5 recipes
-    at reduced length (full-size samples live in test_gpu_fullsize.py)."""
+def run_prefill_stack(sw, cfg_idx, seqlens, layers, *, flags=O.DEFAULT_FLAGS, s=None, density=None, fused=True):
     cfg = gen.CONFIGS[cfg_idx]
+    s = cfg.s if s is None else s
+    density = cfg.density if density is None else density
     seqlens = tuple(cfg.seqlens if seqlens is None else seqlens)
     signs, cols, H = H_of(cfg.d, cfg.r, seed=cfg_idx + 1)
     dtype = torch.float32 if cfg.dtype == "f32" else torch.bfloat16
-    pipe = sw.PrefillPipeline(seqlens, cfg.h_q, cfg.h_kv, cfg.d, cfg.B, cfg.r, cfg.s, cfg.density, signs, cols,
+    pipe = sw.PrefillPipeline(seqlens, cfg.h_q, cfg.h_kv, cfg.d, cfg.B, cfg.r, s, density, signs, cols, flags=flags,
                               dtype=dtype, keep_A=True)
     plans = gen.make_plans(cfg_idx, seqlens) if cfg.planted else None
     R_ref = [None] * len(seqlens)
+    overlaps = []
     for layer in range(layers):
         li = gen.layer_inputs(cfg_idx, layer, device="cuda", seqlens=seqlens, plans=plans)
-        out = pipe.layer(li.Q, li.K, li.V)
+        out = pipe.layer(li.Q, li.K, li.V, fused=fused)
         torch.cuda.synchronize()
         Qn, Kn, Vn = (gen.to_numpy_f64(x) for x in (li.Q, li.K, li.V))
         idx_gpu, cnt_gpu = pipe.idx.cpu().numpy(), pipe.count.cpu().numpy()
@@ -925,20 +925,48 @@ def test_end_to_end_prefill_stack(sw, cfg_idx, seqlens, layers):
         tlo = blo = qlo = 0
         for si, n in enumerate(seqlens):
             b = O.num_blocks(n, cfg.B)
-            tau = O.tau_from_density(cfg.density, b)
-            sel = O.prefill_selection(Qn[tlo:tlo + n], Kn[tlo:tlo + n], R_ref[si], B=cfg.B, H_d=H, s=cfg.s, tau=tau)
+            tau = O.tau_from_density(density, b)
+            sel = O.prefill_selection(Qn[tlo:tlo + n], Kn[tlo:tlo + n], R_ref[si], B=cfg.B, H_d=H, s=s, tau=tau, flags=flags)
             R_ref[si] = sel.R
             assert rowwise_close(pipe.qs[blo:blo + b].cpu().numpy(), sel.qs)
-            assert rowwise_close(pipe.W[qlo:qlo + b * b].cpu().numpy().reshape(b, b), sel.W)
+            assert rowwise_close(pipe.W[qlo:qlo + b * b].cpu().numpy().reshape(b, b), sel.A if flags & O.POW_MATRIX else sel.W)
             assert rowwise_close(R_gpu[qlo:qlo + b * b].reshape(b, b), sel.R)
             ov = check_overlap(idx_gpu[blo:blo + b], cnt_gpu[blo:blo + b], sel, sel.R)
-            assert ov >= 0.99, ov
+            overlaps.append(ov)
             heads = sorted(set([0, cfg.h_q // 2, cfg.h_q - 1]))
             qb = torch.as_tensor(Qn[tlo:tlo + n]).bfloat16().double().numpy()
             kb = torch.as_tensor(Kn[tlo:tlo + n]).bfloat16().double().numpy()
             vb = torch.as_tensor(Vn[tlo:tlo + n]).bfloat16().double().numpy()
             ref = O.sparse_attention(qb, kb, vb, idx_gpu[blo:blo + b], cnt_gpu[blo:blo + b], cfg.B,
-                                     1 / math.sqrt(cfg.d), q_heads=heads)
+                                     1 / math.sqrt(cfg.d), flags=flags, q_heads=heads)
             err = np.abs(got[tlo:tlo + n][:, heads] - ref[:, heads])
             assert err.max() <= ATT_MAX and err.mean() <= ATT_MEAN, (err.max(), err.mean())
             tlo += n; blo += b; qlo += b * b
+    return overlaps
+
+
+@pytest.mark.parametrize("fused", [True, False])
+@pytest.mark.parametrize("cfg_idx,seqlens,layers", [(0, None, 2), (1, (2048 + 19,), 4), (4, (192, 700, 1024), 3)])
+def test_end_to_end_prefill_stack(sw, cfg_idx, seqlens, layers, fused):
+    """Whole hot path, several layers with the walk carried across them; cfg 1 in full, cfg 2 / cfg 5 recipes
+    at reduced length (full-size samples live in test_gpu_fullsize.py).  ``fused`` = sw_sketch_qk +
+    sw_prefill_select, otherwise the plain calls."""
+    ov = run_prefill_stack(sw, cfg_idx, seqlens, layers, fused=fused)
+    assert min(ov) >= 0.99, ov
+
+
+@pytest.mark.parametrize("name,flags,s,density", [
+    ("matrix power s=2 (P4, PAPER.md:25,31)", O.DEFAULT_FLAGS | O.POW_MATRIX, 2, 0.20),
+    ("raw signed scores (P5, PAPER.md:782-784)", O.DEFAULT_FLAGS & ~O.SCORE_SOFTMAX, 2, 0.20),
+    ("paper default s=8, r=64, 10% density (PAPER.md:218,266)", O.DEFAULT_FLAGS, 8, 0.10),
+    ("no row rescale (P9 off)", O.DEFAULT_FLAGS & ~O.ROWNORM, 2, 0.20),
+])
+def test_end_to_end_prefill_stack_other_readings(sw, name, flags, s, density):
+    """The readings other than the default, end to end (cfg-2 recipe, n ~ 4K, 3 layers with the walk carried):
+    values within 1e-3 of the row max at every stage, selected sets equal to the oracle's up to near-ties
+    (north_star).  The >= 99 % overlap figure is asserted where the scores spread the candidates (default,
+    matrix power, no rescale); at s = 8 the element-wise power pushes most candidates of a row below 1e-3 of its
+    maximum, where north_star's own criterion calls them ties, so the overlap is only reported there."""
+    ov = run_prefill_stack(sw, 1, (4096 + 37,), 3, flags=flags, s=s, density=density)
+    if s < 8 and (flags & O.SCORE_SOFTMAX):
+        assert min(ov) >= 0.99, (name, ov)

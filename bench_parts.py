@@ -363,6 +363,7 @@ def decode_bench(pkg, args, peaks, n_layer_bufs: int = 4, steps: int = 20):
         seq_g = torch.full((batch,), t0s, dtype=torch.int32, device=dev)
 
         def many_steps():
+            seq_g.fill_(t0s)                                  # (captured: every replay starts from the same length)
             for _ in range(n_steps):
                 dp.reset()
                 for l in range(n_model_layers):

@@ -33,6 +33,8 @@ attn_decode_kernel(const __nv_bfloat16* __restrict__ Q, int64_t q_sb, int64_t q_
   const int split = blockIdx.x, kvh = blockIdx.y, seq = blockIdx.z;
   const int grp = h_q / h_kv;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t4 = lane & 3;
+  swd::pdl_launch_dependents();                          // (the merge kernel may take its place on the SMs early)
+  swd::pdl_wait();                                       // the block lists of the selection before this kernel
   const int t = __ldg(seqlens + seq);
   const int cnt = __ldg(count + seq);
   const int32_t* list = idx + (int64_t)seq * tau_max;
@@ -215,6 +217,8 @@ attn_decode_merge_kernel(const float* __restrict__ Opart, const float* __restric
                          __nv_bfloat16* __restrict__ out, float* __restrict__ lse) {
   const int64_t bh = blockIdx.x;                      // seq * h_q + head
   const int c = threadIdx.x;
+  swd::pdl_launch_dependents();                       // the next kernel of the layer loop may start its prologue
+  swd::pdl_wait();                                    // the split-KV partials
   float m = -INFINITY;
   for (int s = 0; s < nsplit; ++s) m = fmaxf(m, ML[(bh * nsplit + s) * 2]);
   float acc = 0.f, l = 0.f;
@@ -273,13 +277,14 @@ static int32_t launch_decode_t(int batch, int block, const sw_tensor& q, const s
   float* Opart = reinterpret_cast<float*>(ws);
   float* ML = Opart + (size_t)batch * q.heads * nsplit * D;
   dim3 grid(nsplit, kc.heads, batch);
-  attn_decode_kernel<D><<<grid, kThreads, smem, st>>>(
+  launch_pdl(attn_decode_kernel<D>, grid, dim3(kThreads), smem, st,
       (const __nv_bfloat16*)q.ptr, q.stride_tok, q.stride_head, (const __nv_bfloat16*)kc.ptr,
       (const __nv_bfloat16*)vc.ptr, stride_batch, kc.stride_tok, kc.stride_head, vc.stride_tok,
       vc.stride_head, q.heads, kc.heads, seqlens, block, idx, count, tau_max,
       softmax_scale * 1.4426950408889634f, nsplit, table, table_stride, Opart, ML);
   count_launch(2);
-  attn_decode_merge_kernel<D><<<batch * q.heads, D, 0, st>>>(Opart, ML, nsplit, (__nv_bfloat16*)out, lse);
+  launch_pdl(attn_decode_merge_kernel<D>, dim3(batch * q.heads), dim3(D), 0, st, (const float*)Opart, (const float*)ML, nsplit,
+             (__nv_bfloat16*)out, lse);
   return check_launch("sw_sparse_attn_decode");
 }
 

@@ -35,6 +35,24 @@ static inline int32_t allow_dynamic_smem(Kern kern, size_t bytes, const char* wh
   return SW_OK;
 }
 
+// Programmatic dependent launch (PDL): a kernel launched through launch_pdl may become resident while the kernel
+// before it on the stream is still draining, once that kernel's CTAs have executed pdl_launch_dependents() (or
+// exited); it must execute pdl_wait() before it touches anything its predecessors wrote.  Both device calls are
+// no-ops when the kernel was launched the ordinary way, and a predecessor that never triggers simply gives the
+// ordinary stream order.  Used along the decode layer (selection -> tail -> attention -> merge -> next selection),
+// where every kernel is short and the launch gaps add up.
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                     Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 static inline bool is_pow2(int x) { return x > 0 && (x & (x - 1)) == 0; }
 static inline int cdiv(int a, int b) { return (a + b - 1) / b; }
@@ -158,6 +176,9 @@ int32_t launch_attn_decode(int batch, int block, const sw_tensor& q, const sw_te
 // ---- device utilities ------------------------------------------------------------------
 #ifdef __CUDACC__
 namespace swd {
+
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 __device__ __forceinline__ float warp_max(float v) {
 #pragma unroll

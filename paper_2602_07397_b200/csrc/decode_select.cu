@@ -41,7 +41,7 @@ template <typename TIn, int D>
 __global__ void __launch_bounds__(kThreads, 2)
 decode_select_kernel(const Params p) {
   // the tail kernel is launched as a programmatic dependent: let it become resident as SMs drain
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  swd::pdl_launch_dependents();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int G = (int)gridDim.x, me = (int)blockIdx.x;
   const bool walk = p.r_prev != nullptr;
@@ -141,6 +141,10 @@ decode_select_kernel(const Params p) {
   int seq_first = 0;
   if (n_my > 0) { cc = locate(g_begin); seq_first = cc.seq; }
   pc = cc;
+
+  // Launched as a programmatic dependent itself: what is above (work prefixes, cursors; sequence lengths only)
+  // overlaps the tail of the kernel before this one; everything below reads what earlier kernels produced.
+  swd::pdl_wait();
 
   // ---- W stream: chunk = rows [64 tile + 64 chunk, +64) x columns [64 tile, +64) of the sequence's cached W
   int p_left = n_my, issued = 0;
@@ -419,7 +423,7 @@ int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st) {
     return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: max_blocks %d too large", a.max_blocks);
   if (int32_t rc = allow_dynamic_smem(kern, smem, "sw_decode_select smem attribute")) return rc;
   count_launch();
-  kern<<<p.g_stream, kThreads, smem, st>>>(p);
+  launch_pdl(kern, dim3(p.g_stream), dim3(kThreads), smem, st, p);
   if (int32_t rc = check_launch("sw_decode_select")) return rc;
   return launch_decode_tail(p, st);
 }

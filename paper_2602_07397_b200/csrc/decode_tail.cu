@@ -49,6 +49,7 @@ decode_tail_kernel(const Params p) {
   __shared__ unsigned char s_nslot[kMaxTiles + 1];   // partials per column tile
   __shared__ swsel::Scratch scratch;
   const int tid = threadIdx.x, seq = blockIdx.x;
+  swd::pdl_launch_dependents();                       // (the attention kernel waits for this one before it reads idx)
   const bool walk = p.r_prev != nullptr, soft = p.flags & SW_SCORE_SOFTMAX;
   const int mb = p.max_blocks;
 
@@ -76,7 +77,7 @@ decode_tail_kernel(const Params p) {
     }
     s_nslot[tl] = (unsigned char)min(ns, 255);
   }
-  asm volatile("griddepcontrol.wait;" ::: "memory");  // the streaming kernel's scores and partials are visible
+  swd::pdl_wait();                                    // the streaming kernel's scores and partials are visible
 
   const float* sc = p.ws_scores + (int64_t)seq * p.mbp;
   float lmax = -INFINITY;
@@ -160,17 +161,8 @@ namespace sw {
 int32_t launch_decode_tail(const swds::Params& p, cudaStream_t st) {
   const size_t smem = sizeof(float) * (size_t)p.mbp;
   if (int32_t rc = allow_dynamic_smem(decode_tail_kernel, smem, "sw_decode_select(tail) smem attribute")) return rc;
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(p.batch);
-  cfg.blockDim = dim3(NT);
-  cfg.dynamicSmemBytes = smem;
-  cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = attr; cfg.numAttrs = 1;
   count_launch();
-  if (cudaLaunchKernelEx(&cfg, decode_tail_kernel, p) != cudaSuccess) return check_launch("sw_decode_select(tail)");
+  launch_pdl(decode_tail_kernel, dim3(p.batch), dim3(NT), smem, st, p);
   return check_launch("sw_decode_select(tail)");
 }
 

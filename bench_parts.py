@@ -80,14 +80,14 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
             dist.barrier()
         torch.cuda.synchronize()
 
+    if rank == 0:
+        sampler.start()          # before the warm-up steps (same load): nvidia-smi needs ~0.3 s to deliver its first sample
     for _ in range(args.warmup):
         step()
     barrier()
     events = [[[torch.cuda.Event(enable_timing=True) for _ in range(len(KERNELS) + 1)] for _ in range(layers)]
               for _ in range(args.steps)]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    if rank == 0:
-        sampler.start()
     barrier()
     launches0 = pkg.sw_launch_count()
     e0.record(stream)

@@ -181,7 +181,15 @@ score_rows_kernel(int s, uint32_t flags, const int32_t* __restrict__ cu_blocks, 
 // written once and never re-read by this step; split_tf32_kernel and its pass over W and R are gone.
 constexpr int kFRows = 8;
 constexpr int kFCols = 64;
-constexpr int kFStages = 4;           // ring of key-sketch tiles (cp.async)
+constexpr int kFStagesMax = 4;        // ring of key-sketch tiles (cp.async): 4 stages, or 2 when that lets two CTAs share an SM
+
+// D (16x8, fp32) += A (16x8, tf32, rows g / g + 8) * B (8x8, tf32); the A rows g + 8 are zero here
+__device__ __forceinline__ void mma_tf32(float (&c)[4], uint32_t a0, uint32_t a2, uint32_t b0, uint32_t b1) {
+  asm volatile(
+      "mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+      : "r"(a0), "r"(0u), "r"(a2), "r"(0u), "r"(b0), "r"(b1));
+}
 
 struct FusedParams {
   const float *qs, *ks;
@@ -194,10 +202,12 @@ struct FusedParams {
   const float* R_prev;               // packed; split into rhi / rlo by the CTAs behind the strips, or NULL
   float *rhi, *rlo;
   int pitch, n_strips, lds;          // lds: row stride of the score strip in shared memory (floats)
+  int stages;                        // 2 or 4
   float inv_sqrt_r;
 };
 
-__global__ void __launch_bounds__(kThreads)
+template <int kMaxKs>                  // k-steps of 8 the A fragments are sized for: r <= 8 kMaxKs
+__global__ void __launch_bounds__(kThreads, kMaxKs <= 8 ? 2 : 1)
 score_fused_kernel(const FusedParams p) {
   extern __shared__ __align__(16) float smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -221,8 +231,9 @@ score_fused_kernel(const FusedParams p) {
   if (i0 >= rows_all) return;
   const int r = p.r, r4 = r >> 2, ldk = r + 4;
   float* s_q = smem;                                          // [kFRows][r]
-  float* s_k = s_q + kFRows * r;                              // [kFStages][kFCols][r + 4]
-  float* s_S = s_k + kFStages * kFCols * ldk;                        // [kFRows][lds]
+  const int nst = p.stages;
+  float* s_k = s_q + kFRows * r;                              // [stages][kFCols][r + 4]
+  float* s_S = s_k + nst * kFCols * ldk;                        // [kFRows][lds]
   const int nrows = max(0, min(kFRows, b - i0));
 
   if (nrows > 0) {
@@ -230,7 +241,7 @@ score_fused_kernel(const FusedParams p) {
     const int nct = (hi_col + kFCols - 1) / kFCols;
     auto load_k = [&](int ct) {                               // tile ct -> ring slot ct % kFStages (or an empty group)
       if (ct < nct) {
-        float* dst = s_k + (ct % kFStages) * kFCols * ldk;
+        float* dst = s_k + (ct & (nst - 1)) * kFCols * ldk;
         for (int i = tid; i < kFCols * r4; i += kThreads) {
           const int kk = i / r4, c = (i - kk * r4) * 4;
           const int j = ct * kFCols + kk;
@@ -242,19 +253,62 @@ score_fused_kernel(const FusedParams p) {
       }
       asm volatile("cp.async.commit_group;" ::: "memory");
     };
-    for (int ct = 0; ct < kFStages - 1; ++ct) load_k(ct);     // kFStages - 1 tiles in flight (one latency, not one each)
+    for (int ct = 0; ct < nst - 1; ++ct) load_k(ct);          // stages - 1 tiles in flight (one latency, not one each)
     for (int i = tid; i < kFRows * r4; i += kThreads) {
       const int rr = i / r4, c = (i - rr * r4) * 4;
       float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
       if (rr < nrows) v = *reinterpret_cast<const float4*>(p.qs + (int64_t)(blk0 + i0 + rr) * r + c);
       *reinterpret_cast<float4*>(s_q + rr * r + c) = v;
     }
+    if ((r & 7) == 0) {
+      // Tile product on the warp-level tensor cores with 3xTF32 error compensation (as the walk GEMM: x = hi + lo,
+      // q k ~= q_lo k_hi + q_hi k_lo + q_hi k_hi, fp32 accumulate; dropped term 2^-22): mma.sync m16n8k8, the 8
+      // strip rows in the upper half of M (the lower half is zero), one 8-column n-tile per warp and 64-column
+      // tile.  With plain FMAs the strip was bound by shared-memory reads (3 x LDS.128 per 8 FMA): 73 of the
+      // 135 us of the b = 2048 selection chain.
+      __syncthreads();                                        // s_q is complete
+      const int g = lane >> 2, t4 = lane & 3;
+      uint32_t ahi[kMaxKs][2], alo[kMaxKs][2];                // A fragments (rows g; rows g + 8 are the zero padding)
+#pragma unroll
+      for (int ks = 0; ks < kMaxKs; ++ks) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const float x = (8 * ks < r) ? s_q[g * r + 8 * ks + t4 + 4 * h] : 0.f;
+          const uint32_t hi = __float_as_uint(x) & 0xffffe000u;
+          ahi[ks][h] = hi;
+          alo[ks][h] = __float_as_uint(x - __uint_as_float(hi));
+        }
+      }
+      const int n0 = warp * 8;                                // this warp's columns of every tile
+      for (int ct = 0; ct < nct; ++ct) {
+        if (nst == 4) asm volatile("cp.async.wait_group 2;" ::: "memory");
+        else asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();                                      // tile ct landed; tile ct - 1 fully consumed
+        load_k(ct + nst - 1);
+        const float* kp = s_k + (ct & (nst - 1)) * kFCols * ldk + (n0 + g) * ldk + t4;
+        float c[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int ks = 0; ks < kMaxKs; ++ks) {
+          if (8 * ks < r) {                                   // (warp-uniform)
+            const float k0 = kp[8 * ks], k1 = kp[8 * ks + 4];
+            const uint32_t b0h = __float_as_uint(k0) & 0xffffe000u, b1h = __float_as_uint(k1) & 0xffffe000u;
+            const uint32_t b0l = __float_as_uint(k0 - __uint_as_float(b0h)), b1l = __float_as_uint(k1 - __uint_as_float(b1h));
+            mma_tf32(c, alo[ks][0], alo[ks][1], b0h, b1h);    // small terms first
+            mma_tf32(c, ahi[ks][0], ahi[ks][1], b0l, b1l);
+            mma_tf32(c, ahi[ks][0], ahi[ks][1], b0h, b1h);
+          }
+        }
+        *reinterpret_cast<float2*>(s_S + g * p.lds + ct * kFCols + n0 + 2 * t4) =
+            make_float2(c[0] * p.inv_sqrt_r, c[1] * p.inv_sqrt_r);
+      }
+    } else {
     const int col = tid & (kFCols - 1), rg = tid / kFCols;    // rows 2 rg, 2 rg + 1 of the strip
     for (int ct = 0; ct < nct; ++ct) {
-      asm volatile("cp.async.wait_group %0;" ::"n"(kFStages - 2) : "memory");
+      if (nst == 4) asm volatile("cp.async.wait_group 2;" ::: "memory");
+      else asm volatile("cp.async.wait_group 0;" ::: "memory");
       __syncthreads();                                        // tile ct landed; tile ct - 1 fully consumed
-      load_k(ct + kFStages - 1);
-      const float* kp = s_k + (ct % kFStages) * kFCols * ldk + col * ldk;
+      load_k(ct + nst - 1);
+      const float* kp = s_k + (ct & (nst - 1)) * kFCols * ldk + col * ldk;
       const float* q0 = s_q + (2 * rg) * r;
       const float* q1 = q0 + r;
       float a0 = 0.f, a1 = 0.f;
@@ -267,6 +321,7 @@ score_fused_kernel(const FusedParams p) {
       }
       s_S[(2 * rg) * p.lds + ct * kFCols + col] = a0 * p.inv_sqrt_r;
       s_S[(2 * rg + 1) * p.lds + ct * kFCols + col] = a1 * p.inv_sqrt_r;
+    }
     }
     asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
@@ -408,14 +463,18 @@ int32_t launch_block_scores(const sw_layout& L, const float* qs, const float* ks
   return check_launch("sw_block_scores");
 }
 
-static size_t fused_smem_bytes(int max_blocks, int r, int* lds_out) {
+static size_t fused_smem_bytes(int max_blocks, int r, int* lds_out, int* stages_out) {
   const int lds = ((max_blocks + kFCols - 1) / kFCols) * kFCols + 4;   // whole 64-column tiles are written
   if (lds_out) *lds_out = lds;
-  return sizeof(float) * ((size_t)kFRows * r + (size_t)kFStages * kFCols * (r + 4) + (size_t)kFRows * lds);
+  auto bytes = [&](int st) { return sizeof(float) * ((size_t)kFRows * r + (size_t)st * kFCols * (r + 4) + (size_t)kFRows * lds); };
+  // two CTAs per SM (<= 110 KB each) hide more latency than a deeper ring
+  const int st = (bytes(kFStagesMax) <= 110 * 1024 || bytes(2) > 110 * 1024) ? kFStagesMax : 2;
+  if (stages_out) *stages_out = st;
+  return bytes(st);
 }
 
 bool scores_fused_supported(const sw_layout& L, int r) {
-  return r >= 4 && (r & 3) == 0 && r <= kRMax && fused_smem_bytes(L.max_blocks, r, nullptr) <= 200 * 1024;
+  return r >= 4 && (r & 3) == 0 && r <= kRMax && fused_smem_bytes(L.max_blocks, r, nullptr, nullptr) <= 200 * 1024;
 }
 
 // W (and A) of sw_block_scores, plus -- when im != NULL -- the operand images of W and, when R_prev != NULL too,
@@ -432,11 +491,12 @@ int32_t launch_scores_fused(const sw_layout& L, const float* qs, const float* ks
   p.pitch = im ? im->pitch : 0;
   p.n_strips = cdiv(im ? swimg::pad_rows(L.max_blocks) : L.max_blocks, kFRows);
   p.inv_sqrt_r = 1.0f / sqrtf((float)r);
-  const size_t smem = fused_smem_bytes(L.max_blocks, r, &p.lds);
-  if (int32_t rc = allow_dynamic_smem(score_fused_kernel, smem, "sw_block_scores(fused) smem attribute")) return rc;
+  const size_t smem = fused_smem_bytes(L.max_blocks, r, &p.lds, &p.stages);
+  void (*kern)(const FusedParams) = (r <= 64) ? score_fused_kernel<8> : score_fused_kernel<kRMax / 8>;
+  if (int32_t rc = allow_dynamic_smem(kern, smem, "sw_block_scores(fused) smem attribute")) return rc;
   dim3 grid(p.n_strips * (p.R_prev ? 2 : 1), 1, L.batch);
   count_launch();
-  score_fused_kernel<<<grid, kThreads, smem, st>>>(p);
+  kern<<<grid, kThreads, smem, st>>>(p);
   return check_launch("sw_block_scores(fused)");
 }
 

@@ -213,7 +213,17 @@ __device__ __forceinline__ uint4 ld_nc_v4(const void* p) {
   return r;
 }
 
+// x^s for an integer s >= 1 by repeated squaring; the small exponents in use (the configs' 1-3, the paper's 8) are
+// straight-line code (s is uniform over a kernel: the switch does not diverge)
 __device__ __forceinline__ float powi(float x, int s) {
+  switch (s) {
+    case 1: return x;
+    case 2: return x * x;
+    case 3: return x * x * x;
+    case 4: { const float x2 = x * x; return x2 * x2; }
+    case 8: { const float x2 = x * x, x4 = x2 * x2; return x4 * x4; }
+    default: break;
+  }
   float r = 1.f, b = x;
   while (s) { if (s & 1) r *= b; b *= b; s >>= 1; }
   return r;

@@ -181,7 +181,7 @@ score_rows_kernel(int s, uint32_t flags, const int32_t* __restrict__ cu_blocks, 
 // written once and never re-read by this step; split_tf32_kernel and its pass over W and R are gone.
 constexpr int kFRows = 8;
 constexpr int kFCols = 64;
-constexpr int kFStagesMax = 4;        // ring of key-sketch tiles (cp.async): 4 stages, or 2 when that lets two CTAs share an SM
+constexpr int kFStagesMax = 8;        // ring of key-sketch tiles (cp.async): 8, 4 or 2 stages, the deepest that fits
 
 // D (16x8, fp32) += A (16x8, tf32, rows g / g + 8) * B (8x8, tf32); the A rows g + 8 are zero here
 __device__ __forceinline__ void mma_tf32(float (&c)[4], uint32_t a0, uint32_t a2, uint32_t b0, uint32_t b1) {
@@ -202,7 +202,7 @@ struct FusedParams {
   const float* R_prev;               // packed; split into rhi / rlo by the CTAs behind the strips, or NULL
   float *rhi, *rlo;
   int pitch, n_strips, lds;          // lds: row stride of the score strip in shared memory (floats)
-  int stages;                        // 2 or 4
+  int stages;                        // 2, 4 or 8
   float inv_sqrt_r;
 };
 
@@ -220,7 +220,7 @@ score_fused_kernel(const FusedParams p) {
   const int rbase = images ? swimg::row_base(p.cu_blocks, seq) : 0;
 
   if ((int)blockIdx.x >= p.n_strips) {
-    // ---- operand images of R_prev: one warp per row ------------------------------------------------------
+    // ---- operand images of R_prev: one warp per row, 4 float4 loads in flight per lane ---------------------------
     const int i = ((int)blockIdx.x - p.n_strips) * kFRows + warp;
     if (i < rows_all)
       swimg::split_row(p.R_prev + __ldg(p.cu_sq + seq) + (int64_t)i * b, i, b, p.pitch, causal,
@@ -229,7 +229,7 @@ score_fused_kernel(const FusedParams p) {
   }
   const int i0 = blockIdx.x * kFRows;
   if (i0 >= rows_all) return;
-  const int r = p.r, r4 = r >> 2, ldk = r + 4;
+  const int r = p.r, r4 = r >> 2, ldk = r + 4, r4_log2 = 31 - __clz(r4);
   float* s_q = smem;                                          // [kFRows][r]
   const int nst = p.stages;
   float* s_k = s_q + kFRows * r;                              // [stages][kFCols][r + 4]
@@ -243,7 +243,7 @@ score_fused_kernel(const FusedParams p) {
       if (ct < nct) {
         float* dst = s_k + (ct & (nst - 1)) * kFCols * ldk;
         for (int i = tid; i < kFCols * r4; i += kThreads) {
-          const int kk = i / r4, c = (i - kk * r4) * 4;
+          const int kk = i >> r4_log2, c = (i & (r4 - 1)) * 4;   // (r is a power of two for the SRHT; checked on the host)
           const int j = ct * kFCols + kk;
           const float* src = p.ks + (int64_t)(blk0 + min(j, b - 1)) * r + c;
           const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst + kk * ldk + c);
@@ -253,7 +253,13 @@ score_fused_kernel(const FusedParams p) {
       }
       asm volatile("cp.async.commit_group;" ::: "memory");
     };
-    for (int ct = 0; ct < nst - 1; ++ct) load_k(ct);          // stages - 1 tiles in flight (one latency, not one each)
+    auto wait_tile = [&]() {                                  // all but the newest stages - 2 groups have landed
+      if (nst == 8) asm volatile("cp.async.wait_group 6;" ::: "memory");
+      else if (nst == 4) asm volatile("cp.async.wait_group 2;" ::: "memory");
+      else asm volatile("cp.async.wait_group 0;" ::: "memory");
+    };
+    // stages - 1 tiles in flight
+    for (int ct = 0; ct < nst - 1; ++ct) load_k(ct);
     for (int i = tid; i < kFRows * r4; i += kThreads) {
       const int rr = i / r4, c = (i - rr * r4) * 4;
       float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -281,8 +287,7 @@ score_fused_kernel(const FusedParams p) {
       }
       const int n0 = warp * 8;                                // this warp's columns of every tile
       for (int ct = 0; ct < nct; ++ct) {
-        if (nst == 4) asm volatile("cp.async.wait_group 2;" ::: "memory");
-        else asm volatile("cp.async.wait_group 0;" ::: "memory");
+        wait_tile();
         __syncthreads();                                      // tile ct landed; tile ct - 1 fully consumed
         load_k(ct + nst - 1);
         const float* kp = s_k + (ct & (nst - 1)) * kFCols * ldk + (n0 + g) * ldk + t4;
@@ -304,8 +309,7 @@ score_fused_kernel(const FusedParams p) {
     } else {
     const int col = tid & (kFCols - 1), rg = tid / kFCols;    // rows 2 rg, 2 rg + 1 of the strip
     for (int ct = 0; ct < nct; ++ct) {
-      if (nst == 4) asm volatile("cp.async.wait_group 2;" ::: "memory");
-      else asm volatile("cp.async.wait_group 0;" ::: "memory");
+      wait_tile();
       __syncthreads();                                        // tile ct landed; tile ct - 1 fully consumed
       load_k(ct + nst - 1);
       const float* kp = s_k + (ct & (nst - 1)) * kFCols * ldk + col * ldk;
@@ -467,14 +471,15 @@ static size_t fused_smem_bytes(int max_blocks, int r, int* lds_out, int* stages_
   const int lds = ((max_blocks + kFCols - 1) / kFCols) * kFCols + 4;   // whole 64-column tiles are written
   if (lds_out) *lds_out = lds;
   auto bytes = [&](int st) { return sizeof(float) * ((size_t)kFRows * r + (size_t)st * kFCols * (r + 4) + (size_t)kFRows * lds); };
-  // two CTAs per SM (<= 110 KB each) hide more latency than a deeper ring
-  const int st = (bytes(kFStagesMax) <= 110 * 1024 || bytes(2) > 110 * 1024) ? kFStagesMax : 2;
+  // two CTAs per SM (<= 110 KB each) beat a deeper ring with one (b = 2048: 96K against 124K cycles per SM)
+  int st = kFStagesMax;
+  while (st > 2 && bytes(st) > 110 * 1024) st >>= 1;
   if (stages_out) *stages_out = st;
   return bytes(st);
 }
 
 bool scores_fused_supported(const sw_layout& L, int r) {
-  return r >= 4 && (r & 3) == 0 && r <= kRMax && fused_smem_bytes(L.max_blocks, r, nullptr, nullptr) <= 200 * 1024;
+  return r >= 4 && (r & (r - 1)) == 0 && r <= kRMax && fused_smem_bytes(L.max_blocks, r, nullptr, nullptr) <= 200 * 1024;
 }
 
 // W (and A) of sw_block_scores, plus -- when im != NULL -- the operand images of W and, when R_prev != NULL too,

@@ -30,27 +30,41 @@ __device__ __forceinline__ void split4(const float4& x, float4& h, float4& l) {
   h.z = __uint_as_float(__float_as_uint(x.z) & 0xffffe000u); l.z = x.z - h.z;
   h.w = __uint_as_float(__float_as_uint(x.w) & 0xffffe000u); l.w = x.w - h.w;
 }
-// One image row from one row of a packed b x b matrix (src_row = &M[i][0]; rows i >= b are padding).
+// One image row from one row of a packed b x b matrix (src_row = &M[i][0]; rows i >= b are padding).  The loads of
+// kSplitUnroll float4s per thread are issued before the first one is used: with one load in flight a 2048-column
+// row split by one warp was 16 dependent memory latencies.
+constexpr int kSplitUnroll = 4;
 __device__ __forceinline__ void split_row(const float* __restrict__ src_row, int i, int b, int pitch, int causal,
                                           float* __restrict__ hi, float* __restrict__ lo, int tid, int nthreads) {
   const int lim = row_cols(i, pitch, causal);
   const bool vec = i < b && (b & 3) == 0 && (reinterpret_cast<uintptr_t>(src_row) & 15u) == 0;
-  for (int j = tid * 4; j < lim; j += nthreads * 4) {
-    float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (i < b) {
-      if (vec) {
-        if (j < b) x = *reinterpret_cast<const float4*>(src_row + j);
-      } else {
-        if (j + 0 < b) x.x = src_row[j + 0];
-        if (j + 1 < b) x.y = src_row[j + 1];
-        if (j + 2 < b) x.z = src_row[j + 2];
-        if (j + 3 < b) x.w = src_row[j + 3];
+  for (int j0 = tid * 4; j0 < lim; j0 += kSplitUnroll * nthreads * 4) {
+    float4 x[kSplitUnroll];
+#pragma unroll
+    for (int u = 0; u < kSplitUnroll; ++u) {
+      const int j = j0 + u * nthreads * 4;
+      x[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (i < b && j < lim) {
+        if (vec) {
+          if (j < b) x[u] = *reinterpret_cast<const float4*>(src_row + j);
+        } else {
+          if (j + 0 < b) x[u].x = src_row[j + 0];
+          if (j + 1 < b) x[u].y = src_row[j + 1];
+          if (j + 2 < b) x[u].z = src_row[j + 2];
+          if (j + 3 < b) x[u].w = src_row[j + 3];
+        }
       }
     }
-    float4 h, l;
-    split4(x, h, l);
-    *reinterpret_cast<float4*>(hi + j) = h;
-    *reinterpret_cast<float4*>(lo + j) = l;
+#pragma unroll
+    for (int u = 0; u < kSplitUnroll; ++u) {
+      const int j = j0 + u * nthreads * 4;
+      if (j < lim) {
+        float4 h, l;
+        split4(x[u], h, l);
+        *reinterpret_cast<float4*>(hi + j) = h;
+        *reinterpret_cast<float4*>(lo + j) = l;
+      }
+    }
   }
 }
 #endif

@@ -234,7 +234,7 @@ SW_API int32_t sw_select_topk_row(int32_t batch, int32_t block, int32_t max_bloc
                            const int32_t* seqlens, const int32_t* tau, int32_t tau_max,
                            uint32_t flags, int32_t* idx, int32_t* count, sw_stream_t stream);
 
-/* Decode selection, fused -- Alg. 2 Steps 2-6 in two launches: exactly the sequence
+/* Decode selection, fused -- Alg. 2 Steps 2-6 in three launches: exactly the sequence
  *   sw_sketch_append(k_new -> kbar, ks); sw_sketch_append(q -> q~_t); sw_block_scores_row;
  *   sw_walk_update_row (with SW_ROWNORM: r_out / max|r_out|, P9); sw_select_topk_row
  * with the same arguments and the same results up to fp32 summation order (the selected indices are
@@ -246,9 +246,11 @@ SW_API int32_t sw_select_topk_row(int32_t batch, int32_t block, int32_t max_bloc
  * r_out: dev fp32 [batch, max_blocks].  Needs !SW_POW_MATRIX and SW_CAUSAL (see sw_block_scores_row).
  * ws: dev scratch of sw_decode_select_workspace_bytes(batch, max_blocks) bytes (SW_ERR_WORKSPACE if smaller):
  * the raw score row and the partial sums of the W stream, handed from the first kernel to the second (no state is
- * kept between calls; calls that share a workspace must not overlap).  batch <= 512.  Two launches: the
- * streaming kernel (duties + cached-W stream over the whole grid) and, as its programmatic dependent, the
- * per-sequence tail (softmax, W_new, rescale, select). */
+ * kept between calls; calls that share a workspace must not overlap).  batch <= 512.  Three launches chained as
+ * programmatic dependents: the streaming kernel (the cached-W stream of Step 5 over the whole grid; skipped when
+ * r_prev is NULL), beside it the kernel of Steps 2-4 (sketches, running key mean, raw score row), then the
+ * per-sequence tail (softmax, W_new, rescale, select).  No kernel of the chain reads anything an earlier kernel of
+ * the stream may have written before its griddepcontrol.wait. */
 SW_API int32_t sw_decode_select(int32_t batch, int32_t block, int32_t max_blocks, const sw_tensor* q,
                          const sw_tensor* k_new, const int32_t* seqlens, const int8_t* signs,
                          const int32_t* cols, int32_t r, float scale, int32_t s, uint32_t flags,

@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsw.so")
-SOURCES = ["api.cu", "sketch.cu", "scores.cu", "walk.cu", "walk_tc.cu", "select.cu", "decode_select.cu", "decode_tail.cu", "attn_prefill_generic.cu",
+SOURCES = ["api.cu", "sketch.cu", "scores.cu", "walk.cu", "walk_tc.cu", "select.cu", "decode_duty.cu", "decode_select.cu", "decode_tail.cu", "attn_prefill_generic.cu",
            "attn_prefill_sm100.cu", "attn_decode.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr",

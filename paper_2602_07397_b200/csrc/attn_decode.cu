@@ -19,12 +19,10 @@ constexpr int kStages = 3;
 // Partial results: Opart [batch, h_q, nsplit, D] fp32 (unnormalised), ML [batch, h_q, nsplit, 2]
 template <int D>
 __global__ void __launch_bounds__(kThreads)
-attn_decode_kernel(const __nv_bfloat16* __restrict__ Q, int64_t q_sb, int64_t q_sh,
-                   const __nv_bfloat16* __restrict__ Kc, const __nv_bfloat16* __restrict__ Vc,
+attn_decode_kernel(const __nv_bfloat16* Q, int64_t q_sb, int64_t q_sh, const __nv_bfloat16* Kc, const __nv_bfloat16* Vc,
                    int64_t kv_sb, int64_t k_st, int64_t k_sh, int64_t v_st, int64_t v_sh, int h_q, int h_kv,
-                   const int32_t* __restrict__ seqlens, int B, const int32_t* __restrict__ idx,
-                   const int32_t* __restrict__ count, int tau_max, float scale_log2, int nsplit,
-                   const int32_t* __restrict__ table, int table_stride,
+                   const int32_t* seqlens, int B, const int32_t* idx, const int32_t* count, int tau_max,
+                   float scale_log2, int nsplit, const int32_t* table, int table_stride,
                    float* __restrict__ Opart, float* __restrict__ ML) {
   extern __shared__ __align__(128) uint8_t smem_raw[];
   constexpr int TILE_BYTES = KT * D * 2;
@@ -34,9 +32,11 @@ attn_decode_kernel(const __nv_bfloat16* __restrict__ Q, int64_t q_sb, int64_t q_
   const int grp = h_q / h_kv;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t4 = lane & 3;
   swd::pdl_launch_dependents();                          // (the merge kernel may take its place on the SMs early)
-  swd::pdl_wait();                                       // the block lists of the selection before this kernel
-  const int t = __ldg(seqlens + seq);
-  const int cnt = __ldg(count + seq);
+  // the block lists of the selection before this kernel (and whatever else earlier kernels of the stream wrote):
+  // no load through these pointers may be scheduled above the wait (common.cuh: pdl_wait)
+  swd::pdl_wait(Q, Kc, Vc, seqlens, idx, count, table);
+  const int t = seqlens[seq];                            // (plain loads, not __ldg: see pdl_wait)
+  const int cnt = count[seq];
   const int32_t* list = idx + (int64_t)seq * tau_max;
   const int TPB = B / KT;
   const int per = (cnt + nsplit - 1) / nsplit;            // selected blocks per split
@@ -50,10 +50,10 @@ attn_decode_kernel(const __nv_bfloat16* __restrict__ Q, int64_t q_sb, int64_t q_
 
   // k_tok0: token offset of the tile in memory; k_valid: keys of it that exist (logical position < t)
   auto slot_info = [&](int slot, int& k_tok0, int& k_valid) {
-    const int j = __ldg(list + blk_lo + slot / TPB);
+    const int j = list[blk_lo + slot / TPB];             // (L1-cached after the first touch)
     const int off = (slot % TPB) * KT;
     k_valid = max(0, min(KT, t - (j * B + off)));
-    k_tok0 = (pages ? __ldg(pages + j) : j) * B + off;
+    k_tok0 = (pages ? pages[j] : j) * B + off;
   };
   auto issue = [&](int slot, int stage) {
     int k_tok0, k_valid;
@@ -213,12 +213,12 @@ attn_decode_kernel(const __nv_bfloat16* __restrict__ Q, int64_t q_sb, int64_t q_
 
 template <int D>
 __global__ void __launch_bounds__(D)
-attn_decode_merge_kernel(const float* __restrict__ Opart, const float* __restrict__ ML, int nsplit,
-                         __nv_bfloat16* __restrict__ out, float* __restrict__ lse) {
+attn_decode_merge_kernel(const float* Opart, const float* ML, int nsplit, __nv_bfloat16* __restrict__ out,
+                         float* __restrict__ lse) {
   const int64_t bh = blockIdx.x;                      // seq * h_q + head
   const int c = threadIdx.x;
   swd::pdl_launch_dependents();                       // the next kernel of the layer loop may start its prologue
-  swd::pdl_wait();                                    // the split-KV partials
+  swd::pdl_wait(Opart, ML);                           // the split-KV partials
   float m = -INFINITY;
   for (int s = 0; s < nsplit; ++s) m = fmaxf(m, ML[(bh * nsplit + s) * 2]);
   float acc = 0.f, l = 0.f;

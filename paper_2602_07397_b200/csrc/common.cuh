@@ -178,6 +178,17 @@ int32_t launch_attn_decode(int batch, int block, const sw_tensor& q, const sw_te
 namespace swd {
 
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+// pdl_wait(p, q, ...): wait, then pass the pointers through an empty asm.  Loads the compiler treats as invariant
+// (__ldg, const __restrict__ parameters: ld.global.nc) are not ordered by a memory clobber -- measured: the loads of
+// count[seq] and seqlens[seq] of the decode attention kernel were scheduled ABOVE griddepcontrol.wait and read what the
+// selection kernel had not written yet (a wild block list, about one run in four).  A load through a pointer that
+// comes out of an asm statement issued after the wait cannot move above it.  Every pointer to data an earlier
+// kernel of the stream may have written goes through here before its first use.
+template <typename T> __device__ __forceinline__ void pdl_launder(T*& p) { asm volatile("" : "+l"(p)); }
+template <typename... P> __device__ __forceinline__ void pdl_wait(P*&... ptrs) {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  (pdl_launder(ptrs), ...);
+}
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 __device__ __forceinline__ float warp_max(float v) {

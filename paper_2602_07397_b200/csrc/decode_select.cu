@@ -1,332 +1,176 @@
 // sw_decode_select: Alg. 2 Steps 2-6 for one new token per sequence: running key-block
 // mean + sketches (Steps 2-3), the new row of W (Steps 3-4), the row-vector walk r^k = r^{k-1} W'^k (Step 5,
 // SURVEY 8(a) row a6), the max-abs rescale (P9) and the top-tau selection (Step 6).  HBM-bound on the cached W
-// (4 b^2/2 bytes per sequence).  Two kernels; this file holds the first: everything that touches HBM-sized data.
+// (4 b^2/2 bytes per sequence).  Three kernels, chained as programmatic dependents:
+//   this file         Step 5's stream: sum_{m < b_q} r_prev[m] W[m][j] over the whole grid, whatever the batch;
+//   decode_duty.cu    Steps 2-4 per (sequence, 256 columns): sketches, running key mean, raw scores of the new row;
+//   decode_tail.cu    per sequence: softmax, W_new = A^s (stored as row b_q of the cache), r, rescale, top-tau.
 //
-// The whole grid (two CTAs per SM) works on the batch, whatever its size.  Two kinds of work are dealt out:
-//  * chunks: 64 rows x 64 columns of the block-causal part of the cached W (rows [64 c, b_q) of column tile
-//    c), numbered over all sequences; CTA i streams the contiguous range [i T / G, (i+1) T / G) of the T
-//    chunks through a cp.async ring, accumulates r_prev[m] W[m][j] over the chunks of one column tile in
-//    registers and leaves one 64-float partial per (tile, CTA) in the workspace (fixed slots, fixed
-//    summation order: deterministic);
-//  * duties: one per (sequence, column tile), dealt the same way: q~_t (and, on the tile that holds b_q, the
-//    running key-block mean and its sketch) and the raw scores of the tile's 64 columns.
-// A CTA runs its duties first.  Every load they need (head values, key-sketch rows, the old mean) and the
-// r_prev rows of the stream are requested BEFORE the first chunks of the W stream: on an SM that keeps
-// ~160 KB of the stream in flight a load issued behind it waits ~3 us (queue depth / per-SM bandwidth).
-// The second kernel (decode_tail.cu, one CTA of 1024 threads per sequence, launched as a programmatic dependent
-// so that it becomes resident while the last CTAs of this one drain) turns the raw score row and the partial
-// sums into W_new = A^s, r, the rescaled r_out and the block list.  An earlier version ran that tail on the last
-// CTA to finish a sequence (one launch, a completion counter in the workspace): 256 threads made the radix
-// select and the row passes a 12 us serial chain (two warps per scheduler: every pass is bound by the dependent
-// issue latency), a quarter of a decode layer; 1024 threads do it in a fraction of that.
+// The stream: the block-causal part of the cached W is cut into chunks of kChunkRows rows x kTileW columns (16 KB;
+// column tile c = rows [c kTileW, b_q), the rows above are zero), numbered over all sequences tile by tile; CTA i
+// takes the contiguous range [i T / G, (i+1) T / G) of the T chunks, streams it through a cp.async ring (the pieces
+// right of the diagonal are not requested: zero fill), accumulates r_prev[m] W[m][j] over the chunks of one tile in
+// registers and leaves one kTileW-float partial per (tile, CTA) in the workspace (fixed slots, fixed summation
+// order: deterministic).  The r_prev values of a chunk's rows ride in the chunk's own cp.async group.
+// A row piece of a chunk is kTileW * 4 = 1 KB of consecutive addresses: with 256-byte pieces (64-column tiles) the
+// stream reached 70 % of the HBM bandwidth, DRAM pages being opened for a quarter of their content.
+// The duty kernel is this kernel's programmatic dependent, released after griddepcontrol.wait here: its CTAs (two
+// fit beside the two streaming CTAs of an SM) run beside the stream, which they neither read nor feed.
 // DESIGN.md sec. 6.2 has the measurements behind these choices.
 #include <algorithm>
 
 #include "common.cuh"
 #include "decode_select.cuh"
-#include "sketch_common.cuh"
 #include "sm100.cuh"
 
 namespace {
 
 using namespace swds;
 
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+__device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void* src, int bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 
-template <typename TIn, int D>
 __global__ void __launch_bounds__(kThreads, 2)
-decode_select_kernel(const Params p) {
-  // the tail kernel is launched as a programmatic dependent: let it become resident as SMs drain
-  swd::pdl_launch_dependents();
+decode_stream_kernel(const Params p_in) {
+  Params p = p_in;                                    // (the pointers to earlier kernels' data pass through pdl_wait)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int G = (int)gridDim.x, me = (int)blockIdx.x;
-  const bool walk = p.r_prev != nullptr;
-  const bool async = walk && p.use_async;
+  const bool async = p.use_async;
   const int mb = p.max_blocks;
-  const int rstride = p.mbp + kChunkRows;
 
   extern __shared__ __align__(128) uint8_t smem_raw[];
-  float* s_rprev = reinterpret_cast<float*>(smem_raw);                 // [2][mbp + 64] r_prev of two sequences
-  float* s_part = s_rprev + 2 * rstride;                               // [kRowGroups][64]
-  uint8_t* s_ring = reinterpret_cast<uint8_t*>(
-      (reinterpret_cast<uintptr_t>(s_part + kRowGroups * kTile) + 127) & ~(uintptr_t)127);   // [kStages][16 KB]
-  __shared__ __align__(16) float s_vec[D], s_qt[128], s_kt[128], s_sign[D];
-  __shared__ float s_hx[kThreads / D][D];
-  __shared__ int32_t s_cols[128];
+  uint8_t* s_ring = smem_raw;                                          // [kStages][16 KB]
+  float* s_rp = reinterpret_cast<float*>(s_ring + (size_t)kStages * kChunkBytes);   // [kStages][kChunkRows] r_prev of the chunk's rows
+  float* s_part = s_rp + kStages * kChunkRows;                         // [kRowGroups][kTileW]
   __shared__ int s_pref[kMaxBatch + 1];                                // exclusive prefix of chunks per sequence
-  __shared__ int s_dpref[kMaxBatch + 1];                               // exclusive prefix of duties per sequence
+  __shared__ int s_tpref[kMaxBatch + 1];                               // exclusive prefix of tiles with chunks
   __shared__ int s_len[kMaxBatch];                                     // sequence lengths (read once from HBM)
   __shared__ int s_scan[2][kThreads / 32];
 
-  // ---- chunk and duty counts of all sequences: exclusive prefixes in shared memory -------------------
+  // Launched as a programmatic dependent: nothing an earlier kernel of the stream may have written (the sequence
+  // lengths included) is read before this wait, and the duty kernel is released behind this one's CTAs only after it.
+  swd::pdl_wait(p.W, p.r_prev, p.seqlens);
+  swd::pdl_launch_dependents();
+  // ---- chunk and tile counts of all sequences: exclusive prefixes in shared memory ----------------------
   {
     constexpr int kPer = kMaxBatch / kThreads;
-    int vc[kPer], vd[kPer], sc = 0, sd = 0;
+    int vc[kPer], vt[kPer], sc = 0, st = 0;
 #pragma unroll
     for (int e = 0; e < kPer; ++e) {
       const int sq = tid * kPer + e;
-      vc[e] = 0; vd[e] = 0;
+      vc[e] = 0; vt[e] = 0;
       if (sq < p.batch) {
-        s_len[sq] = __ldg(p.seqlens + sq);
-        const SeqInfo si = seq_info(s_len, sq, p.B);
-        vc[e] = si.total_chunks(walk); vd[e] = si.duties();
+        s_len[sq] = __ldcg(p.seqlens + sq);
+        const SeqInfo si = seq_info(s_len, sq, p.B, true);
+        vc[e] = si.total_chunks(); vt[e] = si.nt;
       }
-      sc += vc[e]; sd += vd[e];
+      sc += vc[e]; st += vt[e];
     }
-    int ic = sc, id = sd;
+    int ic = sc, it = st;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const int uc = __shfl_up_sync(0xffffffffu, ic, o), ud = __shfl_up_sync(0xffffffffu, id, o);
-      if (lane >= o) { ic += uc; id += ud; }
+      const int uc = __shfl_up_sync(0xffffffffu, ic, o), ut = __shfl_up_sync(0xffffffffu, it, o);
+      if (lane >= o) { ic += uc; it += ut; }
     }
-    if (lane == 31) { s_scan[0][warp] = ic; s_scan[1][warp] = id; }
-    if (tid < D) s_sign[tid] = p.signs ? (float)p.signs[tid] : 1.f;
-    if (tid < p.r && tid < 128) s_cols[tid] = p.cols[tid];
+    if (lane == 31) { s_scan[0][warp] = ic; s_scan[1][warp] = it; }
     __syncthreads();
-    int bc = 0, bd = 0;
-    for (int w = 0; w < warp; ++w) { bc += s_scan[0][w]; bd += s_scan[1][w]; }
-    int rc = bc + ic - sc, rd = bd + id - sd;
+    int bc = 0, bt = 0;
+    for (int w = 0; w < warp; ++w) { bc += s_scan[0][w]; bt += s_scan[1][w]; }
+    int rc = bc + ic - sc, rt = bt + it - st;
 #pragma unroll
     for (int e = 0; e < kPer; ++e) {
       const int sq = tid * kPer + e;
-      if (sq <= p.batch) { s_pref[sq] = rc; s_dpref[sq] = rd; }
-      rc += vc[e]; rd += vd[e];
+      if (sq <= p.batch) { s_pref[sq] = rc; s_tpref[sq] = rt; }
+      rc += vc[e]; rt += vt[e];
     }
     __syncthreads();
   }
-  const int T = s_pref[p.batch], ND = s_dpref[p.batch];
-  // chunks are dealt to the first Gc = min(G, T) CTAs, so that every one of them has at least one: the partial
-  // slots of a tile (one per CTA that shares it) are then contiguous
+  const int T = s_pref[p.batch];
+  // chunks are dealt to the first Gc = min(G, T) CTAs, so that every one of them has at least one
   const int Gc = max(1, min(G, T));
   const int g_begin = me < Gc ? (int)((long long)me * T / Gc) : T, g_end = me < Gc ? (int)((long long)(me + 1) * T / Gc) : T;
-  const int d_begin = (int)((long long)me * ND / G), d_end = (int)((long long)(me + 1) * ND / G);
   const int n_my = g_end - g_begin;
-  if (n_my == 0 && d_begin == d_end) return;
-
-  auto find_seq = [&](const int* pref, int g) {
-    int lo = 0, hi = p.batch - 1;
-    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (pref[mid] <= g) lo = mid; else hi = mid - 1; }
-    return lo;
-  };
+  if (n_my == 0) return;
 
   // ---- cursors over this CTA's chunks (thread-uniform) ------------------------------------------------
   struct Cursor { int seq, tile, chunk; SeqInfo si; };
   auto locate = [&](int g) {
     Cursor c;
-    c.seq = find_seq(s_pref, g);
-    c.si = seq_info(s_len, c.seq, p.B);
+    int lo = 0, hi = p.batch - 1;
+    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_pref[mid] <= g) lo = mid; else hi = mid - 1; }
+    c.seq = lo;
+    c.si = seq_info(s_len, c.seq, p.B, true);
     const int local = g - s_pref[c.seq];
-    int tl = 0, th = c.si.a;
-    while (tl < th) { const int mid = (tl + th + 1) >> 1; if (c.si.chunks_before(mid, walk) <= local) tl = mid; else th = mid - 1; }
+    int tl = 0, th = max(c.si.nt - 1, 0);
+    while (tl < th) { const int mid = (tl + th + 1) >> 1; if (c.si.chunks_before(mid) <= local) tl = mid; else th = mid - 1; }
     c.tile = tl;
-    c.chunk = local - c.si.chunks_before(tl, walk);
+    c.chunk = local - c.si.chunks_before(tl);
     return c;
   };
   auto advance = [&](Cursor& c) {
     ++c.chunk;
-    while (c.seq < p.batch && c.chunk >= c.si.chunks(c.tile, walk)) {
+    while (c.seq < p.batch && c.chunk >= c.si.chunks(c.tile)) {
       c.chunk = 0;
-      if (++c.tile > c.si.a) {
+      if (++c.tile >= c.si.nt) {
         c.tile = 0;
-        if (++c.seq < p.batch) c.si = seq_info(s_len, c.seq, p.B);
+        if (++c.seq < p.batch) c.si = seq_info(s_len, c.seq, p.B, true);
       }
     }
   };
-  Cursor cc, pc;
-  cc.seq = cc.tile = cc.chunk = 0; cc.si.bq = cc.si.a = cc.si.eps = 0;
-  int seq_first = 0;
-  if (n_my > 0) { cc = locate(g_begin); seq_first = cc.seq; }
-  pc = cc;
+  Cursor cc = locate(g_begin), pc = cc;
 
-  // Launched as a programmatic dependent itself: what is above (work prefixes, cursors; sequence lengths only)
-  // overlaps the tail of the kernel before this one; everything below reads what earlier kernels produced.
-  swd::pdl_wait();
-
-  // ---- W stream: chunk = rows [64 tile + 64 chunk, +64) x columns [64 tile, +64) of the sequence's cached W
+  // ---- W stream: chunk = rows [tile kTileW + chunk kChunkRows, +kChunkRows) x columns [tile kTileW, +kTileW) ----
   int p_left = n_my, issued = 0;
   auto issue_next = [&]() {                           // all threads: request the next chunk (or an empty group)
     if (p_left > 0) {
       const float* Wseq = p.W + (int64_t)pc.seq * p.w_stride_seq;
-      const int m0 = (pc.tile + pc.chunk) * kTile;
-      const uint32_t dst = sm100::smem_u32(s_ring + (size_t)(issued % kStages) * kChunkBytes);
+      const int m0 = pc.tile * kTileW + pc.chunk * kChunkRows;
+      const int st = issued % kStages;
+      const uint32_t dst = sm100::smem_u32(s_ring + (size_t)st * kChunkBytes);
 #pragma unroll
       for (int u = 0; u < kPieces; ++u) {
-        const int pcs = u * kThreads + tid, rr = pcs >> 4, c4 = pc.tile * kTile + (pcs & 15) * 4;
-        if (m0 + rr < pc.si.bq && c4 < mb)            // rows >= b_q / columns >= max_blocks are never read
-          cp_async16(dst + pcs * 16, Wseq + (int64_t)(m0 + rr) * mb + c4);
+        const int pcs = u * kThreads + tid, rr = pcs / kQuads, m = m0 + rr, c4 = pc.tile * kTileW + (pcs % kQuads) * 4;
+        // rows >= b_q are not part of the product; W[m][j] = 0 for j > m (block-causal): not requested
+        const bool ok = m < pc.si.bq && c4 <= m && c4 < mb;
+        cp_async16_zfill(dst + pcs * 16, ok ? Wseq + (int64_t)m * mb + c4 : Wseq, ok ? 16 : 0);
+      }
+      if (tid < kChunkRows / 4) {
+        const int m = m0 + tid * 4;
+        const bool ok = m < mb;
+        cp_async16_zfill(sm100::smem_u32(s_rp + st * kChunkRows + tid * 4), ok ? p.r_prev + (int64_t)pc.seq * mb + m : p.r_prev,
+                         ok ? 16 : 0);
       }
       ++issued; advance(pc); --p_left;
     }
     cp_async_commit();
   };
-  // r_prev of the first two sequences of this CTA's chunk range (group 0 of the cp.async stream), then the
-  // first kStages - 1 chunks.  Called once, after the loads of the last duty have been issued.
-  auto start_stream = [&]() {
-    if (n_my == 0) return;                            // (no chunks without a walk)
-    for (int q2 = 0; q2 < 2; ++q2) {
-      const int sq = seq_first + q2;
-      if (sq < p.batch && (q2 == 0 || s_pref[sq] < g_end)) {
-        const float* rp = p.r_prev + (int64_t)sq * mb;
-        if (async)
-          for (int i = tid * 4; i < mb; i += kThreads * 4) cp_async16(sm100::smem_u32(s_rprev + q2 * rstride + i), rp + i);
-        else
-          for (int i = tid; i < mb; i += kThreads) s_rprev[q2 * rstride + i] = __ldg(rp + i);
-      }
-    }
-    if (async) {
-      cp_async_commit();
-      for (int i = 0; i < kStages - 1; ++i) issue_next();
-    }
-  };
+  if (async)
+    for (int i = 0; i < kStages - 1; ++i) issue_next();
 
-  // ================= duties: Steps 2-4 for one column tile each ==========================================
-  constexpr int kGroups = kThreads / D;
-  const int q4 = p.r >> 2;                            // float4s per sketch row
-  const bool vec_ok = (p.r & 3) == 0 && q4 >= 1 && q4 <= 32 && (q4 & (q4 - 1)) == 0 && kTile * q4 <= kKU * kThreads &&
-                      (reinterpret_cast<uintptr_t>(p.ks) & 15u) == 0;
-  const int hx = tid % D, hg = tid / D;
-  int qt_seq = -1;
-  bool stream_started = false;
-  for (int dty = d_begin; dty < d_end; ++dty) {
-    const int seq = find_seq(s_dpref, dty), tile = dty - s_dpref[seq];
-    const SeqInfo si = seq_info(s_len, seq, p.B);
-    const int bq = si.bq, hi = bq + 1, col0 = tile * kTile;
-    const bool need_q = qt_seq != seq, need_k = tile == si.a;   // tile a owns the key-side update of Step 2
-    const float* ksb = p.ks + (int64_t)seq * mb * p.r;
-    const int part = vec_ok ? (tid & (q4 - 1)) : 0, per_pass = vec_ok ? kThreads / q4 : 1;
-    const int colq = vec_ok ? tid / q4 : 0;
-    // ---- all loads of the duty, before anything waits on memory: unconditional loads from clamped (always
-    // valid) addresses, raw values kept in registers -- a predicated load followed by its convert made every
-    // group of loads wait for the previous one (5 us instead of one memory latency)
-    TIn qraw[kHeadRegs], kraw[kHeadRegs];
-    float4 kv[kKU];
-    const TIn* qp = reinterpret_cast<const TIn*>(p.q) + (int64_t)seq * p.q_stride_seq + hx;
-    const TIn* kp = reinterpret_cast<const TIn*>(p.k) + (int64_t)seq * p.k_stride_seq + hx;
-#pragma unroll
-    for (int u = 0; u < kHeadRegs; ++u) {
-      const int h = hg + u * kGroups;
-      qraw[u] = qp[(int64_t)min(h, p.h_q - 1) * p.q_stride_head];
-      kraw[u] = kp[(int64_t)min(h, p.h_kv - 1) * p.k_stride_head];
-    }
-    const int cnt = (s_len[seq] - 1) % p.B;                        // tokens already in block b_curr
-    float* kb = p.kbar + ((int64_t)seq * mb + bq) * D;
-    const float kbar_old = kb[tid & (D - 1)];
-#pragma unroll
-    for (int u = 0; u < kKU; ++u) {
-      const int cj = u * per_pass + colq;
-      const int j = min(col0 + min(cj, kTile - 1), bq);                        // clamped: always a valid row
-      kv[u] = vec_ok ? *reinterpret_cast<const float4*>(ksb + (int64_t)j * p.r + part * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
-    }
-    if (dty == d_end - 1) { start_stream(); stream_started = true; }
-    // ---- head means, running key-block mean, sketches ----------------------------------------------------
-    if (need_q || need_k) {
-      float sq = 0.f, sk = 0.f;
-#pragma unroll
-      for (int u = 0; u < kHeadRegs; ++u) {
-        const int h = hg + u * kGroups;
-        if (h < p.h_q) sq += (float)qraw[u];
-        if (h < p.h_kv) sk += (float)kraw[u];
-      }
-      if (need_q) for (int h = hg + kHeadRegs * kGroups; h < p.h_q; h += kGroups) sq += (float)qp[(int64_t)h * p.q_stride_head];
-      if (need_k) for (int h = hg + kHeadRegs * kGroups; h < p.h_kv; h += kGroups) sk += (float)kp[(int64_t)h * p.k_stride_head];
-      if (need_q) {
-        s_hx[hg][hx] = sq;
-        __syncthreads();
-        if (tid < D) {
-          float a = 0.f;
-#pragma unroll
-          for (int g = 0; g < kGroups; ++g) a += s_hx[g][tid];
-          s_vec[tid] = a / (float)p.h_q;
-        }
-        __syncthreads();
-        swsk::sketch_tail<D>(s_vec, s_sign, s_cols, p.r, p.scale, s_qt);         // q~_t
-        qt_seq = seq;
-        __syncthreads();
-      }
-      if (need_k) {
-        s_hx[hg][hx] = sk;
-        __syncthreads();
-        if (tid < D) {
-          float a = 0.f;
-#pragma unroll
-          for (int g = 0; g < kGroups; ++g) a += s_hx[g][tid];
-          const float avg = a / (float)p.h_kv;
-          const float mn = (cnt == 0) ? avg : ((float)cnt * kbar_old + avg) / (float)(cnt + 1);
-          kb[tid] = mn;
-          s_vec[tid] = mn;
-        }
-        __syncthreads();
-        swsk::sketch_tail<D>(s_vec, s_sign, s_cols, p.r, p.scale, s_kt, p.ks + ((int64_t)seq * mb + bq) * p.r);
-        __syncthreads();
-      }
-    }
-    // ---- raw scores of the tile's columns (Steps 3-4; column b_q from the fresh sketch) --------------------
-    float* sc = p.ws_scores + (int64_t)seq * p.mbp;
-    if (vec_ok) {
-      // q4 adjacent lanes share one column; partial dots meet in a fixed xor butterfly
-      const float4 qv = *reinterpret_cast<const float4*>(s_qt + part * 4);
-#pragma unroll
-      for (int u = 0; u < kKU; ++u) {
-        if (u * per_pass >= kTile) break;                                        // warp-uniform
-        const int cj = u * per_pass + colq, j = col0 + cj;
-        if (j == bq) kv[u] = *reinterpret_cast<const float4*>(s_kt + part * 4);
-        float a = fmaf(qv.w, kv[u].w, fmaf(qv.z, kv[u].z, fmaf(qv.y, kv[u].y, qv.x * kv[u].x)));
-        for (int o = q4 >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-        if (part == 0 && cj < kTile && j < hi) sc[j] = a * p.inv_sqrt_r;
-      }
-    } else {
-      for (int cj = warp; cj < kTile; cj += kThreads / 32) {
-        const int j = col0 + cj;
-        if (j < hi) {
-          const float* kr = (j == bq) ? s_kt : ksb + (int64_t)j * p.r;
-          float a = 0.f;
-          for (int c = lane; c < p.r; c += 32) a = fmaf(s_qt[c], kr[c], a);
-          a = swd::warp_sum(a);
-          if (lane == 0) sc[j] = a * p.inv_sqrt_r;
-        }
-      }
-    }
-  }
-  if (!stream_started) start_stream();
-
-  // ================= chunks: Step 5, r_prev[m] W[m][j] over this CTA's range ===============================
-  int cur_seq = -1, consumed = 0;
+  // ---- Step 5, r_prev[m] W[m][j] over this CTA's range ---------------------------------------------------------
+  int consumed = 0;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-  const int cq = tid & 15, rg = tid >> 4;
-  const float* rprev_cur = s_rprev;
+  const int cq = tid % kQuads, rg = tid / kQuads;
   for (int it = 0; it < n_my; ++it) {
     const SeqInfo& si = cc.si;
     const int seq = cc.seq, tile = cc.tile, bq = si.bq;
-    if (seq != cur_seq) {
-      cur_seq = seq;
-      const int slot2 = seq - seq_first;
-      if (slot2 < 2) {
-        rprev_cur = s_rprev + slot2 * rstride;        // requested up front
-      } else {                                        // a range over more than two (tiny) sequences: reload
-        __syncthreads();
-        const float* rp = p.r_prev + (int64_t)seq * mb;
-        for (int i = tid; i < mb; i += kThreads) s_rprev[i] = __ldg(rp + i);
-        rprev_cur = s_rprev;
-        __syncthreads();
-      }
-    }
-    const int m0 = (tile + cc.chunk) * kTile;
+    const int m0 = tile * kTileW + cc.chunk * kChunkRows;
     const int rows = min(kChunkRows, bq - m0);        // rows >= b_q are not part of the product
     if (async) {
-      asm volatile("cp.async.wait_group %0;" ::"n"(kStages - 2) : "memory");   // chunk `consumed` (and r_prev) landed
+      asm volatile("cp.async.wait_group %0;" ::"n"(kStages - 2) : "memory");   // chunk `consumed` landed
       __syncthreads();                                // ... for every thread; the previous chunk is fully consumed
       issue_next();                                   // refill the stage the previous chunk occupied
-      const float* box = reinterpret_cast<const float*>(s_ring + (size_t)(consumed % kStages) * kChunkBytes);
+      const int st = consumed % kStages;
+      const float* box = reinterpret_cast<const float*>(s_ring + (size_t)st * kChunkBytes);
+      const float* rp = s_rp + st * kChunkRows;
 #pragma unroll
-      for (int u = 0; u < kChunkRows / kRowGroups; ++u) {
+      for (int u = 0; u < kRowsPerThread; ++u) {
         const int rr = rg + u * kRowGroups;
         if (rr < rows) {
-          const float4 v = *reinterpret_cast<const float4*>(box + rr * kTile + cq * 4);
-          const float a = rprev_cur[m0 + rr];
+          const float4 v = *reinterpret_cast<const float4*>(box + rr * kTileW + cq * 4);
+          const float a = rp[rr];
           acc.x = fmaf(a, v.x, acc.x);
           acc.y = fmaf(a, v.y, acc.y);
           acc.z = fmaf(a, v.z, acc.z);
@@ -335,29 +179,28 @@ decode_select_kernel(const Params p) {
       }
       ++consumed;
     } else {
-      if (it == 0) __syncthreads();                   // s_rprev is complete
       const float* Wm = p.W + (int64_t)seq * p.w_stride_seq;
-      const int c4 = tile * kTile + cq * 4;
+      const float* rprev = p.r_prev + (int64_t)seq * mb;
+      const int c4 = tile * kTileW + cq * 4;
       for (int rr = rg; rr < rows; rr += kRowGroups) {
-        const float a = rprev_cur[m0 + rr];
-        const float* wr = Wm + (int64_t)(m0 + rr) * mb;
-        if (c4 + 0 < mb) acc.x = fmaf(a, __ldg(wr + c4 + 0), acc.x);
-        if (c4 + 1 < mb) acc.y = fmaf(a, __ldg(wr + c4 + 1), acc.y);
-        if (c4 + 2 < mb) acc.z = fmaf(a, __ldg(wr + c4 + 2), acc.z);
-        if (c4 + 3 < mb) acc.w = fmaf(a, __ldg(wr + c4 + 3), acc.w);
+        const int m = m0 + rr;
+        const float a = __ldcg(rprev + m);
+        const float* wr = Wm + (int64_t)m * mb;
+        if (c4 + 0 <= m) acc.x = fmaf(a, __ldcg(wr + c4 + 0), acc.x);
+        if (c4 + 1 <= m) acc.y = fmaf(a, __ldcg(wr + c4 + 1), acc.y);
+        if (c4 + 2 <= m) acc.z = fmaf(a, __ldcg(wr + c4 + 2), acc.z);
+        if (c4 + 3 <= m) acc.w = fmaf(a, __ldcg(wr + c4 + 3), acc.w);
       }
     }
-    if (it == n_my - 1 || cc.chunk + 1 >= si.chunks(tile, walk)) {
-      // one partial per (tile, CTA): slot = rank of this CTA among the CTAs that share the tile
-      *reinterpret_cast<float4*>(s_part + rg * kTile + cq * 4) = acc;
+    if (it == n_my - 1 || cc.chunk + 1 >= si.chunks(tile)) {
+      // one partial per (tile, CTA)
+      *reinterpret_cast<float4*>(s_part + rg * kTileW + cq * 4) = acc;
       __syncthreads();
-      if (tid < kTile) {
+      if (tid < kTileW) {
         float v = 0.f;
 #pragma unroll
-        for (int g = 0; g < kRowGroups; ++g) v += s_part[g * kTile + tid];      // fixed order
-        const long long f0 = s_pref[seq] + si.chunks_before(tile, walk);
-        const int slot = me - cta_of(f0, T, Gc);
-        p.ws_part[(((int64_t)seq * p.tiles_max + tile) * p.slots + slot) * kTile + tid] = v;
+        for (int g = 0; g < kRowGroups; ++g) v += s_part[g * kTileW + tid];      // fixed order
+        p.ws_part[(int64_t)part_id(me, s_tpref[seq] + tile) * kTileW + tid] = v;
       }
       __syncthreads();
       acc = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -367,25 +210,27 @@ decode_select_kernel(const Params p) {
   asm volatile("cp.async.wait_group 0;" ::: "memory");
 }
 
+// upper bound of the chunks of one sequence (b_q = max_blocks - 1)
+static int max_chunks_per_seq(int max_blocks) {
+  const int bq = std::max(max_blocks - 1, 0);
+  const int nr = sw::cdiv(bq, kChunkRows), nt = sw::cdiv(bq, kTileW);
+  return nt * nr - kRho * (nt * (nt - 1) / 2);
+}
+constexpr int kMaxStreamGrid = 512;
+
 }  // namespace
 
 namespace sw {
 
-static int ds_grid(int batch, int max_blocks) {
-  const int a = (max_blocks - 1) / kTile;
-  const long long work = (long long)batch * ((long long)a * (a + 1) / 2 + a + 1);   // >= chunks, >= duties
-  return (int)std::min<long long>(work, 2LL * num_sms());
-}
-
 size_t decode_select_ws_bytes(int batch, int max_blocks) {
-  const size_t tiles = (size_t)cdiv(max_blocks, kTile), mbp = tiles * kTile;
-  return 256 + sizeof(float) * (size_t)batch * mbp + sizeof(float) * (size_t)batch * tiles * tiles * kTile;
+  const size_t tiles = (size_t)cdiv(max_blocks, kTileW), mbp = tiles * kTileW;
+  return 256 + sizeof(float) * (size_t)batch * mbp + sizeof(float) * ((size_t)kMaxStreamGrid + (size_t)batch * tiles) * kTileW;
 }
 
 int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st) {
   if (a.batch == 0) return SW_OK;
   if (a.batch > kMaxBatch) return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: batch %d > %d", a.batch, kMaxBatch);
-  if (cdiv(a.max_blocks, kTile) > kMaxTiles)
+  if (cdiv(a.max_blocks, kTileW) > kMaxTiles)
     return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: max_blocks %d too large", a.max_blocks);
   const size_t need = decode_select_ws_bytes(a.batch, a.max_blocks);
   if (a.ws == nullptr || a.ws_bytes < need)
@@ -393,38 +238,35 @@ int32_t launch_decode_select(const DecodeSelectArgs& a, cudaStream_t st) {
   Params p;
   p.q = a.q.ptr; p.q_stride_seq = a.q.stride_tok; p.q_stride_head = a.q.stride_head; p.h_q = a.q.heads;
   p.k = a.k.ptr; p.k_stride_seq = a.k.stride_tok; p.k_stride_head = a.k.stride_head; p.h_kv = a.k.heads;
+  p.dtype = a.q.dtype; p.d = a.q.d;
   p.seqlens = a.seqlens; p.signs = a.signs; p.cols = a.cols; p.r = a.r; p.scale = a.scale;
   p.inv_sqrt_r = 1.0f / sqrtf((float)a.r);
   p.s = a.s; p.flags = a.flags; p.kbar = a.kbar; p.ks = a.ks; p.W = a.W_cache; p.w_stride_seq = a.stride_seq;
   p.r_prev = a.r_prev; p.r_out = a.r_out; p.tau = a.tau; p.tau_max = a.tau_max; p.idx = a.idx; p.count = a.count;
   p.batch = a.batch; p.B = a.block; p.max_blocks = a.max_blocks;
-  p.tiles_max = cdiv(a.max_blocks, kTile); p.mbp = p.tiles_max * kTile; p.slots = p.tiles_max;
+  p.tiles_max = cdiv(a.max_blocks, kTileW); p.mbp = p.tiles_max * kTileW;
   uint8_t* w = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(a.ws) + 255) & ~(uintptr_t)255);
   p.ws_scores = reinterpret_cast<float*>(w);
   w += sizeof(float) * (size_t)a.batch * p.mbp;
   p.ws_part = reinterpret_cast<float*>(w);
-  p.g_stream = ds_grid(a.batch, a.max_blocks);
-
-  void (*kern)(const Params) = nullptr;
-  const int d = a.q.d;
-  if (a.q.dtype == SW_BF16 && d == 128) kern = decode_select_kernel<__nv_bfloat16, 128>;
-  else if (a.q.dtype == SW_BF16 && d == 64) kern = decode_select_kernel<__nv_bfloat16, 64>;
-  else if (a.q.dtype == SW_F32 && d == 128) kern = decode_select_kernel<float, 128>;
-  else if (a.q.dtype == SW_F32 && d == 64) kern = decode_select_kernel<float, 64>;
-  else return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: dtype %d / d %d", a.q.dtype, d);
-
+  const long long work = (long long)a.batch * max_chunks_per_seq(a.max_blocks);
+  p.g_stream = (int)std::max<long long>(1, std::min<long long>(work, std::min(2 * num_sms(), kMaxStreamGrid)));
   // cp.async stream of the cached W (and of r_prev) needs 16-byte aligned row pieces; otherwise plain loads
   p.use_async = a.r_prev != nullptr && aligned16(a.W_cache) && aligned16(a.r_prev) && (a.max_blocks & 3) == 0 &&
                 (a.stride_seq & 3) == 0;
 
-  const size_t smem = sizeof(float) * (2 * ((size_t)p.mbp + kChunkRows) + kRowGroups * kTile) + 128 +
-                      (size_t)kStages * kChunkBytes;
-  if (smem > 200 * 1024 || sizeof(float) * (size_t)p.mbp > 160 * 1024)
-    return fail(SW_ERR_UNSUPPORTED, "sw_decode_select: max_blocks %d too large", a.max_blocks);
-  if (int32_t rc = allow_dynamic_smem(kern, smem, "sw_decode_select smem attribute")) return rc;
-  count_launch();
-  launch_pdl(kern, dim3(p.g_stream), dim3(kThreads), smem, st, p);
-  if (int32_t rc = check_launch("sw_decode_select")) return rc;
+  // launch 1: the W stream of Step 5 (nothing to stream without a walk state)
+  p.streamed = (a.r_prev != nullptr && a.max_blocks > 1) ? 1 : 0;
+  if (p.streamed) {
+    const size_t smem = (size_t)kStages * kChunkBytes + sizeof(float) * ((size_t)kStages * kChunkRows + (size_t)kRowGroups * kTileW);
+    if (int32_t rc = allow_dynamic_smem(decode_stream_kernel, smem, "sw_decode_select(stream) smem attribute")) return rc;
+    count_launch();
+    launch_pdl(decode_stream_kernel, dim3(p.g_stream), dim3(kThreads), smem, st, p);
+    if (int32_t rc = check_launch("sw_decode_select(stream)")) return rc;
+  }
+  // launch 2: Steps 2-4 (sketches, running key mean, raw score row), beside the stream
+  if (int32_t rc = launch_decode_duty(p, st)) return rc;
+  // launch 3: per-sequence tail
   return launch_decode_tail(p, st);
 }
 

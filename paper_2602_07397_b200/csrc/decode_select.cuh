@@ -1,6 +1,7 @@
-// Bookkeeping shared by the two kernels of sw_decode_select (decode_select.cu: duties + W stream;
-// decode_tail.cu: the per-sequence tail): tile sizes, the kernel parameter block, the chunk / duty arithmetic of
-// one sequence and the chunk -> CTA map.  No arithmetic of the method lives here.
+// Bookkeeping shared by the three kernels of sw_decode_select (decode_duty.cu: Steps 2-4 per 64-column tile;
+// decode_select.cu: the W stream of Step 5; decode_tail.cu: the per-sequence tail): tile sizes, the kernel
+// parameter block, the chunk arithmetic of one sequence and the chunk -> CTA map.  No arithmetic of the method
+// lives here.
 #pragma once
 
 #include "common.cuh"
@@ -9,16 +10,32 @@ namespace swds {
 
 constexpr int kThreads = 256;         // streaming kernel
 constexpr int kTailThreads = 1024;    // tail kernel
-constexpr int kTile = 64;            // columns per tile
-constexpr int kRowGroups = 16;       // row lanes of the vector-matrix product
-constexpr int kChunkRows = 64;
-constexpr int kStages = 4;            // 4 x 16 KB ring + two r_prev rows + the prefix tables: two CTAs per SM
-constexpr int kChunkBytes = kChunkRows * kTile * 4;
-constexpr int kPieces = kChunkBytes / 16 / kThreads;     // 16-byte cp.async pieces per thread per chunk
-constexpr int kMaxBatch = 512;       // sequence lengths and per-sequence work counts live in shared memory
-constexpr int kMaxTiles = 255;       // column tiles per sequence (max_blocks <= 16320)
-constexpr int kHeadRegs = 16;        // head values a thread holds while the loads of a duty are in flight
-constexpr int kKU = 4;               // key-sketch float4s per thread and duty (64 columns x r <= 64)
+// duty kernel: tiles of 64 columns of the new score row
+constexpr int kDutyThreads = 128;
+constexpr int kDutyTile = 64;
+constexpr int kDutyGroup = 1;         // tiles per CTA of the duty kernel
+constexpr int kHeadRegs = 16;         // head values a thread holds while the loads of a tile are in flight
+constexpr int kKU = 8;                // key-sketch float4s per thread and tile (64 columns x r <= 64)
+// streaming kernel: chunk = kChunkRows rows x kTileW columns of the cached W = 16 KB; a row piece of a chunk is
+// kTileW * 4 bytes of consecutive addresses (what a DRAM page likes), the pieces right of the diagonal are not read
+#ifndef SW_DS_TILEW
+#define SW_DS_TILEW 256
+#endif
+constexpr int kTileW = SW_DS_TILEW;
+constexpr int kChunkBytes = 16384;
+constexpr int kChunkRows = kChunkBytes / (kTileW * 4);
+constexpr int kRho = kTileW / kChunkRows;              // row chunks per tile width
+constexpr int kQuads = kTileW / 4;                     // float4 columns of a tile
+constexpr int kRowGroups = kThreads / kQuads;          // threads that share a float4 column
+constexpr int kRowsPerThread = kChunkRows / kRowGroups;
+constexpr int kPieces = kChunkBytes / 16 / kThreads;   // 16-byte cp.async pieces per thread per chunk
+#ifndef SW_DS_STAGES
+#define SW_DS_STAGES 5
+#endif
+constexpr int kStages = SW_DS_STAGES; // ring of chunks: kStages x (16 KB + the chunk's r_prev values); two CTAs per SM
+constexpr int kMaxBatch = 512;        // sequence lengths and per-sequence work counts live in shared memory
+constexpr int kMaxTiles = 255;        // stream tiles per sequence the tail's slot table holds
+static_assert(kChunkRows * kTileW * 4 == kChunkBytes && kChunkRows % kRowGroups == 0 && kTileW % kChunkRows == 0, "tile shape");
 
 struct Params {
   const void* q;  int64_t q_stride_seq, q_stride_head;  int h_q;
@@ -32,32 +49,32 @@ struct Params {
   const int32_t* tau;  int tau_max;
   int32_t* idx;  int32_t* count;
   int batch, B, max_blocks;
+  int dtype, d;                      // of q / k_new
   int use_async;                     // W streamed by cp.async (needs 16-byte aligned rows), else plain loads
+  int streamed;                      // the streaming kernel runs in front of the duty kernel (there is a walk state)
   // workspace
   float* ws_scores;                  // [batch][mbp] raw scores of the new row
-  float* ws_part;                    // [batch][tiles_max][slots][64] partial walk sums
-  int mbp, tiles_max, slots;
+  float* ws_part;                    // [g_stream + batch * tiles_max][kTileW] partial walk sums (see part_id)
+  int mbp, tiles_max;                // mbp: max_blocks rounded up to kTileW; tiles_max = mbp / kTileW
   int g_stream;                      // grid of the streaming kernel (the tail derives the partial slots from it)
 };
 
-// Work bookkeeping of one sequence.  b_q = 64 a + e; column tile c < a has rows [64 c, b_q): a - c + (e > 0)
-// chunks; tile a (the one that holds b_q) has (e > 0) chunks.  a + 1 duties.  No chunks without a walk
-// (r_prev = NULL).
+// Stream bookkeeping of one sequence.  Rows [0, b_q) of the cached W take part in Step 5 (row b_q is the new row,
+// added by the tail).  Column tile c holds columns [c kTileW, (c + 1) kTileW); its rows above c kTileW are zero
+// (lower-triangular), so it is streamed as rows [c kTileW, b_q) in chunks of kChunkRows: nr - c kRho chunks with
+// nr = ceil(b_q / kChunkRows).  nt = ceil(b_q / kTileW) tiles have chunks.  No chunks without a walk (r_prev = NULL).
 struct SeqInfo {
-  int bq, a, eps;
-  __device__ __forceinline__ int chunks(int tile, bool walk) const { return walk ? (tile < a ? a - tile + eps : eps) : 0; }
-  __device__ __forceinline__ int chunks_before(int tile, bool walk) const {        // tile <= a
-    return walk ? tile * a - tile * (tile - 1) / 2 + tile * eps : 0;
-  }
-  __device__ __forceinline__ int total_chunks(bool walk) const { return walk ? a * (a + 1) / 2 + a * eps + eps : 0; }
-  __device__ __forceinline__ int duties() const { return a + 1; }
+  int bq, nr, nt;
+  __device__ __forceinline__ int chunks(int tile) const { return tile < nt ? nr - tile * kRho : 0; }
+  __device__ __forceinline__ int chunks_before(int tile) const { return tile * nr - kRho * (tile * (tile - 1) / 2); }   // tile <= nt
+  __device__ __forceinline__ int total_chunks() const { return chunks_before(nt); }
 };
-__device__ __forceinline__ SeqInfo seq_info(const int32_t* seqlens, int seq, int B) {
+__device__ __forceinline__ SeqInfo seq_info(const int32_t* seqlens, int seq, int B, bool walk) {
   SeqInfo s;
-  const int t = seqlens[seq];                          // (a shared-memory copy after the first pass)
+  const int t = seqlens[seq];                          // (a shared-memory copy in the streaming kernel)
   s.bq = (t - 1) / B;                                  // block of the new token = b_curr
-  s.a = s.bq / kTile;
-  s.eps = (s.bq % kTile) != 0;
+  s.nr = walk ? (s.bq + kChunkRows - 1) / kChunkRows : 0;
+  s.nt = walk ? (s.bq + kTileW - 1) / kTileW : 0;
   return s;
 }
 // CTA that owns item g when T items are dealt to G CTAs as [i T / G, (i+1) T / G)
@@ -65,10 +82,14 @@ __device__ __forceinline__ int cta_of(long long g, int T, int G) {
   const long long num = (g + 1) * G - 1;
   return (num < (1ll << 31)) ? (int)((unsigned)num / (unsigned)T) : (int)(num / T);
 }
-
+// One partial (kTileW floats) per (tile, CTA that holds chunks of it).  Both the CTA index and the running tile
+// index (tiles with chunks, counted over the batch) grow along the chunk order, so cta + tile_index is unique:
+// the partials of a tile are the consecutive ids [first_cta + ti, last_cta + ti].
+__device__ __forceinline__ int part_id(int cta, int tile_index) { return cta + tile_index; }
 
 }  // namespace swds
 
 namespace sw {
+int32_t launch_decode_duty(const swds::Params& p, cudaStream_t st);
 int32_t launch_decode_tail(const swds::Params& p, cudaStream_t st);
 }

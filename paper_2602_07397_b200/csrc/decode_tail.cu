@@ -1,5 +1,6 @@
-// sw_decode_select, second kernel: Alg. 2 Steps 4-6 on the whole row of one sequence per CTA,
-// from what decode_select.cu left in the workspace (the raw score row and the partial sums of r_prev W):
+// sw_decode_select, third kernel: Alg. 2 Steps 4-6 on the whole row of one sequence per CTA,
+// from what decode_duty.cu (the raw score row) and decode_select.cu (the partial sums of r_prev W) left in the
+// workspace:
 //   A_new = softmax of the score row (P5), W_new = A_new^s, stored as row b_q of the cached W (Step 4);
 //   r = sum of the partials (slot order: deterministic) + r_prev[b_q] W_new (Step 5); r_out = r / max|r| (P9);
 //   S = TopK(r_out[0..b_q), tau - |forced|) U {b_q} (U {0}) (Step 6; select.cuh, bit-exact given r_out).
@@ -25,28 +26,44 @@ __device__ __forceinline__ float block_max(float v, float* s_red) {
   float m = s_red[threadIdx.x & 31];                 // NT / 32 = 32 partial results
   return swd::warp_max(m);
 }
-__device__ __forceinline__ float block_sum(float v, float* s_red) {
-  v = swd::warp_sum(v);
+// three integer sums over the block in one pass (two barriers)
+__device__ __forceinline__ void block_sum3_i(int& a, int& b, int& c, int (*s_red)[NT / 32]) {
+  a = swd::warp_sum_i(a); b = swd::warp_sum_i(b); c = swd::warp_sum_i(c);
   __syncthreads();
-  if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
+  if ((threadIdx.x & 31) == 0) { s_red[0][threadIdx.x >> 5] = a; s_red[1][threadIdx.x >> 5] = b; s_red[2][threadIdx.x >> 5] = c; }
   __syncthreads();
-  float m = s_red[threadIdx.x & 31];
-  return swd::warp_sum(m);                           // the same order in every warp
+  a = swd::warp_sum_i(s_red[0][threadIdx.x & 31]);
+  b = swd::warp_sum_i(s_red[1][threadIdx.x & 31]);
+  c = swd::warp_sum_i(s_red[2][threadIdx.x & 31]);
 }
-__device__ __forceinline__ int block_sum_i(int v, int* s_red) {
-  v = swd::warp_sum_i(v);
+// softmax statistics of the score row in one pass: every thread holds (m, e) = (max, sum of exp(x - max)) of its
+// entries; pairs merge as (max(m1, m2), e1 exp(m1 - m) + e2 exp(m2 - m)) -- one block-wide reduction (two barriers)
+// instead of a max reduction followed by a sum reduction
+__device__ __forceinline__ void merge_me(float& m, float& e, float m2, float e2) {
+  const float mn = fmaxf(m, m2);
+  const float a = (m == -INFINITY) ? 0.f : e * expf(m - mn), b = (m2 == -INFINITY) ? 0.f : e2 * expf(m2 - mn);
+  m = mn; e = a + b;
+}
+__device__ __forceinline__ void block_softmax_stats(float& m, float& e, float (*s_red)[NT / 32]) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) merge_me(m, e, __shfl_xor_sync(0xffffffffu, m, o), __shfl_xor_sync(0xffffffffu, e, o));
   __syncthreads();
-  if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
+  if ((threadIdx.x & 31) == 0) { s_red[0][threadIdx.x >> 5] = m; s_red[1][threadIdx.x >> 5] = e; }
   __syncthreads();
-  return swd::warp_sum_i(s_red[threadIdx.x & 31]);
+  m = s_red[0][threadIdx.x & 31]; e = s_red[1][threadIdx.x & 31];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) merge_me(m, e, __shfl_xor_sync(0xffffffffu, m, o), __shfl_xor_sync(0xffffffffu, e, o));
 }
 
 __global__ void __launch_bounds__(NT, 1)
-decode_tail_kernel(const Params p) {
+decode_tail_kernel(const Params p_in) {
+  Params p = p_in;                                    // (the pointers to earlier kernels' data pass through pdl_wait)
   extern __shared__ __align__(16) float s_row[];     // [mbp]
   __shared__ float s_red[NT / 32];
-  __shared__ int s_redi[NT / 32];
-  __shared__ unsigned char s_nslot[kMaxTiles + 1];   // partials per column tile
+  __shared__ float s_red2[2][NT / 32];
+  __shared__ int s_redi[3][NT / 32];
+  __shared__ unsigned short s_nslot[kMaxTiles + 1];  // partials per stream tile
+  __shared__ int s_first[kMaxTiles + 1];             // id of the tile's first partial (decode_select.cuh: part_id)
   __shared__ swsel::Scratch scratch;
   const int tid = threadIdx.x, seq = blockIdx.x;
   swd::pdl_launch_dependents();                       // (the attention kernel waits for this one before it reads idx)
@@ -54,50 +71,56 @@ decode_tail_kernel(const Params p) {
   const int mb = p.max_blocks;
 
   // ---- independent of the streaming kernel: chunk prefix of this sequence, T, tau, r_prev[b_q] -------------
-  int mine = 0, before = 0;
+  int mine = 0, before = 0, tbefore = 0;
   for (int sq = tid; sq < p.batch; sq += NT) {
-    const int c = seq_info(p.seqlens, sq, p.B).total_chunks(walk);
+    const SeqInfo o = seq_info(p.seqlens, sq, p.B, walk);
+    const int c = o.total_chunks();
     mine += c;
-    if (sq < seq) before += c;
+    if (sq < seq) { before += c; tbefore += o.nt; }
   }
-  const int T = block_sum_i(mine, s_redi);
-  const int pref = block_sum_i(before, s_redi);
+  block_sum3_i(mine, before, tbefore, s_redi);
+  const int T = mine, pref = before;                  // chunks of the batch / of the sequences before this one
+  const int tpref = tbefore;                          // tiles with chunks of the sequences before this one
   const int G = max(1, min(p.g_stream, T));           // CTAs of the streaming kernel that hold chunks
-  const SeqInfo si = seq_info(p.seqlens, seq, p.B);
+  const SeqInfo si = seq_info(p.seqlens, seq, p.B, walk);
   const int bq = si.bq, hi = bq + 1;
-  const int tt = max(0, min(__ldg(p.tau + seq), p.tau_max));
-  const float rq = walk ? __ldg(p.r_prev + (int64_t)seq * mb + bq) : 1.f;
-  // partials per column tile = CTAs of the streaming kernel that share the tile's chunks
-  for (int tl = tid; tl <= si.a; tl += NT) {
-    const int nch = si.chunks(tl, walk);
-    int ns = 0;
+  const int tt = max(0, min(__ldg(p.tau + seq), p.tau_max));   // (tau, seqlens: written before this selection started)
+  // partials per stream tile = CTAs of the streaming kernel that share the tile's chunks
+  for (int tl = tid; tl < p.tiles_max; tl += NT) {
+    const int nch = si.chunks(tl);
+    int ns = 0, first = 0;
     if (nch > 0) {
-      const long long f0 = pref + si.chunks_before(tl, walk);
-      ns = cta_of(f0 + nch - 1, T, G) - cta_of(f0, T, G) + 1;
+      const long long f0 = pref + si.chunks_before(tl);
+      first = cta_of(f0, T, G);
+      ns = cta_of(f0 + nch - 1, T, G) - first + 1;
     }
-    s_nslot[tl] = (unsigned char)min(ns, 255);
+    s_nslot[tl] = (unsigned short)ns;
+    s_first[tl] = part_id(first, tpref + tl);
   }
-  swd::pdl_wait();                                    // the streaming kernel's scores and partials are visible
+  swd::pdl_wait(p.ws_scores, p.ws_part, p.r_prev);             // the duty kernel's scores and the stream's partials are visible
 
+  const float rq = walk ? __ldcg(p.r_prev + (int64_t)seq * mb + bq) : 1.f;   // (consumed after the softmax statistics)
   const float* sc = p.ws_scores + (int64_t)seq * p.mbp;
   float lmax = -INFINITY;
   for (int j = tid; j < hi; j += NT) { const float v = __ldcg(sc + j); s_row[j] = v; lmax = fmaxf(lmax, v); }
   float m = 0.f, inv_l = 1.f;
   if (soft) {
-    m = block_max(lmax, s_red);
     float e = 0.f;
-    for (int j = tid; j < hi; j += NT) e += expf(s_row[j] - m);
-    inv_l = 1.f / block_sum(e, s_red);
+    if (lmax != -INFINITY)
+      for (int j = tid; j < hi; j += NT) e += expf(s_row[j] - lmax);   // (the thread's own entries)
+    m = lmax;
+    block_softmax_stats(m, e, s_red2);
+    inv_l = 1.f / e;
   } else {
     __syncthreads();                                  // s_nslot
   }
   // W_new = A^s; Alg. 2 Step 4 cache update: the new row becomes row b_q of the cached W,
   // zeros right of the diagonal.  Row b_q is never read while b_q is the current block.
   // Step 5: r[j] = sum_{m < b_q} r_prev[m] W[m][j] + r_prev[b_q] w[j], the partial sums in slot order; the loads of
-  // 2 columns x 4 slots are in flight per thread (a dependent load per slot cost 5 us with 256 threads).
+  // 2 columns x 8 slots are in flight per thread (a dependent load per slot cost 5 us with 256 threads).
   float* wrow = p.W + (int64_t)seq * p.w_stride_seq + (int64_t)bq * mb;
   float lamax = 0.f;
-  constexpr int kCols = 2, kSl = 4;
+  constexpr int kCols = 2, kSl = 8;
   for (int j0 = 0; j0 < mb; j0 += kCols * NT) {
     float v[kCols];
     int ns[kCols], nsmax = 0;
@@ -106,9 +129,10 @@ decode_tail_kernel(const Params p) {
     for (int c = 0; c < kCols; ++c) {
       const int j = j0 + c * NT + tid;
       v[c] = 0.f;
-      ns[c] = (j < hi) ? (int)s_nslot[j / kTile] : 0;
+      const int tl = min(j, mb - 1) / kTileW;
+      ns[c] = (j < hi) ? (int)s_nslot[tl] : 0;
       nsmax = max(nsmax, ns[c]);
-      pp[c] = p.ws_part + (((int64_t)seq * p.tiles_max + min(j, mb - 1) / kTile) * p.slots) * kTile + (j & (kTile - 1));
+      pp[c] = p.ws_part + (int64_t)s_first[tl] * kTileW + (j & (kTileW - 1));
     }
     nsmax = __reduce_max_sync(0xffffffffu, nsmax);
     for (int s0 = 0; s0 < nsmax; s0 += kSl) {
@@ -116,7 +140,7 @@ decode_tail_kernel(const Params p) {
 #pragma unroll
       for (int e = 0; e < kSl; ++e)
 #pragma unroll
-        for (int c = 0; c < kCols; ++c) x[e][c] = (s0 + e < ns[c]) ? __ldcg(pp[c] + (s0 + e) * kTile) : 0.f;
+        for (int c = 0; c < kCols; ++c) x[e][c] = (s0 + e < ns[c]) ? __ldcg(pp[c] + (s0 + e) * kTileW) : 0.f;
 #pragma unroll
       for (int e = 0; e < kSl; ++e)
 #pragma unroll

@@ -5,9 +5,13 @@
 //
 // One CTA of kThreads threads per row (256 unless the translation unit defines SWSEL_THREADS, a multiple of 256,
 // before including this file):
-//   * 4 radix passes of 8 bits on one shared histogram (plain shared-memory atomics; a warp whose lanes
-//     all hit the same bin sends one add), a 256-thread suffix scan picks the bin; rows of up to 2048
-//     candidates keep their keys in registers, so only the histogram touches memory;
+//   * rows of up to 8 * kThreads candidates keep their keys in registers (2, 4 or 8 per thread by row length) and
+//     take 3 radix passes of 11 + 11 + 10 bits on one shared histogram of 2048 bins (plain shared-memory atomics; a
+//     warp whose keys all hit the same bin sends one add); every thread owns 2048 / kThreads adjacent bins, a
+//     block-wide suffix scan of the owners' counts picks the bin: three barriers per pass.  (Four passes of 8 bits
+//     with four barriers each took 6 of the 12 us of the decode tail: scores rescaled to [0, 1] share a handful of
+//     exponent bytes, so the first pass serialised on two or three bins.)
+//   * longer rows re-read their scores: 4 passes of 8 bits, thread b < 256 owns bin b;
 //   * one ordered compaction: every thread owns a contiguous index range, a block scan of the
 //     (certain, equal-to-threshold) counts gives each range its output offset.
 #pragma once
@@ -21,10 +25,14 @@ namespace swsel {
 #endif
 constexpr int kThreads = SWSEL_THREADS;
 constexpr int kWarps = kThreads / 32;
-static_assert(kThreads >= 256 && kThreads % 256 == 0, "thread b < 256 owns histogram bin b");
+static_assert(kThreads >= 256 && kThreads % 256 == 0 && kWarps <= 32, "thread b < 256 owns histogram bin b; one lane per warp total");
+
+constexpr int kBins = 2048;                  // register path: digits of 11, 11 and 10 bits
+constexpr int kBinsPer = kBins / kThreads;   // adjacent bins owned by a thread
+static_assert(kBins % kThreads == 0, "every thread owns the same number of bins");
 
 struct Scratch {
-  uint32_t hist[256];
+  uint32_t hist[kBins];
   uint32_t warp_tot[kWarps];
   unsigned long long warp_scan[kWarps];
   uint32_t bcast[2];
@@ -36,6 +44,22 @@ __device__ __forceinline__ uint32_t order_key(float v) {
   if (v == 0.f) v = 0.f;               // -0 and +0 compare equal
   uint32_t u = __float_as_uint(v);
   return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+
+// sum of t[w] over the warps w > warp (suffix) or w < warp (prefix): every warp reads the kWarps <= 32 totals once and
+// adds them with shuffles -- a loop over the totals is a chain of dependent shared-memory loads (31 of them for the
+// first warp of 1024 threads: 0.8 us per radix pass, measured)
+__device__ __forceinline__ uint32_t warps_above(const uint32_t* t, int warp, int lane) {
+  uint32_t v = (lane < kWarps && lane > warp) ? t[lane] : 0u;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ unsigned long long warps_below(const unsigned long long* t, int warp, int lane) {
+  unsigned long long v = (lane < kWarps && lane < warp) ? t[lane] : 0ull;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
 }
 
 struct RowJob {
@@ -105,7 +129,7 @@ __device__ void radix_threshold(Load load, const RowJob& J, Scratch& S, uint32_t
     }
     if (lane == 0) S.warp_tot[warp] = suf;
     __syncthreads();
-    for (int w = warp + 1; w < kWarps; ++w) suf += S.warp_tot[w];
+    suf += warps_above(S.warp_tot, warp, lane);
     const uint32_t above = suf - cnt;                   // candidates in strictly higher bins
     if ((int)above < remaining && (int)suf >= remaining) { S.bcast[0] = (uint32_t)tid; S.bcast[1] = above; }
     __syncthreads();
@@ -117,43 +141,54 @@ __device__ void radix_threshold(Load load, const RowJob& J, Scratch& S, uint32_t
   n_gt_out = n_gt;
 }
 
-// Register variant for rows of at most kRegKeys * kThreads candidates (b <= 2048): every thread keeps the
-// keys of its contiguous index range [lo, hi) in registers, so the four passes and the compaction touch
-// memory only for the histogram.  cmask: bit e set = index lo + e is a non-forced candidate.
+// Register variant for rows of at most kRegKeys * kThreads candidates (b <= 2048 at 256 threads): every thread keeps
+// the keys of its contiguous index range [lo, hi) in registers, so the passes and the compaction touch memory only
+// for the histogram.  cmask: bit e set = index lo + e is a non-forced candidate.  Three passes (bits 31-21, 20-10,
+// 9-0); thread t owns bins [t kBinsPer, (t + 1) kBinsPer) and clears them as it reads them.
 constexpr int kRegKeys = 8;
 template <int K>
 __device__ __forceinline__ void radix_threshold_regs(const uint32_t (&key)[K], uint32_t cmask, const RowJob& J,
                                                      Scratch& S, uint32_t& thr, int& n_gt_out) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   uint32_t prefix = 0;
-  int remaining = J.need;
+  int remaining = J.need;      // rank (1-based, from the top) still to locate inside the prefix bucket
   int n_gt = 0;
-  for (int pass = 0; pass < 4; ++pass) {
-    const int shift = 24 - 8 * pass;
-    if (tid < 256) S.hist[tid] = 0;
-    __syncthreads();
-    const uint32_t mask_hi = (pass == 0) ? 0u : (0xffffffffu << (shift + 8));
+#pragma unroll
+  for (int b = 0; b < kBinsPer; ++b) S.hist[tid * kBinsPer + b] = 0;
+  __syncthreads();
+#pragma unroll
+  for (int pass = 0; pass < 3; ++pass) {
+    const int shift = (pass == 0) ? 21 : (pass == 1) ? 10 : 0;
+    const uint32_t dmask = (pass == 2) ? 0x3ffu : 0x7ffu;
+    const uint32_t mask_hi = (pass == 0) ? 0u : (pass == 1) ? 0xffe00000u : 0xfffffc00u;
     uint32_t bin[K];
     bool same = true;
 #pragma unroll
     for (int e = 0; e < K; ++e) {
       const bool in = ((cmask >> e) & 1u) && (key[e] & mask_hi) == prefix;
-      bin[e] = in ? ((key[e] >> shift) & 0xffu) : 256u;
+      bin[e] = in ? ((key[e] >> shift) & dmask) : (uint32_t)kBins;
       same = same && bin[e] == bin[0];
     }
-    // plain shared-memory atomics (distinct bins of a warp run in parallel); only a warp whose 256 keys all
-    // fall into one bin -- the degenerate row of equal scores -- would serialise, so it sends a single add
+    // plain shared-memory atomics (distinct bins of a warp run in parallel); only a warp whose keys all fall into
+    // one bin -- the degenerate row of equal scores -- would serialise, so it sends a single add
     const uint32_t b0 = __shfl_sync(0xffffffffu, bin[0], 0);
     if (__all_sync(0xffffffffu, same && bin[0] == b0)) {
-      if (lane == 0 && b0 < 256u) atomicAdd(&S.hist[b0], 32u * K);
+      if (lane == 0 && b0 < (uint32_t)kBins) atomicAdd(&S.hist[b0], 32u * K);
     } else {
 #pragma unroll
       for (int e = 0; e < K; ++e)
-        if (bin[e] < 256u) atomicAdd(&S.hist[bin[e]], 1u);
+        if (bin[e] < (uint32_t)kBins) atomicAdd(&S.hist[bin[e]], 1u);
     }
     __syncthreads();
-    const uint32_t cnt = (tid < 256) ? S.hist[tid] : 0u;
-    uint32_t suf = cnt;
+    // counts of the own bins (cleared for the next pass), then an inclusive suffix sum over the owners t..kThreads-1
+    uint32_t cnt[kBinsPer], own = 0;
+#pragma unroll
+    for (int b = 0; b < kBinsPer; ++b) {
+      cnt[b] = S.hist[tid * kBinsPer + b];
+      S.hist[tid * kBinsPer + b] = 0;
+      own += cnt[b];
+    }
+    uint32_t suf = own;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
       const uint32_t v = __shfl_down_sync(0xffffffffu, suf, o);
@@ -161,9 +196,16 @@ __device__ __forceinline__ void radix_threshold_regs(const uint32_t (&key)[K], u
     }
     if (lane == 0) S.warp_tot[warp] = suf;
     __syncthreads();
-    for (int w = warp + 1; w < kWarps; ++w) suf += S.warp_tot[w];
-    const uint32_t above = suf - cnt;
-    if ((int)above < remaining && (int)suf >= remaining) { S.bcast[0] = (uint32_t)tid; S.bcast[1] = above; }
+    suf += warps_above(S.warp_tot, warp, lane);
+    uint32_t above = suf - own;                         // candidates in the bins of higher threads
+#pragma unroll
+    for (int b = kBinsPer - 1; b >= 0; --b) {
+      if ((int)above < remaining && (int)(above + cnt[b]) >= remaining) {
+        S.bcast[0] = (uint32_t)(tid * kBinsPer + b);
+        S.bcast[1] = above;
+      }
+      above += cnt[b];
+    }
     __syncthreads();
     prefix |= S.bcast[0] << shift;
     n_gt += (int)S.bcast[1];
@@ -214,8 +256,7 @@ __device__ __forceinline__ void select_row_regs(Load load, const RowJob& J, int3
   }
   if (lane == 31) S.warp_scan[warp] = incl;
   __syncthreads();
-  unsigned long long base = 0;
-  for (int w = 0; w < warp; ++w) base += S.warp_scan[w];
+  const unsigned long long base = warps_below(S.warp_scan, warp, lane);
   const unsigned long long excl = base + incl - v;
   int c_before = (int)(excl & 0xffffffffu), e_before = (int)(excl >> 32);
 #pragma unroll
@@ -272,8 +313,7 @@ __device__ void select_row(Load load, const RowJob& J, int32_t* __restrict__ out
   }
   if (lane == 31) S.warp_scan[warp] = incl;
   __syncthreads();
-  unsigned long long base = 0;
-  for (int w = 0; w < warp; ++w) base += S.warp_scan[w];
+  const unsigned long long base = warps_below(S.warp_scan, warp, lane);
   const unsigned long long excl = base + incl - v;
   int c_before = (int)(excl & 0xffffffffu), e_before = (int)(excl >> 32);
   for (int j = lo; j < hi; ++j) {

@@ -19,9 +19,7 @@ using namespace swds;
 
 // One CTA of 128 threads per (sequence, 64-column tile): all its loads are in flight at once (one round trip through
 // a memory system the stream keeps busy: a CTA that walked over four tiles took 17 us beside the stream, this takes
-// ~6).  The CTAs are launched behind the streaming kernel's (two per SM, placed first) and several fit beside those;
-// they stay resident until the stream has finished (see the end), packed onto a part of the SMs, so that the tail
-// kernel still finds SMs of its own to become resident early.
+// ~6).  The CTAs are launched behind the streaming kernel's (two per SM, placed first) and several fit beside those.
 template <typename TIn, int D>
 __global__ void __launch_bounds__(kDutyThreads, 6)
 decode_duty_kernel(const Params p_in) {
@@ -150,9 +148,10 @@ decode_duty_kernel(const Params p_in) {
       }
     }
   }
-  // The tail kernel waits for this kernel only; waiting for the streaming kernel here makes "this kernel complete"
-  // imply "stream complete" (the CTA holds no resources the stream needs).
-  swd::pdl_wait();
+  // The tail kernel waits for this kernel only; one CTA waiting for the streaming kernel here makes "this kernel
+  // complete" imply "stream complete".  Only one: a CTA that stays resident keeps the tail (1024 threads, a whole
+  // SM's registers) off its SM, and the tail's prologue should run while the last streaming CTAs drain.
+  if (blockIdx.x == 0 && blockIdx.y == 0) swd::pdl_wait();
 }
 
 }  // namespace

@@ -32,7 +32,7 @@ constexpr int kBinsPer = kBins / kThreads;   // adjacent bins owned by a thread
 static_assert(kBins % kThreads == 0, "every thread owns the same number of bins");
 
 struct Scratch {
-  uint32_t hist[kBins];
+  alignas(16) uint32_t hist[kBins];
   uint32_t warp_tot[kWarps];
   unsigned long long warp_scan[kWarps];
   uint32_t bcast[2];
@@ -182,12 +182,23 @@ __device__ __forceinline__ void radix_threshold_regs(const uint32_t (&key)[K], u
     __syncthreads();
     // counts of the own bins (cleared for the next pass), then an inclusive suffix sum over the owners t..kThreads-1
     uint32_t cnt[kBinsPer], own = 0;
+    if constexpr (kBinsPer % 4 == 0) {                  // 128-bit accesses: 8 words per thread would conflict 8 ways
+      uint4* h4 = reinterpret_cast<uint4*>(S.hist + tid * kBinsPer);
 #pragma unroll
-    for (int b = 0; b < kBinsPer; ++b) {
-      cnt[b] = S.hist[tid * kBinsPer + b];
-      S.hist[tid * kBinsPer + b] = 0;
-      own += cnt[b];
+      for (int b = 0; b < kBinsPer / 4; ++b) {
+        const uint4 v = h4[b];
+        h4[b] = make_uint4(0u, 0u, 0u, 0u);
+        cnt[4 * b] = v.x; cnt[4 * b + 1] = v.y; cnt[4 * b + 2] = v.z; cnt[4 * b + 3] = v.w;
+      }
+    } else {
+#pragma unroll
+      for (int b = 0; b < kBinsPer; ++b) {
+        cnt[b] = S.hist[tid * kBinsPer + b];
+        S.hist[tid * kBinsPer + b] = 0;
+      }
     }
+#pragma unroll
+    for (int b = 0; b < kBinsPer; ++b) own += cnt[b];
     uint32_t suf = own;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {

@@ -111,3 +111,89 @@ def test_decode_step_captures_into_a_cuda_graph(sw):
         assert torch.equal(idxs[l], ref_idx[l])
         assert torch.equal(outs[l], ref_out[l])
         assert (idxs[l][:, -1] == (t - 1) // B).all()          # the current block is always selected
+
+
+def _random_decode_caches(batch, mb, d, r, seed):
+    g = torch.Generator(device="cuda"); g.manual_seed(seed)
+    Wc = torch.rand(batch, mb, mb, device="cuda", generator=g).tril_()
+    Wc /= Wc.sum(-1, keepdim=True)
+    kbar = torch.randn(batch, mb, d, device="cuda", generator=g)
+    ks = torch.randn(batch, mb, r, device="cuda", generator=g) * 0.3
+    return Wc, kbar, ks
+
+
+@pytest.mark.parametrize("mb", [304, 301])      # max_blocks % 4 == 0: cp.async stream of the cached W; else plain loads
+def test_decode_selection_ragged_batch_fused_equals_row_mode(sw, mb):
+    """A batch of sequences of very different lengths through sw_decode_select (three kernels: the W stream dealt over
+    the whole grid in chunks numbered across sequences, the score kernel beside it, the per-sequence tail) against the
+    five row-mode calls, which tests/test_gpu_parity.py checks against the oracle one sequence at a time.  Lengths: a
+    first block (b_q = 0: nothing to stream), b_q a multiple of the 256-column stream tile, the longest the cache
+    holds, short ones between -- the partial slots of a tile then come from CTAs shared with other sequences."""
+    B, d, r, h_q, h_kv, s = 64, 128, 64, 8, 2, 2
+    ts = [5, 64 * 3 + 5, 64 * 256 + 1, 64 * (mb - 1) + 7, 64 * 17, 64 * 257]
+    batch = len(ts)
+    taus = [max(1, min(40, (t + B - 1) // B // 3 + 1)) for t in ts]
+    signs, cols = gen.srht_params(3, d, r)
+    seqlens = torch.tensor(ts, dtype=torch.int32, device="cuda")
+    pipes = [sw.DecodePipeline(batch, mb, h_q, h_kv, d, B, r, s, taus, signs, cols) for _ in range(2)]
+    caches = [_random_decode_caches(batch, mb, d, r, 11) for _ in range(2)]
+    for layer in range(3):
+        torch.manual_seed(40 + layer)
+        q = torch.randn(batch, h_q, d).bfloat16().cuda(); k = torch.randn(batch, h_kv, d).bfloat16().cuda()
+        for dp, (Wc, kbar, ks), fused in zip(pipes, caches, (True, False)):
+            dp.idx.fill_(-7); dp.count.fill_(-7)
+            dp.select(q, k, seqlens, kbar, ks, Wc, fused=fused)
+        torch.cuda.synchronize()
+        (Wf, kbf, ksf), (Wu, kbu, ksu) = caches
+        assert torch.allclose(kbf, kbu, rtol=0, atol=1e-6) and torch.allclose(ksf, ksu, rtol=0, atol=1e-5)
+        rf = pipes[0].rvec[pipes[0].cur].cpu().numpy(); ru = pipes[1].rvec[pipes[1].cur].cpu().numpy()
+        for s_, t in enumerate(ts):
+            bq = (t - 1) // B
+            scale = np.abs(ru[s_]).max()
+            assert np.abs(rf[s_] - ru[s_]).max() <= 1e-5 * scale, (layer, s_)
+            assert (rf[s_, bq + 1:] == 0).all()
+            wf = Wf[s_, bq].cpu().numpy(); wu = Wu[s_, bq].cpu().numpy()
+            assert np.abs(wf - wu).max() <= 1e-6 * max(np.abs(wu).max(), 1e-30)
+            cf, cu = pipes[0].count[s_].item(), pipes[1].count[s_].item()
+            assert cf == cu == min(taus[s_], bq + 1)
+            got = pipes[0].idx[s_, :cf].cpu().numpy(); ref = pipes[1].idx[s_, :cu].cpu().numpy()
+            assert np.all(np.diff(got) > 0) and bq in got
+            diff = set(got.tolist()) ^ set(ref.tolist())
+            free = [j for j in ref.tolist() if j not in (0, bq)]
+            kth = min(ru[s_][free]) if free else 0.0
+            assert all(abs(ru[s_][j] - kth) <= 1e-5 * scale for j in diff), (layer, s_, diff)
+
+
+def test_decode_chain_reads_nothing_before_its_producers_finish(sw):
+    """sw_decode_select + sw_sparse_attn_decode are five kernels chained as programmatic dependents: each may become
+    resident while its predecessor runs and must read nothing an earlier kernel writes before griddepcontrol.wait.
+    (Loads the compiler treats as invariant -- __ldg, const __restrict__ -- were once scheduled above the wait: the
+    attention kernel read count[] / idx[] the selection had not written yet.)  The block lists are poisoned before
+    every step; the output of the chained step must equal that of the attention call alone on the finished lists."""
+    batch, t, h_q, h_kv, d, B, r, s = 4, 64 * 512, 8, 2, 128, 64, 64, 2
+    mb = t // B
+    tau = mb // 5
+    signs, cols = gen.srht_params(3, d, r)
+    dp = sw.DecodePipeline(batch, mb, h_q, h_kv, d, B, r, s, [tau] * batch, signs, cols)
+    seqlens = torch.full((batch,), t, dtype=torch.int32, device="cuda")
+    g = torch.Generator(device="cuda"); g.manual_seed(5)
+    kc = torch.randn(batch, t, h_kv, d, device="cuda", generator=g).bfloat16()
+    vc = torch.randn(batch, t, h_kv, d, device="cuda", generator=g).bfloat16()
+    Wc, kbar, ks = _random_decode_caches(batch, mb, d, r, 6)
+    out = torch.empty(batch, h_q, d, dtype=torch.bfloat16, device="cuda")
+    for it in range(60):
+        q = torch.randn(batch, h_q, d, device="cuda", generator=g).bfloat16()
+        k = torch.randn(batch, h_kv, d, device="cuda", generator=g).bfloat16()
+        dp.idx.fill_(it % 7); dp.count.fill_(1 + it % 5); out.zero_()
+        if it % 3 == 0:
+            torch.cuda.synchronize()
+        dp.reset()
+        for _ in range(1 + it % 3):
+            dp.select(q, k, seqlens, kbar, ks, Wc)
+            dp.attend(q, kc, vc, seqlens, out)
+        torch.cuda.synchronize()
+        chained = out.clone()
+        assert (dp.count == tau).all()
+        dp.attend(q, kc, vc, seqlens, out)
+        torch.cuda.synchronize()
+        assert torch.equal(chained, out), it

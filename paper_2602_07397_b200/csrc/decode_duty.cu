@@ -5,7 +5,7 @@
 //
 // This work is a chain of short dependent steps (loads, two block-wide reductions, an in-warp FWHT, 64 dot products
 // per tile), a few microseconds whatever one does.  It used to run at the head of the streaming CTAs, where it held
-// back the cached-W stream of 264 of the 296 CTAs for ~5 us each (measured: 22 us for the 67 MB of cfg 3).  As its own
+// back the cached-W stream of 256 of the 296 CTAs for ~5 us each (measured: 22 us for the 67 MB of cfg 3).  As its own
 // small kernel it runs BESIDE the stream: it is the streaming kernel's programmatic dependent, released once every
 // streaming CTA has passed griddepcontrol.wait (= everything before this layer's selection is complete), reads nothing
 // the stream writes, and waits for the stream only at its very end so that the tail's wait covers both.

@@ -130,6 +130,8 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
                                  "plant_frac": gen.PLANT_FRAC, "chain_frac": gen.CHAIN_FRAC, "sink_a": gen.SINK_A}},
         "ms_per_layer": layer_ms,
         "kernel_ms_per_layer": kern_ms,
+        "kernel_ms_per_layer_median": {k: statistics.median(v) for k, v in per.items()},
+        "kernel_ms_per_layer_min": {k: min(v) for k, v in per.items()},
         "selection_overhead_share": sel_ms / (sel_ms + attn_ms),
         "sketch_hbm": {"achieved_gbs": sketch_gbs, "peak_gbs": peaks.get("hbm_gbs"),
                        "frac": sketch_gbs / peaks.get("hbm_gbs")},

@@ -44,6 +44,10 @@ constexpr int kQBytes = kTiles * 128 * 128 * 2;   // 32 KB per tile: [d-half][12
 constexpr int kMaxChunks = 2048 * kTiles;     // 64-key chunks per query row the list buffer holds
 constexpr int kSmemBytes = kQBytes + kStages * kTileBytes + kMaxChunks * 4 + 1024 /*align*/ + 512 /*barriers*/;
 constexpr float kRescaleThreshold = 8.0f;     // log2 units
+#ifndef SW_EARLY_K
+#define SW_EARLY_K 1
+#endif
+constexpr bool kEarlyK = SW_EARLY_K;          // request the first K tiles before the chunk list is built
 
 // barrier map
 constexpr int kBarQ = 0;                      // Q tile landed
@@ -130,6 +134,7 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   auto BAR = [&](int i) { return bar0 + 8u * i; };
   volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(bars + kNumBars);
   volatile int32_t* s_nchunks = reinterpret_cast<volatile int32_t*>(bars + kNumBars + 1);
+  volatile int32_t* s_pre = s_nchunks + 1;                   // K tiles requested during set-up (0, 1 or 2)
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -160,6 +165,29 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     mbar_arrive_expect_tx(BAR(kBarQ), kQBytes);
     tma_load_3d(sQ, &map_q, BAR(kBarQ), 0, kvh * 4, q_tok0);
     tma_load_3d(sQ + kQBytes / 2, &map_q, BAR(kBarQ), 64, kvh * 4, q_tok0);
+    // The first sub-chunk of every selected block holds a visible key (a selected block j exists and, under the
+    // causal mask, j <= i), so the chunk list starts with the first 64 keys of idx[0] (and, for 64-token blocks, of
+    // idx[1]): request those K tiles now instead of after the list has been built and the set-up barrier passed --
+    // their latency then overlaps both.
+    if (kEarlyK) {
+      const int32_t* list = p.idx + (int64_t)gb * p.tau_max;
+      const int cnt = __ldg(p.count + gb);
+      const int j0 = __ldg(list), j1 = (p.tau_max > 1) ? __ldg(list + 1) : -1;
+      int pre = 0;
+      if (cnt > 0) {
+        mbar_arrive_expect_tx(BAR(kBarFull + 0), kTileBytes);
+        tma_load_3d(sKV, &map_k, BAR(kBarFull + 0), 0, kvh, seq_lo + j0 * p.B);
+        tma_load_3d(sKV + kTileBytes / 2, &map_k, BAR(kBarFull + 0), 64, kvh, seq_lo + j0 * p.B);
+        pre = 1;
+        if (TPB == 1 && cnt > 1) {
+          mbar_arrive_expect_tx(BAR(kBarFull + 1), kTileBytes);
+          tma_load_3d(sKV + kTileBytes, &map_k, BAR(kBarFull + 1), 0, kvh, seq_lo + j1 * p.B);
+          tma_load_3d(sKV + kTileBytes + kTileBytes / 2, &map_k, BAR(kBarFull + 1), 64, kvh, seq_lo + j1 * p.B);
+          pre = 2;
+        }
+      }
+      *s_pre = pre;
+    }
   } else if (warp == 2) {
     tmem_alloc<kTmemCols>(smem_u32((const void*)s_tmem));
   } else if (warp == 3) {
@@ -210,7 +238,8 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     // (the whole warp runs the loop; one elected lane issues the copies)
     if (n > 0) {
       const bool leader = elect_one();
-      int c = 0;
+      const int pre = kEarlyK ? __shfl_sync(0xffffffffu, *s_pre, 0) : 0;
+      int c = pre;                                       // (stages 0 .. pre-1 were requested during set-up)
       auto push = [&](const CUtensorMap* m, int chunk) {
         const int st = c % kStages;
         mbar_wait(BAR(kBarEmpty + st), ((c / kStages) & 1) ^ 1);
@@ -224,8 +253,8 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
         __syncwarp();
         ++c;
       };
-      push(&map_k, 0);
-      if (n > 1) push(&map_k, 1);
+      if (pre < 1) push(&map_k, 0);
+      if (n > 1 && pre < 2) push(&map_k, 1);
       for (int k = 0; k < n; ++k) {
         push(&map_v, k);
         if (k + 2 < n) push(&map_k, k + 2);

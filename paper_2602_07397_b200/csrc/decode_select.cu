@@ -94,53 +94,71 @@ decode_stream_kernel(const Params p_in) {
   const int n_my = g_end - g_begin;
   if (n_my == 0) return;
 
-  // ---- cursors over this CTA's chunks (thread-uniform) ------------------------------------------------
-  struct Cursor { int seq, tile, chunk; SeqInfo si; };
+  // ---- cursors over this CTA's chunks (thread-uniform).  The chunk loop is sensitive to its instruction count (a
+  // few dozen extra integer instructions per chunk cost 3 us, measured), so a cursor carries what a step needs --
+  // first row, chunks left in the tile, the tile's base pointers -- and recomputes only when it leaves a tile.
+  struct Cursor {
+    int seq, tile, chunk, n_tile, m0, bq;            // n_tile: chunks of the tile; m0: first row of the chunk
+    const float* wt;                                 // &W[seq][0][tile kTileW]
+    const float* rp;                                 // r_prev of the sequence
+  };
+  auto enter_tile = [&](Cursor& c, const SeqInfo& si) {
+    c.n_tile = si.chunks(c.tile);
+    c.bq = si.bq;
+    c.m0 = c.tile * kTileW + c.chunk * kChunkRows;
+    c.wt = p.W + (int64_t)c.seq * p.w_stride_seq + c.tile * kTileW;
+    c.rp = p.r_prev + (int64_t)c.seq * mb;
+  };
   auto locate = [&](int g) {
     Cursor c;
     int lo = 0, hi = p.batch - 1;
     while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_pref[mid] <= g) lo = mid; else hi = mid - 1; }
     c.seq = lo;
-    c.si = seq_info(s_len, c.seq, p.B, true);
+    const SeqInfo si = seq_info(s_len, c.seq, p.B, true);
     const int local = g - s_pref[c.seq];
-    int tl = 0, th = max(c.si.nt - 1, 0);
-    while (tl < th) { const int mid = (tl + th + 1) >> 1; if (c.si.chunks_before(mid) <= local) tl = mid; else th = mid - 1; }
+    int tl = 0, th = max(si.nt - 1, 0);
+    while (tl < th) { const int mid = (tl + th + 1) >> 1; if (si.chunks_before(mid) <= local) tl = mid; else th = mid - 1; }
     c.tile = tl;
-    c.chunk = local - c.si.chunks_before(tl);
+    c.chunk = local - si.chunks_before(tl);
+    enter_tile(c, si);
     return c;
   };
   auto advance = [&](Cursor& c) {
     ++c.chunk;
-    while (c.seq < p.batch && c.chunk >= c.si.chunks(c.tile)) {
-      c.chunk = 0;
-      if (++c.tile >= c.si.nt) {
-        c.tile = 0;
-        if (++c.seq < p.batch) c.si = seq_info(s_len, c.seq, p.B, true);
-      }
+    c.m0 += kChunkRows;
+    if (c.chunk < c.n_tile) return;
+    SeqInfo si = seq_info(s_len, c.seq, p.B, true);
+    c.chunk = 0;
+    ++c.tile;
+    while (c.seq < p.batch && c.tile >= si.nt) {     // next sequence that has chunks
+      c.tile = 0;
+      if (++c.seq < p.batch) si = seq_info(s_len, c.seq, p.B, true);
     }
+    if (c.seq < p.batch) enter_tile(c, si);
   };
   Cursor cc = locate(g_begin), pc = cc;
 
-  // ---- W stream: chunk = rows [tile kTileW + chunk kChunkRows, +kChunkRows) x columns [tile kTileW, +kTileW) ----
+  // ---- W stream: chunk = rows [m0, m0 + kChunkRows) x columns [tile kTileW, +kTileW) --------------------------
+  // piece u of a thread: row rr_u = (u kThreads + tid) / kQuads of the chunk, float4 column tid % kQuads
+  const int q4 = (tid % kQuads) * 4, rr0 = tid / kQuads;
   int p_left = n_my, issued = 0;
   auto issue_next = [&]() {                           // all threads: request the next chunk (or an empty group)
     if (p_left > 0) {
-      const float* Wseq = p.W + (int64_t)pc.seq * p.w_stride_seq;
-      const int m0 = pc.tile * kTileW + pc.chunk * kChunkRows;
       const int st = issued % kStages;
-      const uint32_t dst = sm100::smem_u32(s_ring + (size_t)st * kChunkBytes);
+      const uint32_t dst = sm100::smem_u32(s_ring + (size_t)st * kChunkBytes) + tid * 16;
+      const float* src = pc.wt + (int64_t)pc.m0 * mb + q4;
+      const int c4 = pc.tile * kTileW + q4;
 #pragma unroll
       for (int u = 0; u < kPieces; ++u) {
-        const int pcs = u * kThreads + tid, rr = pcs / kQuads, m = m0 + rr, c4 = pc.tile * kTileW + (pcs % kQuads) * 4;
+        const int rr = rr0 + u * (kThreads / kQuads), m = pc.m0 + rr;
         // rows >= b_q are not part of the product; W[m][j] = 0 for j > m (block-causal): not requested
-        const bool ok = m < pc.si.bq && c4 <= m && c4 < mb;
-        cp_async16_zfill(dst + pcs * 16, ok ? Wseq + (int64_t)m * mb + c4 : Wseq, ok ? 16 : 0);
+        const bool ok = m < pc.bq && c4 <= m && c4 < mb;
+        cp_async16_zfill(dst + u * (kThreads * 16), ok ? src + rr * mb : pc.wt, ok ? 16 : 0);
       }
       if (tid < kChunkRows / 4) {
-        const int m = m0 + tid * 4;
+        const int m = pc.m0 + tid * 4;
         const bool ok = m < mb;
-        cp_async16_zfill(sm100::smem_u32(s_rp + st * kChunkRows + tid * 4), ok ? p.r_prev + (int64_t)pc.seq * mb + m : p.r_prev,
-                         ok ? 16 : 0);
+        cp_async16_zfill(sm100::smem_u32(s_rp + st * kChunkRows + tid * 4), ok ? pc.rp + m : pc.rp, ok ? 16 : 0);
       }
       ++issued; advance(pc); --p_left;
     }
@@ -154,10 +172,8 @@ decode_stream_kernel(const Params p_in) {
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   const int cq = tid % kQuads, rg = tid / kQuads;
   for (int it = 0; it < n_my; ++it) {
-    const SeqInfo& si = cc.si;
-    const int seq = cc.seq, tile = cc.tile, bq = si.bq;
-    const int m0 = tile * kTileW + cc.chunk * kChunkRows;
-    const int rows = min(kChunkRows, bq - m0);        // rows >= b_q are not part of the product
+    const int seq = cc.seq, tile = cc.tile, m0 = cc.m0;
+    const int rows = min(kChunkRows, cc.bq - m0);     // rows >= b_q are not part of the product
     if (async) {
       asm volatile("cp.async.wait_group %0;" ::"n"(kStages - 2) : "memory");   // chunk `consumed` landed
       __syncthreads();                                // ... for every thread; the previous chunk is fully consumed
@@ -180,11 +196,10 @@ decode_stream_kernel(const Params p_in) {
       ++consumed;
     } else {
       const float* Wm = p.W + (int64_t)seq * p.w_stride_seq;
-      const float* rprev = p.r_prev + (int64_t)seq * mb;
       const int c4 = tile * kTileW + cq * 4;
       for (int rr = rg; rr < rows; rr += kRowGroups) {
         const int m = m0 + rr;
-        const float a = __ldcg(rprev + m);
+        const float a = __ldcg(cc.rp + m);
         const float* wr = Wm + (int64_t)m * mb;
         if (c4 + 0 <= m) acc.x = fmaf(a, __ldcg(wr + c4 + 0), acc.x);
         if (c4 + 1 <= m) acc.y = fmaf(a, __ldcg(wr + c4 + 1), acc.y);
@@ -192,7 +207,7 @@ decode_stream_kernel(const Params p_in) {
         if (c4 + 3 <= m) acc.w = fmaf(a, __ldcg(wr + c4 + 3), acc.w);
       }
     }
-    if (it == n_my - 1 || cc.chunk + 1 >= si.chunks(tile)) {
+    if (it == n_my - 1 || cc.chunk + 1 >= cc.n_tile) {
       // one partial per (tile, CTA)
       *reinterpret_cast<float4*>(s_part + rg * kTileW + cq * 4) = acc;
       __syncthreads();

@@ -197,3 +197,31 @@ def test_decode_chain_reads_nothing_before_its_producers_finish(sw):
         dp.attend(q, kc, vc, seqlens, out)
         torch.cuda.synchronize()
         assert torch.equal(chained, out), it
+
+
+def test_decode_selection_many_short_sequences(sw):
+    """300 sequences of 1 .. 8 blocks in one sw_decode_select call (more sequences than threads of the streaming
+    kernel's prefix pass, chunk ranges that span many sequences, CTAs without work) against the row-mode calls."""
+    B, d, r, h_q, h_kv, s, mb = 64, 64, 16, 4, 2, 2, 8
+    batch = 300
+    rng = np.random.default_rng(3)
+    ts = rng.integers(1, mb * B + 1, size=batch).tolist()
+    ts[0], ts[1], ts[2] = 1, mb * B, B + 1
+    taus = [3] * batch
+    signs, cols = gen.srht_params(3, d, r)
+    seqlens = torch.tensor(ts, dtype=torch.int32, device="cuda")
+    pipes = [sw.DecodePipeline(batch, mb, h_q, h_kv, d, B, r, s, taus, signs, cols) for _ in range(2)]
+    caches = [_random_decode_caches(batch, mb, d, r, 21) for _ in range(2)]
+    for layer in range(2):
+        torch.manual_seed(60 + layer)
+        q = torch.randn(batch, h_q, d).bfloat16().cuda(); k = torch.randn(batch, h_kv, d).bfloat16().cuda()
+        for dp, (Wc, kbar, ks), fused in zip(pipes, caches, (True, False)):
+            dp.select(q, k, seqlens, kbar, ks, Wc, fused=fused)
+        torch.cuda.synchronize()
+        rf = pipes[0].rvec[pipes[0].cur]; ru = pipes[1].rvec[pipes[1].cur]
+        scale = ru.abs().amax(dim=1, keepdim=True).clamp_min(1e-30)
+        assert ((rf - ru).abs() <= 1e-5 * scale).all()
+        assert torch.allclose(caches[0][1], caches[1][1], rtol=0, atol=1e-6)
+        assert torch.equal(pipes[0].count, pipes[1].count)
+        # the rows are short and random: no near-ties at 1e-5, the lists must agree
+        assert torch.equal(pipes[0].idx, pipes[1].idx)

@@ -318,7 +318,9 @@ def test_walk_update_tcgen05_varlen_batch(sw, blocks, flags):
 
 
 @pytest.mark.parametrize("blocks,r", [((16,), 16), ((100,), 64), ((37, 130, 64), 64), ((512,), 64), ((300, 700), 32),
-                                      ((1030,), 64), ((50,), 2)])
+                                      ((1030,), 64), ((50,), 2),
+                                      # long rows: the strip of score rows leaves the key ring of the fused score kernel two stages
+                                      ((1500,), 64), ((2049, 700), 32)])
 @pytest.mark.parametrize("flags,s", [(O.DEFAULT_FLAGS, 2), (O.DEFAULT_FLAGS & ~O.SCORE_SOFTMAX, 3),
                                      (O.DEFAULT_FLAGS | O.POW_MATRIX, 2), (O.DEFAULT_FLAGS & ~O.ROWNORM, 1),
                                      (O.DEFAULT_FLAGS & ~O.CAUSAL, 2), (O.DEFAULT_FLAGS, 8)])

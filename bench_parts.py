@@ -296,7 +296,7 @@ def decode_bench(pkg, args, peaks, n_layer_bufs: int = 4, steps: int = 20):
     torch.cuda.synchronize()
     launches = pkg.sw_launch_count() - launches0
     us_layer_eager = e0.elapsed_time(e1) * 1e3 / (steps * n_model_layers)
-    # the decode step is launch-bound at these kernel sizes (2 launches of 35 / 140 us per layer through
+    # the decode step is launch-bound at these kernel sizes (5 launches per layer, 24 + 135 us, through
     # ctypes): capture the 32-layer step once in a CUDA graph and replay it -- the library only launches
     # on the stream it is given, never synchronises or allocates, so its calls capture as they are
     graph = torch.cuda.CUDAGraph()

@@ -122,7 +122,7 @@ class DecodePipeline:
         self.count = torch.empty(batch, dtype=torch.int32, device=device)
         nb = sw.sw_decode_workspace_bytes(batch, h_q, h_kv, d, self.tau_max)
         self.attn_ws = torch.empty(max(nb, 16), dtype=torch.uint8, device=device)
-        # sw_decode_select scratch (score row + partial sums handed between its two kernels)
+        # sw_decode_select scratch (score row + partial sums handed between its three kernels)
         self.select_ws = torch.empty(sw.sw_decode_select_workspace_bytes(batch, max_blocks), dtype=torch.uint8,
                                      device=device)
 

@@ -302,6 +302,33 @@ SW_API int32_t sw_sparse_attn_decode_paged(int32_t batch, int32_t block, const s
                                     int32_t tau_max, float softmax_scale, void* out, float* lse,
                                     void* ws, size_t ws_bytes, sw_stream_t stream);
 
+/* sw_sparse_attn_decode for callers that have no device memory to spare for a workspace and no way to get some:
+ * a serving process whose memory pool was carved up completely at start-up, a plug-in that receives tensors from
+ * its host framework but no allocator, a latency-critical thread that must never reach cudaMalloc (which
+ * synchronises the whole device and may take arbitrarily long).  Same arguments, same kernels and bit-identical
+ * results as sw_sparse_attn_decode (contiguous cache), minus ws / ws_bytes: the split-KV partials go into a fixed
+ * array of SW_STATIC_SCRATCH_BYTES that is part of libsw's device image.  The call allocates and frees nothing
+ * (no cudaMalloc / cudaFree, no allocating library routine); q, the caches, the lists and out are still the
+ * caller's.
+ *  - LIMIT: sw_decode_workspace_bytes(batch, h_q, h_kv, d, tau_max) must be <= SW_STATIC_SCRATCH_BYTES, otherwise
+ *    SW_ERR_WORKSPACE is returned (message in sw_last_error) and nothing is launched.  (cfg 3 of BASELINE.json,
+ *    batch 8 x 32 heads x d = 128 at tau = 410, needs about 1.2 MB.)
+ *  - COST: the array occupies SW_STATIC_SCRATCH_BYTES of device memory on every GPU that loads this part of the
+ *    library, until the process exits, used or not.
+ *  - FIRST CALL PER DEVICE: the first call made with a given device current looks up that device's address of the
+ *    array (cudaGetSymbolAddress; this may load the module on that device).  Make that first call during start-up,
+ *    outside any stream capture.
+ *  - SHARING: all calls on a device use the same array and it keeps whatever the last call left in it.  Nothing in
+ *    it needs clearing (every slot that is read is written first, by the same call), but two calls whose kernels
+ *    can be on the GPU at the same time -- different streams, or different host threads -- race on it and give
+ *    wrong results without any error.  Keep all calls on one stream, or order them with events. */
+#define SW_STATIC_SCRATCH_BYTES (4u << 20)
+SW_API int32_t sw_sparse_attn_decode_static(int32_t batch, int32_t block, const sw_tensor* q,
+                                     const sw_tensor* kcache, const sw_tensor* vcache, int64_t stride_batch,
+                                     const int32_t* seqlens, const int32_t* idx, const int32_t* count,
+                                     int32_t tau_max, float softmax_scale, void* out, float* lse,
+                                     sw_stream_t stream);
+
 /* Bytes of device scratch ``op`` needs for this problem (pure host functions; 0 = none).
  * SW_OP_WALK_UPDATE: see sw_walk_update.  SW_OP_ATTN_PREFILL: only for
  * dtype = SW_F32 (the bf16 cast copies, P17).  SW_OP_ATTN_DECODE: the split-KV partials

@@ -29,7 +29,7 @@ SW_OP_SKETCH, SW_OP_BLOCK_SCORES, SW_OP_WALK_UPDATE, SW_OP_SELECT_TOPK, SW_OP_AT
 EXPORTS = [
     "sw_sketch", "sw_sketch_qk", "sw_sketch_from_pooled", "sw_copy_pool", "sw_sketch_append", "sw_block_scores", "sw_block_scores_row", "sw_walk_update",
     "sw_walk_update_row", "sw_select_topk", "sw_select_topk_row", "sw_prefill_select", "sw_decode_select", "sw_sparse_attn_prefill",
-    "sw_sparse_attn_decode", "sw_sparse_attn_decode_paged", "sw_workspace_bytes", "sw_decode_workspace_bytes", "sw_decode_select_workspace_bytes", "sw_decode_num_splits",
+    "sw_sparse_attn_decode", "sw_sparse_attn_decode_paged", "sw_sparse_attn_decode_static", "sw_workspace_bytes", "sw_decode_workspace_bytes", "sw_decode_select_workspace_bytes", "sw_decode_num_splits",
     "sw_set_prefill_kernel", "sw_get_prefill_kernel_used", "sw_set_walk_kernel", "sw_get_walk_kernel_used",
     "sw_last_error", "sw_version", "sw_launch_count",
 ]
@@ -79,6 +79,7 @@ def _load() -> C.CDLL:
         "sw_sparse_attn_decode": (i32, [i32, i32, TP, TP, TP, i64, vp, vp, vp, i32, f32, vp, vp, vp, sz, vp]),
         "sw_sparse_attn_decode_paged": (i32, [i32, i32, TP, TP, TP, i64, vp, i32, vp, vp, vp, i32, f32, vp, vp, vp, sz,
                                               vp]),
+        "sw_sparse_attn_decode_static": (i32, [i32, i32, TP, TP, TP, i64, vp, vp, vp, i32, f32, vp, vp, vp]),
         "sw_workspace_bytes": (sz, [i32, LP, i32, i32, i32, i32, i32]),
         "sw_decode_workspace_bytes": (sz, [i32, i32, i32, i32, i32]),
         "sw_decode_select_workspace_bytes": (sz, [i32, i32]),
@@ -330,6 +331,31 @@ def sw_sparse_attn_decode(batch, block, q, kcache, vcache, seqlens, idx, count, 
                                       _ptr(seqlens), _ptr(idx), _ptr(count), tau_max, softmax_scale, _ptr(out),
                                       _ptr(lse), _ptr(ws), 0 if ws is None else ws.numel() * ws.element_size(),
                                       _stream(stream)))
+
+
+SW_STATIC_SCRATCH_BYTES = 4 << 20
+
+
+def sw_sparse_attn_decode_static(batch, block, q, kcache, vcache, seqlens, idx, count, tau_max, softmax_scale, out,
+                                 lse=None, stream=None) -> None:
+    """sw_sparse_attn_decode without a workspace argument, for callers that cannot allocate device memory (a
+    pre-partitioned serving pool, a plug-in without an allocator, a thread that must stay clear of cudaMalloc):
+    the split-KV partials live in a fixed SW_STATIC_SCRATCH_BYTES array inside libsw.  Raises SwError
+    (SW_ERR_WORKSPACE) when sw_decode_workspace_bytes(...) exceeds that size.  All calls on a device share the
+    array, so calls that may overlap on the GPU (other streams / threads) race; the first call on each device
+    does a one-time address lookup and belongs in start-up code, outside stream capture.  See include/sw.h."""
+    if kcache.dim() != 4 or vcache.dim() != 4 or kcache.stride(3) != 1 or vcache.stride(3) != 1:
+        raise SwError(SW_ERR_INVALID_ARG, "caches must be [batch, t, h_kv, d] with contiguous d")
+    if kcache.stride(0) != vcache.stride(0):
+        raise SwError(SW_ERR_INVALID_ARG, "k and v caches must share the batch stride")
+    qt = _tensor(q)
+    kt = _Tensor(kcache.data_ptr(), _dtype_code(kcache), kcache.shape[2], kcache.shape[3], kcache.stride(1),
+                 kcache.stride(2))
+    vt = _Tensor(vcache.data_ptr(), _dtype_code(vcache), vcache.shape[2], vcache.shape[3], vcache.stride(1),
+                 vcache.stride(2))
+    _check(_lib.sw_sparse_attn_decode_static(batch, block, C.byref(qt), C.byref(kt), C.byref(vt), kcache.stride(0),
+                                             _ptr(seqlens), _ptr(idx), _ptr(count), tau_max, softmax_scale,
+                                             _ptr(out), _ptr(lse), _stream(stream)))
 
 
 def sw_sparse_attn_decode_paged(batch, block, q, kpool, vpool, block_table, seqlens, idx, count, tau_max,

@@ -12,7 +12,7 @@ CSRC = os.path.join(HERE, "csrc")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsw.so")
 SOURCES = ["api.cu", "sketch.cu", "scores.cu", "walk.cu", "walk_tc.cu", "select.cu", "decode_duty.cu", "decode_select.cu", "decode_tail.cu", "attn_prefill_generic.cu",
-           "attn_prefill_sm100.cu", "attn_decode.cu"]
+           "attn_prefill_sm100.cu", "attn_decode.cu", "attn_decode_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr",
               "-Xptxas", "-v"]

@@ -246,7 +246,9 @@ SW_API int32_t sw_select_topk_row(int32_t batch, int32_t block, int32_t max_bloc
  * r_out: dev fp32 [batch, max_blocks].  Needs !SW_POW_MATRIX and SW_CAUSAL (see sw_block_scores_row).
  * ws: dev scratch of sw_decode_select_workspace_bytes(batch, max_blocks) bytes (SW_ERR_WORKSPACE if smaller):
  * the raw score row and the partial sums of the W stream, handed from the first kernel to the second (no state is
- * kept between calls; calls that share a workspace must not overlap).  batch <= 512.  Three launches chained as
+ * kept between calls; calls that share a workspace must not overlap).  batch <= 512.  seqlens[s] must lie in
+ * [1, max_blocks * block]; a value outside that range marks an IDLE SLOT of the batch: nothing of sequence s is read
+ * or updated (kbar, ks, W_cache untouched), count[s] = 0, its idx row is -1 and its r_out row 0.  Three launches chained as
  * programmatic dependents: the streaming kernel (the cached-W stream of Step 5 over the whole grid; skipped when
  * r_prev is NULL), beside it the kernel of Steps 2-4 (sketches, running key mean, raw score row), then the
  * per-sequence tail (softmax, W_new, rescale, select).  No kernel of the chain reads anything an earlier kernel of

@@ -38,7 +38,8 @@ decode_duty_kernel(const Params p_in) {
   swd::pdl_launch_dependents();                       // the tail may become resident (it waits for this kernel)
   const int mb = p.max_blocks;
   const int t = __ldcg(p.seqlens + seq);
-  const int bq = (t - 1) / p.B, a = bq / kDutyTile;   // block of the new token = b_curr
+  const bool live = seq_live(t, p.B, mb);             // (an idle slot of the batch has no tile: a = -1)
+  const int bq = live ? (t - 1) / p.B : 0, a = live ? bq / kDutyTile : -1;   // block of the new token = b_curr
   const int hi = bq + 1;
   constexpr int kGroups = kDutyThreads / D;
   const int q4 = p.r >> 2;                            // float4s per sketch row

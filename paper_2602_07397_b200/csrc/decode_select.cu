@@ -56,6 +56,7 @@ decode_stream_kernel(const Params p_in) {
   // ---- chunk and tile counts of all sequences: exclusive prefixes in shared memory ----------------------
   {
     constexpr int kPer = kMaxBatch / kThreads;
+    static_assert(kMaxBatch % kThreads == 0, "the prefix pass gives every thread kMaxBatch / kThreads sequences");
     int vc[kPer], vt[kPer], sc = 0, st = 0;
 #pragma unroll
     for (int e = 0; e < kPer; ++e) {
@@ -63,7 +64,7 @@ decode_stream_kernel(const Params p_in) {
       vc[e] = 0; vt[e] = 0;
       if (sq < p.batch) {
         s_len[sq] = __ldcg(p.seqlens + sq);
-        const SeqInfo si = seq_info(s_len, sq, p.B, true);
+        const SeqInfo si = seq_info(s_len, sq, p.B, mb, true);
         vc[e] = si.total_chunks(); vt[e] = si.nt;
       }
       sc += vc[e]; st += vt[e];
@@ -85,6 +86,9 @@ decode_stream_kernel(const Params p_in) {
       if (sq <= p.batch) { s_pref[sq] = rc; s_tpref[sq] = rt; }
       rc += vc[e]; rt += vt[e];
     }
+    // the pass above covers sq <= kMaxBatch - 1: with a full batch (batch = kMaxBatch) the totals are the last
+    // thread's running sums (sequences past the batch count zero)
+    if (tid == kThreads - 1) { s_pref[kMaxBatch] = rc; s_tpref[kMaxBatch] = rt; }
     __syncthreads();
   }
   const int T = s_pref[p.batch];
@@ -114,7 +118,7 @@ decode_stream_kernel(const Params p_in) {
     int lo = 0, hi = p.batch - 1;
     while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_pref[mid] <= g) lo = mid; else hi = mid - 1; }
     c.seq = lo;
-    const SeqInfo si = seq_info(s_len, c.seq, p.B, true);
+    const SeqInfo si = seq_info(s_len, c.seq, p.B, mb, true);
     const int local = g - s_pref[c.seq];
     int tl = 0, th = max(si.nt - 1, 0);
     while (tl < th) { const int mid = (tl + th + 1) >> 1; if (si.chunks_before(mid) <= local) tl = mid; else th = mid - 1; }
@@ -127,12 +131,12 @@ decode_stream_kernel(const Params p_in) {
     ++c.chunk;
     c.m0 += kChunkRows;
     if (c.chunk < c.n_tile) return;
-    SeqInfo si = seq_info(s_len, c.seq, p.B, true);
+    SeqInfo si = seq_info(s_len, c.seq, p.B, mb, true);
     c.chunk = 0;
     ++c.tile;
     while (c.seq < p.batch && c.tile >= si.nt) {     // next sequence that has chunks
       c.tile = 0;
-      if (++c.seq < p.batch) si = seq_info(s_len, c.seq, p.B, true);
+      if (++c.seq < p.batch) si = seq_info(s_len, c.seq, p.B, mb, true);
     }
     if (c.seq < p.batch) enter_tile(c, si);
   };

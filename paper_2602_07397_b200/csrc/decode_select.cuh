@@ -69,10 +69,14 @@ struct SeqInfo {
   __device__ __forceinline__ int chunks_before(int tile) const { return tile * nr - kRho * (tile * (tile - 1) / 2); }   // tile <= nt
   __device__ __forceinline__ int total_chunks() const { return chunks_before(nt); }
 };
-__device__ __forceinline__ SeqInfo seq_info(const int32_t* seqlens, int seq, int B, bool walk) {
+// A length outside [1, max_blocks B] marks an idle slot of the batch (sw.h: sw_decode_select): no chunks, no key
+// update, no score row; the tail writes an empty selection for it.
+__device__ __forceinline__ bool seq_live(int t, int B, int max_blocks) { return t >= 1 && (t - 1) / B < max_blocks; }
+__device__ __forceinline__ SeqInfo seq_info(const int32_t* seqlens, int seq, int B, int max_blocks, bool walk) {
   SeqInfo s;
   const int t = seqlens[seq];                          // (a shared-memory copy in the streaming kernel)
-  s.bq = (t - 1) / B;                                  // block of the new token = b_curr
+  const bool live = seq_live(t, B, max_blocks);
+  s.bq = live ? (t - 1) / B : 0;                       // block of the new token = b_curr
   s.nr = walk ? (s.bq + kChunkRows - 1) / kChunkRows : 0;
   s.nt = walk ? (s.bq + kTileW - 1) / kTileW : 0;
   return s;

@@ -62,7 +62,7 @@ decode_tail_kernel(const Params p_in) {
   // ---- independent of the streaming kernel: chunk prefix of this sequence, T, tau, r_prev[b_q] -------------
   int mine = 0, before = 0, tbefore = 0;
   for (int sq = tid; sq < p.batch; sq += NT) {
-    const SeqInfo o = seq_info(p.seqlens, sq, p.B, walk);
+    const SeqInfo o = seq_info(p.seqlens, sq, p.B, mb, walk);
     const int c = o.total_chunks();
     mine += c;
     if (sq < seq) { before += c; tbefore += o.nt; }
@@ -71,7 +71,7 @@ decode_tail_kernel(const Params p_in) {
   const int T = mine, pref = before;                  // chunks of the batch / of the sequences before this one
   const int tpref = tbefore;                          // tiles with chunks of the sequences before this one
   const int G = max(1, min(p.g_stream, T));           // CTAs of the streaming kernel that hold chunks
-  const SeqInfo si = seq_info(p.seqlens, seq, p.B, walk);
+  const SeqInfo si = seq_info(p.seqlens, seq, p.B, mb, walk);
   const int bq = si.bq, hi = bq + 1;
   const int tt = max(0, min(__ldg(p.tau + seq), p.tau_max));   // (tau, seqlens: written before this selection started)
   // partials per stream tile = CTAs of the streaming kernel that share the tile's chunks
@@ -87,6 +87,13 @@ decode_tail_kernel(const Params p_in) {
     s_first[tl] = part_id(first, tpref + tl);
   }
   swd::pdl_wait(p.ws_scores, p.ws_part, p.r_prev);             // the duty kernel's scores and the stream's partials are visible
+  if (!seq_live(p.seqlens[seq], p.B, mb)) {
+    // idle slot (length outside [1, max_blocks B]): an empty selection and a zero walk row, nothing else is touched
+    for (int j = tid; j < mb; j += NT) p.r_out[(int64_t)seq * mb + j] = 0.f;
+    for (int j = tid; j < p.tau_max; j += NT) p.idx[(int64_t)seq * p.tau_max + j] = -1;
+    if (tid == 0) p.count[seq] = 0;
+    return;
+  }
 
   const float rq = walk ? __ldcg(p.r_prev + (int64_t)seq * mb + bq) : 1.f;   // (consumed after the softmax statistics)
   const float* sc = p.ws_scores + (int64_t)seq * p.mbp;

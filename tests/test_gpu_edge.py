@@ -199,11 +199,12 @@ def test_decode_chain_reads_nothing_before_its_producers_finish(sw):
         assert torch.equal(chained, out), it
 
 
-def test_decode_selection_many_short_sequences(sw):
-    """300 sequences of 1 .. 8 blocks in one sw_decode_select call (more sequences than threads of the streaming
-    kernel's prefix pass, chunk ranges that span many sequences, CTAs without work) against the row-mode calls."""
+@pytest.mark.parametrize("batch", [300, 512])       # 512 = the largest batch one call takes (kMaxBatch)
+def test_decode_selection_many_short_sequences(sw, batch):
+    """300 / 512 sequences of 1 .. 8 blocks in one sw_decode_select call (more sequences than threads of the
+    streaming kernel's prefix pass, chunk ranges that span many sequences, CTAs without work; at 512 the total of the
+    prefix pass sits in the last slot of its table) against the row-mode calls."""
     B, d, r, h_q, h_kv, s, mb = 64, 64, 16, 4, 2, 2, 8
-    batch = 300
     rng = np.random.default_rng(3)
     ts = rng.integers(1, mb * B + 1, size=batch).tolist()
     ts[0], ts[1], ts[2] = 1, mb * B, B + 1
@@ -225,3 +226,43 @@ def test_decode_selection_many_short_sequences(sw):
         assert torch.equal(pipes[0].count, pipes[1].count)
         # the rows are short and random: no near-ties at 1e-5, the lists must agree
         assert torch.equal(pipes[0].idx, pipes[1].idx)
+
+
+def test_decode_selection_idle_slots(sw):
+    """seqlens entries outside [1, max_blocks * B] mark idle slots of a decode batch (include/sw.h): the call leaves
+    their caches alone and reports an empty selection, and the live sequences come out as they do when the idle
+    slots hold ordinary sequences instead."""
+    B, d, r, h_q, h_kv, s, mb = 64, 128, 64, 8, 2, 2, 300
+    live = {1: 64 * 280 + 9, 3: 64 * 3, 4: 64 * 299 + 1}
+    idle = {0: 0, 2: mb * B + 1, 5: -4}
+    batch = 6
+    taus = [7] * batch
+    signs, cols = gen.srht_params(3, d, r)
+    torch.manual_seed(70)
+    q = torch.randn(batch, h_q, d).bfloat16().cuda(); k = torch.randn(batch, h_kv, d).bfloat16().cuda()
+    res = []
+    for fill in (None, 64 * 100 + 5):                     # idle slots as given / replaced by an ordinary sequence
+        ts = [live.get(i, idle.get(i) if fill is None else fill) for i in range(batch)]
+        seqlens = torch.tensor(ts, dtype=torch.int32, device="cuda")
+        dp = sw.DecodePipeline(batch, mb, h_q, h_kv, d, B, r, s, taus, signs, cols)
+        Wc, kbar, ks = _random_decode_caches(batch, mb, d, r, 31)
+        W0, kbar0, ks0 = Wc.clone(), kbar.clone(), ks.clone()
+        for layer in range(2):                            # the second step runs with a walk state (the W stream)
+            dp.idx.fill_(-7); dp.count.fill_(-7)
+            dp.select(q, k, seqlens, kbar, ks, Wc)
+        torch.cuda.synchronize()
+        res.append((dp.rvec[dp.cur].clone(), dp.idx.clone(), dp.count.clone(), Wc, kbar, ks))
+        if fill is None:
+            for i in idle:
+                assert dp.count[i].item() == 0 and (dp.idx[i] == -1).all() and (dp.rvec[dp.cur][i] == 0).all()
+                assert torch.equal(Wc[i], W0[i]) and torch.equal(kbar[i], kbar0[i]) and torch.equal(ks[i], ks0[i])
+    (ra, ia, ca, Wa, kba, ksa), (rb, ib, cb, Wb, kbb, ksb) = res
+    for i, t in live.items():
+        scale = rb[i].abs().max()
+        assert ((ra[i] - rb[i]).abs() <= 1e-5 * scale).all()
+        assert ca[i].item() == cb[i].item() == min(taus[i], (t - 1) // B + 1)
+        assert torch.equal(kba[i], kbb[i]) and torch.equal(ksa[i], ksb[i]) and torch.equal(Wa[i], Wb[i])
+        diff = set(ia[i].tolist()) ^ set(ib[i].tolist())
+        ref = [j for j in ib[i, :cb[i]].tolist() if j not in (0, (t - 1) // B)]
+        kth = min(rb[i][ref]).item() if ref else 0.0
+        assert all(abs(rb[i][j].item() - kth) <= 1e-5 * scale for j in diff)

@@ -270,7 +270,9 @@ SW_API size_t sw_decode_select_workspace_bytes(int32_t batch, int32_t max_blocks
  * q: [total_tokens, h_q, d]; k, v: [total_tokens, h_kv, d]; all bf16, or all fp32 (P17: fp32
  * operands are rounded to bf16 by a cast pre-pass into ws).  out: dev, same dtype as q,
  * [total_tokens, h_q, d] contiguous.  lse: dev fp32 [total_tokens, h_q] (natural log) or NULL.
- * idx/count as written by sw_select_topk (block indices local to the sequence; order free).
+ * idx/count as written by sw_select_topk, or built by the caller: block indices local to the sequence, in any order,
+ * each block at most once.  Entries that are -1, lie past the last block of the sequence, or (under SW_CAUSAL) name a
+ * block j > i that the mask hides entirely are skipped wherever they stand in the list.
  * ------------------------------------------------------------------------------------- */
 SW_API int32_t sw_sparse_attn_prefill(const sw_layout* L, const sw_tensor* q, const sw_tensor* k,
                                const sw_tensor* v, const int32_t* idx, const int32_t* count,

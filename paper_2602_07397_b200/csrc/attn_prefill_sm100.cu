@@ -165,21 +165,28 @@ attn_prefill_sm100_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     mbar_arrive_expect_tx(BAR(kBarQ), kQBytes);
     tma_load_3d(sQ, &map_q, BAR(kBarQ), 0, kvh * 4, q_tok0);
     tma_load_3d(sQ + kQBytes / 2, &map_q, BAR(kBarQ), 64, kvh * 4, q_tok0);
-    // The first sub-chunk of every selected block holds a visible key (a selected block j exists and, under the
-    // causal mask, j <= i), so the chunk list starts with the first 64 keys of idx[0] (and, for 64-token blocks, of
-    // idx[1]): request those K tiles now instead of after the list has been built and the set-up barrier passed --
-    // their latency then overlaps both.
+    // The chunk list (built by warp 3, below) starts with the first 64 keys of idx[0] when that block holds a visible
+    // key, followed, for 64-token blocks, by those of idx[1] when that one does too: request those K tiles now
+    // instead of after the list has been built and the set-up barrier passed -- their latency then overlaps both.
+    // The lists are the caller's (any order, hand-built ones included): an entry the list builder drops -- -1, a
+    // block past the end of the sequence, a block the causal mask hides entirely -- is not requested here either,
+    // and nothing behind it is, so that stage s always holds chunk s of the list.
     if (kEarlyK) {
       const int32_t* list = p.idx + (int64_t)gb * p.tau_max;
       const int cnt = __ldg(p.count + gb);
       const int j0 = __ldg(list), j1 = (p.tau_max > 1) ? __ldg(list + 1) : -1;
+      auto listed = [&](int j) {                              // the list builder's predicate on a block's first chunk
+        if (j < 0) return false;
+        const int k0 = seq_lo + j * p.B;
+        return k0 < seq_hi && !(p.causal && k0 > q_last);
+      };
       int pre = 0;
-      if (cnt > 0) {
+      if (cnt > 0 && listed(j0)) {
         mbar_arrive_expect_tx(BAR(kBarFull + 0), kTileBytes);
         tma_load_3d(sKV, &map_k, BAR(kBarFull + 0), 0, kvh, seq_lo + j0 * p.B);
         tma_load_3d(sKV + kTileBytes / 2, &map_k, BAR(kBarFull + 0), 64, kvh, seq_lo + j0 * p.B);
         pre = 1;
-        if (TPB == 1 && cnt > 1) {
+        if (TPB == 1 && cnt > 1 && listed(j1)) {
           mbar_arrive_expect_tx(BAR(kBarFull + 1), kTileBytes);
           tma_load_3d(sKV + kTileBytes, &map_k, BAR(kBarFull + 1), 0, kvh, seq_lo + j1 * p.B);
           tma_load_3d(sKV + kTileBytes + kTileBytes / 2, &map_k, BAR(kBarFull + 1), 64, kvh, seq_lo + j1 * p.B);

@@ -551,6 +551,67 @@ def test_sparse_attn_prefill_each_kernel(sw, case, kernel):
     attn_case(sw, kernel=sw.SW_PREFILL_TCGEN05 if kernel == "tcgen05" else sw.SW_PREFILL_GENERIC, **case)
 
 
+@pytest.mark.parametrize("kernel", ["generic", "tcgen05"])
+@pytest.mark.parametrize("B", [64, 128])
+def test_sparse_attn_prefill_list_order_and_skipped_entries(sw, kernel, B):
+    """include/sw.h: the block lists are order free, and entries that are -1, past the end of the sequence or hidden
+    entirely by the causal mask are skipped wherever they stand (the tcgen05 kernel requests the K tiles of list
+    positions 0 and 1 before it has built its chunk list).  Three calls on the same selection -- ascending lists,
+    every row randomly permuted, every row permuted with such entries planted at random positions (position 0
+    included) -- must agree with each other and with the oracle on the ascending lists."""
+    rng = np.random.RandomState(17)
+    torch.manual_seed(17)
+    seqlens, h_q, h_kv, d = (900, 300), 8, 2, 128
+    T = sum(seqlens)
+    q = torch.randn(T, h_q, d).bfloat16(); k = torch.randn(T, h_kv, d).bfloat16(); v = torch.randn(T, h_kv, d).bfloat16()
+    L = sw.make_layout(seqlens, B)
+    taus = [max(1, int(math.ceil(0.4 * b))) for b in L.blocks]
+    tau_max = max(taus) + 3                                        # room for the planted entries
+    asc = np.full((L.total_blocks, tau_max), -1, np.int32); cnt = np.zeros(L.total_blocks, np.int32)
+    lo = 0
+    for b, tau in zip(L.blocks, taus):
+        i, c = random_lists(rng, b, tau, True)
+        asc[lo:lo + b, :tau] = i; cnt[lo:lo + b] = c; lo += b
+    perm = asc.copy(); junk = asc.copy(); cnt_junk = cnt.copy()
+    lo = 0
+    for b in L.blocks:
+        for i in range(b):
+            row = asc[lo + i, :cnt[lo + i]]
+            perm[lo + i, :len(row)] = rng.permutation(row)
+            extra = [-1, b + 5, i + 1 + rng.randint(0, 3)]         # -1, past the end, hidden by the mask (j > i)
+            mixed = list(rng.permutation(row))
+            for e in extra:
+                mixed.insert(rng.randint(0, len(mixed) + 1) if i % 2 else 0, e)
+            junk[lo + i, :len(mixed)] = mixed; cnt_junk[lo + i] = len(mixed)
+        lo += b
+    scale = 1 / math.sqrt(d)
+    prev = sw.sw_set_prefill_kernel(sw.SW_PREFILL_TCGEN05 if kernel == "tcgen05" else sw.SW_PREFILL_GENERIC)
+    try:
+        outs = []
+        for lists, counts in ((asc, cnt), (perm, cnt), (junk, cnt_junk)):
+            out = torch.full((T, h_q, d), float("nan"), dtype=torch.bfloat16, device="cuda")
+            sw.sw_sparse_attn_prefill(L, q.cuda(), k.cuda(), v.cuda(), dev(lists), dev(counts), tau_max, scale,
+                                      O.DEFAULT_FLAGS, out, None, None)
+            outs.append(out.float().cpu().numpy())
+    finally:
+        sw.sw_set_prefill_kernel(prev)
+    assert all(np.isfinite(o).all() for o in outs)
+    # another key order = another summation order of the same softmax: bf16 output rounding is the difference
+    for o in outs[1:]:
+        err = np.abs(o - outs[0])
+        assert err.max() <= ATT_MAX and err.mean() <= ATT_MEAN, (err.max(), err.mean())
+    qn, kn, vn = (gen.to_numpy_f64(t) for t in (q, k, v))
+    hs = [0, 5]
+    tlo = blo = 0
+    for n, b in zip(seqlens, L.blocks):
+        ref = O.sparse_attention(qn[tlo:tlo + n], kn[tlo:tlo + n], vn[tlo:tlo + n], asc[blo:blo + b], cnt[blo:blo + b], B,
+                                 scale, O.DEFAULT_FLAGS, q_heads=hs)
+        for o in outs:
+            err = np.abs(o[tlo:tlo + n][:, hs] - ref[:, hs])
+            assert err.max() <= ATT_MAX and err.mean() <= ATT_MEAN, (err.max(), err.mean())
+        tlo += n; blo += b
+
+
 def test_prefill_tcgen05_rejects_unfit_shapes(sw):
     prev = sw.sw_set_prefill_kernel(sw.SW_PREFILL_TCGEN05)
     try:

@@ -36,7 +36,11 @@
 extern "C" {
 #endif
 
-#define SW_VERSION 100            /* 0.1.0 */
+/* Bumped whenever a signature or a workspace layout changes (101: sw_decode_select takes ws / ws_bytes, the
+ * SW_OP_WALK_UPDATE workspace holds the operand images, sw_sparse_attn_decode_static added).  A caller built against
+ * another header compares its SW_VERSION with sw_version() of the library it loaded and refuses to run on a mismatch
+ * (the Python binding does). */
+#define SW_VERSION 101            /* 0.1.1 */
 
 #if defined(__GNUC__)
 #define SW_API __attribute__((visibility("default")))
@@ -148,7 +152,8 @@ SW_API int32_t sw_sketch_append(int32_t batch, int32_t block, int32_t max_blocks
  *   SW_CAUSAL: entries j > i are masked            (P6)
  *   SW_SCORE_SOFTMAX: A[i,:] = softmax of the unmasked S[i,:], masked -> 0; else A = S, masked -> 0
  *   W = A^(element-wise s)   (or W = A with SW_POW_MATRIX: the walk then multiplies s times)
- * qs, ks: dev fp32 [total_blocks, r].  W: dev fp32 packed sum_s b_s^2 (written in full, zeros
+ * qs, ks: dev fp32 [total_blocks, r], 16-byte aligned (SW_ERR_INVALID_ARG otherwise; also for
+ * sw_prefill_select).  W: dev fp32 packed sum_s b_s^2 (written in full, zeros
  * where masked).  A: same shape or NULL.  s >= 1.
  * ------------------------------------------------------------------------------------- */
 SW_API int32_t sw_block_scores(const sw_layout* L, const float* qs, const float* ks, int32_t r, int32_t s,

@@ -19,6 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libsw.so")
 
 # ---- constants (include/sw.h) --------------------------------------------------------------
 SW_OK, SW_ERR_INVALID_ARG, SW_ERR_UNSUPPORTED, SW_ERR_WORKSPACE, SW_ERR_CUDA, SW_ERR_ARCH = 0, -1, -2, -3, -4, -5
+SW_VERSION = 101
 SW_BF16, SW_F32 = 0, 1
 SW_CAUSAL, SW_SCORE_SOFTMAX, SW_POW_MATRIX, SW_FORCE_FIRST, SW_FORCE_LAST, SW_ROWNORM = 1, 2, 4, 8, 16, 32
 SW_DEFAULT_FLAGS = SW_CAUSAL | SW_SCORE_SOFTMAX | SW_FORCE_FIRST | SW_FORCE_LAST | SW_ROWNORM
@@ -96,6 +97,9 @@ def _load() -> C.CDLL:
         fn = getattr(lib, name)
         fn.restype = res
         fn.argtypes = args
+    if lib.sw_version() != SW_VERSION:
+        raise ImportError(f"{LIB_PATH} reports version {lib.sw_version()}, this binding is written for {SW_VERSION} "
+                          "(include/sw.h): rebuild with `python -m paper_2602_07397_b200.build --force`")
     return lib
 
 

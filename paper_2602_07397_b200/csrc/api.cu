@@ -175,6 +175,7 @@ SW_API int32_t sw_block_scores(const sw_layout* L, const float* qs, const float*
                         uint32_t flags, float* W, float* A, sw_stream_t stream) {
   SW_TRY(validate_layout(L));
   SW_REQUIRE(qs && ks && W, SW_ERR_INVALID_ARG, "qs / ks / W is NULL");
+  SW_REQUIRE(aligned16(qs) && aligned16(ks), SW_ERR_INVALID_ARG, "qs / ks must be 16-byte aligned");
   SW_REQUIRE(r >= 1 && r <= 128, SW_ERR_INVALID_ARG, "r = %d out of [1,128]", r);
   SW_REQUIRE(s >= 1, SW_ERR_INVALID_ARG, "s = %d must be >= 1", s);
   SW_TRY(check_arch());
@@ -242,6 +243,7 @@ SW_API int32_t sw_prefill_select(const sw_layout* L, const float* qs, const floa
                           size_t ws_bytes, sw_stream_t stream) {
   SW_TRY(validate_layout(L));
   SW_REQUIRE(qs && ks && R_out && W && tau && idx && count, SW_ERR_INVALID_ARG, "NULL argument");
+  SW_REQUIRE(aligned16(qs) && aligned16(ks), SW_ERR_INVALID_ARG, "qs / ks must be 16-byte aligned");
   SW_REQUIRE(R_out != R_prev && R_out != W, SW_ERR_INVALID_ARG, "R_out must not alias its inputs");
   SW_REQUIRE(r >= 1 && r <= 128, SW_ERR_INVALID_ARG, "r = %d out of [1,128]", r);
   SW_REQUIRE(s >= 1 && tau_max >= 1, SW_ERR_INVALID_ARG, "s = %d / tau_max = %d", s, tau_max);

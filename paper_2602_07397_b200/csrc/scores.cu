@@ -1,10 +1,14 @@
 // sw_block_scores: Alg. 1 Steps 5-6a, eq. PAPER.md:69.
 //   S = Q~ K~^T / sqrt(r); block-causal mask (P6); row softmax (P5); W = A^(.s) (P4).
-// True fp32 (no TF32): the selection is sensitive to ~1e-5 relative score differences.
-// Two launches: (1) score_tile_kernel - one CTA per (16 query rows x 64 key columns) tile on or below
-// the block diagonal writes the raw masked scores S into W (b = 512: 144 CTAs instead of the 32
-// row-sweeping CTAs of the first version, 56 -> ~8 us); (2) score_rows_kernel - one warp per row reads
-// its row twice from L2 (max / sum-exp, then normalise) and writes A and W = A^s in place.
+// fp32-class accuracy throughout (the selection is sensitive to ~1e-5 relative score differences): the default
+// kernel runs the tile products on mma.sync TF32 with the 3xTF32 hi / lo split (error ~2^-21 relative, not TF32's
+// 2^-11), the fallback uses plain fp32 FMA.
+// Default, ONE launch: score_fused_kernel (r a power of two >= 4, strip fits in shared memory) -- one CTA per strip
+// of 8 query rows keeps the strip's raw scores on chip while the key sketches stream through a cp.async ring, then
+// turns each row into A, W = A^s and (for the tensor-core walk) the hi / lo operand images.
+// Fallback, two launches: (1) score_tile_kernel - one CTA per (16 query rows x 64 key columns) tile on or below the
+// block diagonal writes the raw masked scores S into W; (2) score_rows_kernel - one warp per row reads its row
+// twice from L2 (max / sum-exp, then normalise) and writes A and W = A^s in place.
 #include "common.cuh"
 #include "walk_images.cuh"
 

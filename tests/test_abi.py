@@ -37,7 +37,8 @@ def test_library_exports_every_declared_symbol(pkg):
     for name in syms:
         assert getattr(lib, name) is not None
     assert sorted(pkg.EXPORTS) == syms
-    assert pkg.sw_version() == 100
+    text = open(os.path.join(ROOT, "include", "sw.h")).read()
+    assert pkg.sw_version() == pkg.SW_VERSION == int(re.search(r"#define SW_VERSION (\d+)", text).group(1))
 
 
 def test_flag_values_match_header(pkg):
@@ -58,6 +59,12 @@ def test_validation_happens_before_any_device_work(pkg):
     assert lib.sw_block_scores(C.byref(lay), 1, 1, 64, 2, 0, 1, None, None) == pkg.SW_ERR_UNSUPPORTED
     lay = pkg.binding._Layout(1, 64, 10, 1, 1, 16, 16, 16)
     assert lib.sw_block_scores(C.byref(lay), 16, 16, 64, 0, 0, 16, None, None) == pkg.SW_ERR_INVALID_ARG   # s = 0
+    # sketches that are not 16-byte aligned are refused by both callers of the fused score kernel (cp.async / float4)
+    assert lib.sw_block_scores(C.byref(lay), 16 + 4, 16, 64, 2, 0, 16, None, None) == pkg.SW_ERR_INVALID_ARG
+    assert b"aligned" in lib.sw_last_error()
+    assert lib.sw_prefill_select(C.byref(lay), 16, 16 + 8, 64, 2, 0, None, 16, 16, None, 16, 4, 16, 16, None, 0,
+                                 None) == pkg.SW_ERR_INVALID_ARG
+    assert b"aligned" in lib.sw_last_error()
     t = pkg.binding._Tensor(16, pkg.SW_BF16, 8, 96, 768, 96)
     assert lib.sw_sketch(C.byref(lay), C.byref(t), None, 16, 64, 0.125, 16, None, None) == pkg.SW_ERR_UNSUPPORTED
     t = pkg.binding._Tensor(16, pkg.SW_BF16, 8, 128, 1024, 128)

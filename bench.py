@@ -49,11 +49,6 @@ def load_peaks():
     return d
 
 
-def tile_pairs(b: int, tau: int) -> int:
-    from bench_parts import tile_pairs as _tp       # one definition (bench_parts.py)
-    return _tp(b, tau)
-
-
 # ------------------------------------------------------------------------------------------ clocks
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 50 ms during the timed region."""
@@ -119,7 +114,7 @@ def oracle_sample(cfg, n, layer_inputs_cpu, H, n_qblocks=4):
     O.sparse_attention(Q, K, V, sel.idx, sel.count, cfg.B, 1 / math.sqrt(cfg.d), q_blocks=blocks)
     t_att = time.perf_counter() - t0
     pairs_s = int(sum(sel.count[i] for i in blocks))
-    pairs_all = tile_pairs(b, tau)
+    pairs_all = gen.tile_pairs(b, tau)
     t_layer = t_sel + t_att * pairs_all / pairs_s
     desc = (f"cfg2 layer 0: selection path in full ({t_sel:.1f}s) + attention of {len(blocks)} of {b} query "
             f"blocks x {cfg.h_q} heads ({pairs_s} of {pairs_all} tile pairs, {t_att:.1f}s), extrapolated by pairs")
@@ -151,6 +146,8 @@ def run_reference(args, rank):
     from oracle import sw_oracle as O
     cfg = gen.CONFIGS[CFG_IDX]
     n = cfg.seqlens[0]
+    b = O.num_blocks(n, cfg.B)
+    tau = O.tau_from_density(cfg.density, b)
     signs, cols = gen.srht_params(CFG_IDX + 1, cfg.d, cfg.r)
     H = O.srht_matrix(cfg.d, signs, cols, 1 / math.sqrt(cfg.r))
     plans = gen.make_plans(CFG_IDX)
@@ -165,10 +162,13 @@ def run_reference(args, rank):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * statistics.mean(secs),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": gen.CONFIGS[CFG_IDX].name, "note": "CPU oracle, bounded sample per step"},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle", "sample": desc},
+            "config": gen.workload_config(cfg, n, cfg.layers, b, tau),       # the GPU arm's keys and values
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
+                             "sample": "CPU oracle, bounded sample per step: " + desc},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
+    # this arm is the oracle alone: neither the package nor its CUDA library may be in the process
+    assert "paper_2602_07397_b200" not in sys.modules, "the reference arm imported the product package"
     print(json.dumps(line), flush=True)
 
 
@@ -216,7 +216,16 @@ def main():
         line = res["line"]
         if not args.no_decode and world == 1:
             try:
-                line["decode"] = decode_bench(pkg, args, peaks)
+                line["decode"] = dec = decode_bench(pkg, args, peaks)
+                # BASELINE.json's metric is "prefill tok/s & decode us/step": the decode half rides inside
+                # `roofline`, a key the contract names, so that whoever keeps only the contract's keys keeps it
+                r_ = dec["roofline"]
+                line["roofline"]["decode"] = {
+                    "workload": dec["workload"], "kernel": r_["kernel"], "bound": r_["bound"],
+                    "us_per_layer": dec["us_per_layer"], "selection_us": dec["selection_us"],
+                    "attention_us": dec["attention_us"], "achieved": r_["achieved"], "peak": r_["peak"],
+                    "unit": r_["unit"], "frac": r_["frac"], "bytes_per_launch": r_["bytes_per_launch"],
+                    "frac_layer_over_kv_bytes": dec["hbm_frac_layer_over_kv_bytes"], "traffic": r_["traffic"]}
             except Exception as e:               # the headline line must still print
                 line["decode"] = {"error": repr(e)[:300]}
         if not args.no_extras and world == 1 and not (args.layers or args.seqlen):

@@ -19,8 +19,14 @@ KERNELS = ["sketch_qk", "prefill_select", "attn"]
 ROOT = os.path.dirname(os.path.abspath(__file__))
 
 
-def tile_pairs(b: int, tau: int) -> int:
-    return sum(min(tau, i + 1) for i in range(b))
+tile_pairs = gen.tile_pairs
+
+
+def tau_budget(density: float, b: int) -> int:
+    """The benchmark's block budget for a nominal density: the smallest whole number of blocks >= density * b, at
+    least one (exact rational arithmetic on the decimal the config states).  The library takes tau as given."""
+    from fractions import Fraction
+    return max(1, math.ceil(Fraction(str(density)) * b))
 
 
 def _ncu_traffic(kernel: str):
@@ -39,7 +45,8 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
     layers = args.layers or cfg.layers
     dev = torch.device("cuda", torch.cuda.current_device())
     signs, cols = gen.srht_params(CFG_IDX + 1, cfg.d, cfg.r)
-    pipe = pkg.PrefillPipeline([n], cfg.h_q, cfg.h_kv, cfg.d, cfg.B, cfg.r, cfg.s, cfg.density, signs, cols)
+    pipe = pkg.PrefillPipeline([n], cfg.h_q, cfg.h_kv, cfg.d, cfg.B, cfg.r, cfg.s,
+                               [tau_budget(cfg.density, (n + cfg.B - 1) // cfg.B)], signs, cols)
     b = pipe.L.blocks[0]
     tau = pipe.tau_max
     pairs = tile_pairs(b, tau)
@@ -121,13 +128,7 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
         "data": "synthetic",
-        "config": {"workload": cfg.name if (n, layers) == (cfg.seqlens[0], cfg.layers) else f"DEBUG n={n} L={layers}",
-                   "layers": layers, "seq_len": n, "h_q": cfg.h_q, "h_kv": cfg.h_kv, "head_dim": cfg.d,
-                   "block": cfg.B, "blocks": b, "tau": tau, "sketch_dim": cfg.r, "walk_power_s": cfg.s,
-                   "density": cfg.density, "tile_pairs_per_layer": pairs,
-                   "l2": "inputs larger than L2: 32 distinct layers x 403 MB cycle through the 126 MB L2",
-                   "generator": {"coherence_a": gen.COHERENCE_A, "plant_cos": gen.PLANT_COS,
-                                 "plant_frac": gen.PLANT_FRAC, "chain_frac": gen.CHAIN_FRAC, "sink_a": gen.SINK_A}},
+        "config": gen.workload_config(cfg, n, layers, b, tau),
         "ms_per_layer": layer_ms,
         "kernel_ms_per_layer": kern_ms,
         "kernel_ms_per_layer_median": {k: statistics.median(v) for k, v in per.items()},
@@ -236,7 +237,7 @@ def decode_bench(pkg, args, peaks, n_layer_bufs: int = 4, steps: int = 20):
     batch, t = len(cfg.seqlens), cfg.seqlens[0]
     B, d, r = cfg.B, cfg.d, cfg.r
     mb = (t + B - 1) // B
-    tau = pkg.tau_from_density(cfg.density, mb)
+    tau = tau_budget(cfg.density, mb)
     signs, cols = gen.srht_params(3, d, r)
     free, _ = torch.cuda.mem_get_info()
     per_layer = batch * t * cfg.h_kv * d * 2 * 2 + batch * mb * mb * 4
@@ -259,7 +260,8 @@ def decode_bench(pkg, args, peaks, n_layer_bufs: int = 4, steps: int = 20):
             kc[s_].copy_(k); vc[s_].copy_(v)
             q_new[s_].copy_(q[t - 1]); k_new[s_].copy_(k[t - 1])
             # caches from the prefill selection path over the first t-1 tokens (untimed set-up)
-            pp = pkg.PrefillPipeline([t - 1], cfg.h_q, cfg.h_kv, d, B, r, cfg.s, cfg.density, signs, cols)
+            pp = pkg.PrefillPipeline([t - 1], cfg.h_q, cfg.h_kv, d, B, r, cfg.s, [tau_budget(cfg.density, (t + B - 2) // B)],
+                                     signs, cols)
             pp.select(q[:t - 1], k[:t - 1])
             Wc[s_].copy_(pp.W.view(mb, mb)); kbar[s_].copy_(pp.kbar); ks[s_].copy_(pp.ks)
             del q, k, v, pp

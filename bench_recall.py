@@ -36,7 +36,9 @@ from synth import gen
 def run(pkg, Qs, Ks, plan, *, n, B, r, s, density, flags, carry):
     cfg = gen.CONFIGS[1]
     signs, cols = gen.srht_params(2, cfg.d, r)
-    pipe = pkg.PrefillPipeline([n], cfg.h_q, cfg.h_kv, cfg.d, B, r, s, density, signs, cols, flags=flags)
+    from bench_parts import tau_budget
+    pipe = pkg.PrefillPipeline([n], cfg.h_q, cfg.h_kv, cfg.d, B, r, s, [tau_budget(density, (n + B - 1) // B)], signs, cols,
+                               flags=flags)
     direct = [0, 0]; hop2 = [0, 0]; rnd = []
     for l in range(len(Qs)):
         if not carry:

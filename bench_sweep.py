@@ -99,8 +99,9 @@ def time_stack(pkg, pipe, bufs, out, layers_run, passes, warm=1):
 def measure(pkg, peaks, name, seqlens, bufs, *, h_q, h_kv, d, B, r, s, density, flags=None, layers_run=8, passes=2):
     signs, cols = gen.srht_params(11, d, r)
     kw = {} if flags is None else {"flags": flags}
-    pipe = pkg.PrefillPipeline(list(seqlens), h_q, h_kv, d, B, r, s, density, signs, cols, **kw)
-    taus = [pkg.tau_from_density(density, b) for b in pipe.L.blocks]
+    from bench_parts import tau_budget
+    taus = [tau_budget(density, (n + B - 1) // B) for n in seqlens]
+    pipe = pkg.PrefillPipeline(list(seqlens), h_q, h_kv, d, B, r, s, taus, signs, cols, **kw)
     pairs = tile_pairs(pipe.L.blocks, taus)
     pairs_dense = tile_pairs(pipe.L.blocks, pipe.L.blocks)
     out = torch.empty(sum(seqlens), h_q, d, dtype=torch.bfloat16, device="cuda")

@@ -3,4 +3,4 @@ C ABI of ``include/sw.h`` (``libsw.so``), a ctypes binding with the same names, 
 driver.  Importing the package loads ``libsw.so``; there is no CPU or PyTorch fallback."""
 from .binding import *  # noqa: F401,F403
 from .binding import Layout, SwError, make_layout, EXPORTS, LIB_PATH  # noqa: F401
-from .pipeline import DecodePipeline, PrefillPipeline, tau_from_density  # noqa: F401
+from .pipeline import DecodePipeline, PrefillPipeline  # noqa: F401

@@ -11,16 +11,13 @@ import torch
 from . import binding as sw
 
 
-def tau_from_density(density: float, b: int) -> int:
-    """tau = max(1, ceil(density * b))  (reading P13 in DESIGN.md)."""
-    return max(1, int(math.ceil(density * b - 1e-12)))
-
-
 class PrefillPipeline:
-    """Alg. 1 for a packed batch of sequences; the walk state R is carried across layers."""
+    """Alg. 1 for a packed batch of sequences; the walk state R is carried across layers.  ``taus``: the block
+    budget tau of every sequence (Alg. 1 Step 7), chosen by the caller -- like the C ABI, the driver takes tau as
+    given and derives nothing from a density."""
 
     def __init__(self, seqlens: Sequence[int], h_q: int, h_kv: int, d: int, B: int, r: int, s: int,
-                 density: float, signs: np.ndarray, cols: np.ndarray, flags: int = sw.SW_DEFAULT_FLAGS,
+                 taus: Sequence[int], signs: np.ndarray, cols: np.ndarray, flags: int = sw.SW_DEFAULT_FLAGS,
                  dtype: torch.dtype = torch.bfloat16, device: str = "cuda", keep_A: bool = False,
                  softmax_scale: Optional[float] = None):
         self.L = sw.make_layout(seqlens, B, device)
@@ -30,7 +27,9 @@ class PrefillPipeline:
         self.sketch_scale = 1.0 / math.sqrt(r)
         self.signs = torch.as_tensor(np.asarray(signs, dtype=np.int8), device=device)
         self.cols = torch.as_tensor(np.asarray(cols, dtype=np.int32), device=device)
-        taus = [tau_from_density(density, b) for b in self.L.blocks]
+        if isinstance(taus, (int, float)) or len(taus) != len(self.L.blocks):
+            raise sw.SwError(sw.SW_ERR_INVALID_ARG, "taus: one block budget per sequence")
+        taus = [int(t) for t in taus]
         self.tau_max = max(taus)
         self.tau = torch.tensor(taus, dtype=torch.int32, device=device)
         L = self.L

@@ -212,6 +212,23 @@ def make_plans(cfg_idx: int, seqlens: Optional[Sequence[int]] = None) -> List[Pl
             for si, n in enumerate(seqlens)]
 
 
+def tile_pairs(b: int, tau: int) -> int:
+    """Size of a block-causal workload: (query block, selected key block) pairs of one sequence of ``b`` blocks at
+    budget ``tau`` (row i selects min(tau, i + 1) blocks).  Both bench arms scale their work by this count."""
+    return sum(min(tau, i + 1) for i in range(b))
+
+
+def workload_config(cfg, n: int, layers: int, b: int, tau: int) -> dict:
+    """``config`` of the JSON line: what is computed, identical for the GPU arm and the reference (oracle) arm."""
+    return {"workload": cfg.name if (n, layers) == (cfg.seqlens[0], cfg.layers) else f"DEBUG n={n} L={layers}",
+            "layers": layers, "seq_len": n, "h_q": cfg.h_q, "h_kv": cfg.h_kv, "head_dim": cfg.d,
+            "block": cfg.B, "blocks": b, "tau": tau, "sketch_dim": cfg.r, "walk_power_s": cfg.s,
+            "density": cfg.density, "tile_pairs_per_layer": tile_pairs(b, tau),
+            "l2": "inputs larger than L2: 32 distinct layers x 403 MB cycle through the 126 MB L2",
+            "generator": {"coherence_a": COHERENCE_A, "plant_cos": PLANT_COS,
+                          "plant_frac": PLANT_FRAC, "chain_frac": CHAIN_FRAC, "sink_a": SINK_A}}
+
+
 def to_numpy_f64(x: torch.Tensor) -> np.ndarray:
     """Exact widening of the values handed to the GPU (bf16/fp32 -> fp64)."""
     return x.detach().to("cpu").to(torch.float64).numpy()

@@ -99,7 +99,7 @@ def test_no_cpu_fallback_without_gpu(pkg):
 def test_host_only_helpers(pkg):
     assert pkg.sw_decode_num_splits(8, 8, 128, 410) >= 1
     assert pkg.sw_decode_workspace_bytes(8, 32, 8, 128, 410) > 0
-    assert pkg.tau_from_density(0.2, 512) == 103 and pkg.tau_from_density(0.25, 16) == 4
+    assert not hasattr(pkg, "tau_from_density")      # the budget is the caller's: the package derives nothing from a density
 
 
 def test_make_layout_offsets(pkg):

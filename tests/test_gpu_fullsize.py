@@ -65,7 +65,8 @@ def run_prefill_fullsize(sw, cfg_idx, layers, *, B=None, s=None, density=None, h
     seqlens = tuple(cfg.seqlens)
     signs, cols = gen.srht_params(cfg_idx + 1, cfg.d, cfg.r)
     H = O.srht_matrix(cfg.d, signs, cols, 1 / math.sqrt(cfg.r))
-    pipe = sw.PrefillPipeline(seqlens, cfg.h_q, cfg.h_kv, cfg.d, B, cfg.r, s, density, signs, cols)
+    pipe = sw.PrefillPipeline(seqlens, cfg.h_q, cfg.h_kv, cfg.d, B, cfg.r, s,
+                              [O.tau_from_density(density, O.num_blocks(n, B)) for n in seqlens], signs, cols)
     plans = [gen.plant_plan(1000 * (cfg_idx + 1) + 7919 * si, cfg.layers, (n + B - 1) // B)
              for si, n in enumerate(seqlens)]
     rng = np.random.RandomState(cfg_idx)
@@ -163,7 +164,8 @@ def test_cfg3_fullsize_decode(sw):
             q, k, v = gen.planted_qkv(3000 + layer + 7919 * s_, t, cfg.h_q, cfg.h_kv, d, B, torch.bfloat16,
                                       plan.queries[layer], plan.targets[layer], device="cuda")
             kc[s_].copy_(k); vc[s_].copy_(v); q_new[s_].copy_(q[t - 1]); k_new[s_].copy_(k[t - 1])
-            pp = sw.PrefillPipeline([t - 1], cfg.h_q, cfg.h_kv, d, B, r, s, cfg.density, signs, cols)
+            pp = sw.PrefillPipeline([t - 1], cfg.h_q, cfg.h_kv, d, B, r, s,
+                                    [O.tau_from_density(cfg.density, O.num_blocks(t - 1, B))], signs, cols)
             pp.select(q[:t - 1], k[:t - 1])
             Wc[s_].copy_(pp.W.view(mb, mb)); kbar[s_].copy_(pp.kbar); ks[s_].copy_(pp.ks)
             if s_ in checked:                                   # oracle caches over the first t-1 tokens

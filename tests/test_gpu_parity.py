@@ -26,6 +26,22 @@ def sw():
     return pkg
 
 
+def record_overlap(test, case, overlaps):
+    """Append the measured selection overlap (GPU block lists vs the oracle's, per layer and sequence) of an
+    end-to-end case to the markdown table named by $SW_OVERLAP_LOG (profiles/overlap_r3.md is such a file); no-op
+    when the variable is unset.  The figures are recorded for every reading, also where no threshold is asserted."""
+    import os
+    path = os.environ.get("SW_OVERLAP_LOG")
+    if not path:
+        return
+    new = not os.path.exists(path)
+    with open(path, "a") as f:
+        if new:
+            f.write("| test | case | min overlap | mean overlap | per layer / sequence |\n|---|---|---|---|---|\n")
+        f.write(f"| `{test}` | {case} | {min(overlaps):.5f} | {float(np.mean(overlaps)):.5f} | "
+                f"{' '.join(f'{o:.4f}' for o in overlaps)} |\n")
+
+
 def rowwise_close(got, ref, rel=REL):
     got = np.asarray(got, np.float64); ref = np.asarray(ref, np.float64)
     scale = np.abs(ref).max(axis=-1, keepdims=True)
@@ -745,7 +761,8 @@ def test_selection_chain_paper_default_s8_heavy_tails(sw, b, flags):
     with R carried, against the fp64 oracle.  In fp32 W = A^8 leaves the normal range for A < ~2e-5 (reading
     P20 in DESIGN.md): such entries are <= 1e-37 of the row maximum, far inside the 1e-3 value tolerance, and
     the candidates they decide between are near-ties in north_star's sense (within 1e-3 of the row max of each
-    other), which is what the set comparison allows."""
+    other), which is what the set comparison allows.  The overlap with the oracle's lists stays >= 99 % all the same
+    (measured 0.9916 .. 1.0000 per layer, profiles/overlap_r3.md) and is asserted."""
     r, B, s, layers = 64, 64, 8, 3
     if flags & O.POW_MATRIX:
         s = 3
@@ -753,6 +770,7 @@ def test_selection_chain_paper_default_s8_heavy_tails(sw, b, flags):
     L = sw.make_layout([b * B], B)
     ws = torch.empty(sw.sw_workspace_bytes(sw.SW_OP_WALK_UPDATE, L), dtype=torch.uint8, device="cuda")
     R_prev_gpu, R_ref = None, None
+    overlaps = []
     tau_d = dev(np.asarray([tau], np.int32))
     for layer in range(layers):
         qs, ks = heavy_tailed_sketches(50 + layer, b, r)
@@ -772,12 +790,17 @@ def test_selection_chain_paper_default_s8_heavy_tails(sw, b, flags):
         idx_ref, cnt_ref = O.select_topk(R_ref, tau, flags)
         idx_g, cnt_g = idx.cpu().numpy(), cnt.cpu().numpy()
         assert np.array_equal(cnt_g, cnt_ref)
+        overlaps.append(sum(len(set(idx_g[i, :cnt_g[i]].tolist()) & set(idx_ref[i, :cnt_ref[i]].tolist()))
+                            for i in range(b)) / int(cnt_ref.sum()))
         for i in range(b):
             assert near_tie_only(idx_g[i, :cnt_g[i]], idx_ref[i, :cnt_ref[i]], R_ref[i], {0, i}), (layer, i)
             # everything the oracle ranks clearly above the cut is selected by the GPU too
             clear = [j for j in idx_ref[i, :cnt_ref[i]] if R_ref[i, j] > 2 * REL * np.abs(R_ref[i]).max()]
             assert set(clear) <= set(idx_g[i, :cnt_g[i]].tolist())
         R_prev_gpu = R
+    record_overlap("test_selection_chain_paper_default_s8_heavy_tails",
+                   f"b={b} s={s} {'matrix power' if flags & O.POW_MATRIX else 'element-wise power'}", overlaps)
+    assert min(overlaps) >= 0.99, overlaps
 
 
 # ------------------------------------------------------------------------------ decode selection path
@@ -810,7 +833,8 @@ def decode_case(sw, t, tau, fused, flags, B=64, s=None, layers=3, scale_q=1.0):
         torch.manual_seed(100 + layer)
         Q = ((torch.randn(t, h_q, d) + 0.5) * scale_q).bfloat16(); K = (torch.randn(t, h_kv, d) + 0.5).bfloat16()
         # caches from the GPU prefill selection path over the first t-1 tokens
-        pp = sw.PrefillPipeline([n_pre], h_q, h_kv, d, B, r, s, 0.5, signs, cols, flags)
+        pp = sw.PrefillPipeline([n_pre], h_q, h_kv, d, B, r, s, [O.tau_from_density(0.5, O.num_blocks(n_pre, B))], signs,
+                                cols, flags)
         pp.select(Q[:n_pre].cuda(), K[:n_pre].cuda())
         kbar = torch.zeros(1, mb, d, device="cuda"); ks = torch.zeros(1, mb, r, device="cuda")
         kbar[0, :b_pre] = pp.kbar; ks[0, :b_pre] = pp.ks
@@ -911,7 +935,8 @@ def test_decode_many_steps_across_a_block_boundary(sw, fused, nblk):
     K = [(torch.randn(t_end, h_kv, d) + 0.5).bfloat16() for _ in range(layers)]
     gpu, ora = [], []
     for l in range(layers):
-        pp = sw.PrefillPipeline([n_pre], h_q, h_kv, d, B, r, s, 0.5, signs, cols, flags)
+        pp = sw.PrefillPipeline([n_pre], h_q, h_kv, d, B, r, s, [O.tau_from_density(0.5, O.num_blocks(n_pre, B))], signs,
+                                cols, flags)
         pp.select(Q[l][:n_pre].cuda(), K[l][:n_pre].cuda())
         kbar = torch.zeros(1, mb, d, device="cuda"); ks = torch.zeros(1, mb, r, device="cuda")
         kbar[0, :b_pre] = pp.kbar; ks[0, :b_pre] = pp.ks
@@ -972,8 +997,9 @@ def run_prefill_stack(sw, cfg_idx, seqlens, layers, *, flags=O.DEFAULT_FLAGS, s=
     seqlens = tuple(cfg.seqlens if seqlens is None else seqlens)
     signs, cols, H = H_of(cfg.d, cfg.r, seed=cfg_idx + 1)
     dtype = torch.float32 if cfg.dtype == "f32" else torch.bfloat16
-    pipe = sw.PrefillPipeline(seqlens, cfg.h_q, cfg.h_kv, cfg.d, cfg.B, cfg.r, s, density, signs, cols, flags=flags,
-                              dtype=dtype, keep_A=True)
+    pipe = sw.PrefillPipeline(seqlens, cfg.h_q, cfg.h_kv, cfg.d, cfg.B, cfg.r, s,
+                              [O.tau_from_density(density, O.num_blocks(n, cfg.B)) for n in seqlens], signs, cols,
+                              flags=flags, dtype=dtype, keep_A=True)
     plans = gen.make_plans(cfg_idx, seqlens) if cfg.planted else None
     R_ref = [None] * len(seqlens)
     overlaps = []
@@ -1015,6 +1041,7 @@ def test_end_to_end_prefill_stack(sw, cfg_idx, seqlens, layers, fused):
     at reduced length (full-size samples live in test_gpu_fullsize.py).  ``fused`` = sw_sketch_qk +
     sw_prefill_select, otherwise the plain calls."""
     ov = run_prefill_stack(sw, cfg_idx, seqlens, layers, fused=fused)
+    record_overlap("test_end_to_end_prefill_stack", f"{gen.CONFIGS[cfg_idx].name} seqlens={seqlens} fused={fused}", ov)
     assert min(ov) >= 0.99, ov
 
 
@@ -1027,9 +1054,8 @@ def test_end_to_end_prefill_stack(sw, cfg_idx, seqlens, layers, fused):
 def test_end_to_end_prefill_stack_other_readings(sw, name, flags, s, density):
     """The readings other than the default, end to end (cfg-2 recipe, n ~ 4K, 3 layers with the walk carried):
     values within 1e-3 of the row max at every stage, selected sets equal to the oracle's up to near-ties
-    (north_star).  The >= 99 % overlap figure is asserted where the scores spread the candidates (default,
-    matrix power, no rescale); at s = 8 the element-wise power pushes most candidates of a row below 1e-3 of its
-    maximum, where north_star's own criterion calls them ties, so the overlap is only reported there."""
+    (north_star), and north_star's >= 99 % overlap for every reading, the paper's default s = 8 and the raw-score
+    reading included (measured 1.0000 on all four, profiles/overlap_r3.md)."""
     ov = run_prefill_stack(sw, 1, (4096 + 37,), 3, flags=flags, s=s, density=density)
-    if s < 8 and (flags & O.SCORE_SOFTMAX):
-        assert min(ov) >= 0.99, (name, ov)
+    record_overlap("test_end_to_end_prefill_stack_other_readings", name, ov)
+    assert min(ov) >= 0.99, (name, ov)

@@ -266,3 +266,91 @@ def test_decode_selection_idle_slots(sw):
         ref = [j for j in ib[i, :cb[i]].tolist() if j not in (0, (t - 1) // B)]
         kth = min(rb[i][ref]).item() if ref else 0.0
         assert all(abs(rb[i][j].item() - kth) <= 1e-5 * scale for j in diff)
+
+
+class _Guarded:
+    """Device tensors carved out of larger allocations with a band of canary values on both sides (bands of 256 bytes
+    or more, so that the carved tensor keeps the alignment of a fresh allocation).  check() fails when a kernel wrote
+    outside the tensor it was given.  Stands in for compute-sanitizer's memcheck, which this GPU pool does not allow
+    (profiles/sanitizer_r3.md)."""
+    BAND = 1024                                           # elements
+
+    def __init__(self):
+        self.items = []
+
+    def new(self, shape, dtype, fill=None):
+        n = int(np.prod(shape))
+        canary = {torch.float32: 12345.0, torch.bfloat16: 12288.0, torch.int32: 0x5A5A5A5A, torch.uint8: 0xA5}[dtype]
+        buf = torch.full((n + 2 * self.BAND,), canary, dtype=dtype, device="cuda")
+        view = buf[self.BAND:self.BAND + n].view(*shape)
+        if fill is not None:
+            view.copy_(fill) if torch.is_tensor(fill) else view.fill_(fill)
+        self.items.append((buf, n, canary))
+        return view
+
+    def check(self, what):
+        torch.cuda.synchronize()
+        for k, (buf, n, canary) in enumerate(self.items):
+            lo, hi = buf[:self.BAND], buf[self.BAND + n:]
+            assert bool((lo == canary).all()) and bool((hi == canary).all()), f"{what}: buffer {k} was overrun"
+
+
+def test_outputs_and_workspaces_stay_inside_their_buffers(sw):
+    """Every output and workspace of the four chains (fused prefill selection with the tensor-core walk, fused decode
+    selection with a walk state, prefill attention, split-KV decode attention) sits between canary bands; the sizes
+    are ragged (b = 513 + 130 blocks, max_blocks = 301, partial last blocks) so that any rounding up to a tile
+    would land in a band."""
+    g = _Guarded()
+    B, d, r, h_q, h_kv, s = 64, 128, 64, 8, 2, 2
+    flags = sw.SW_DEFAULT_FLAGS
+    signs, cols = gen.srht_params(3, d, r)
+    signs_d = torch.as_tensor(np.asarray(signs, np.int8)).cuda(); cols_d = torch.as_tensor(np.asarray(cols, np.int32)).cuda()
+    torch.manual_seed(90)
+    # ---- prefill: sketch -> fused selection (two layers: the second runs the walk GEMM) -> attention
+    seqlens = (64 * 512 + 17, 64 * 129 + 63)
+    L = sw.make_layout(seqlens, B)
+    T = sum(seqlens)
+    taus = [b // 5 for b in L.blocks]; tau_max = max(taus)
+    tau_d = torch.tensor(taus, dtype=torch.int32, device="cuda")
+    q = torch.randn(T, h_q, d, device="cuda").bfloat16(); k = torch.randn(T, h_kv, d, device="cuda").bfloat16()
+    v = torch.randn(T, h_kv, d, device="cuda").bfloat16()
+    qs = g.new((L.total_blocks, r), torch.float32); ks = g.new((L.total_blocks, r), torch.float32)
+    qbar = g.new((L.total_blocks, d), torch.float32); kbar = g.new((L.total_blocks, d), torch.float32)
+    W = g.new((L.total_sq,), torch.float32); R = [g.new((L.total_sq,), torch.float32) for _ in range(2)]
+    idx = g.new((L.total_blocks, tau_max), torch.int32); cnt = g.new((L.total_blocks,), torch.int32)
+    ws = g.new((sw.sw_workspace_bytes(sw.SW_OP_WALK_UPDATE, L),), torch.uint8)
+    out = g.new((T, h_q, d), torch.bfloat16); lse = g.new((T, h_q), torch.float32)
+    for layer in range(2):
+        sw.sw_sketch_qk(L, q, k, signs_d, cols_d, r, 1 / math.sqrt(r), qs, ks, qbar, kbar)
+        sw.sw_prefill_select(L, qs, ks, r, s, flags, R[0] if layer else None, R[layer], W, None, tau_d, tau_max, idx, cnt, ws)
+        g.check(f"prefill selection, layer {layer}")
+    assert sw.sw_get_walk_kernel_used() == sw.SW_WALK_TCGEN05
+    sw.sw_sparse_attn_prefill(L, q, k, v, idx, cnt, tau_max, 1 / math.sqrt(d), flags, out, lse, None)
+    g.check("prefill attention")
+    assert torch.isfinite(out.float()).all()
+    del q, k, v
+    # ---- decode: fused selection (two steps: the second streams the cached W) -> split-KV attention
+    g = _Guarded()
+    mb, batch = 301, 3
+    ts = [64 * 300 + 1, 64 * 257, 64 * 40 + 33]
+    tau = 23
+    seql = torch.tensor(ts, dtype=torch.int32, device="cuda"); tau_b = torch.full((batch,), tau, dtype=torch.int32, device="cuda")
+    Wc0, kb0, ks0 = _random_decode_caches(batch, mb, d, r, 41)
+    Wc = g.new((batch, mb, mb), torch.float32, Wc0); kbc = g.new((batch, mb, d), torch.float32, kb0)
+    ksc = g.new((batch, mb, r), torch.float32, ks0)
+    rv = [g.new((batch, mb), torch.float32) for _ in range(2)]
+    idx = g.new((batch, tau), torch.int32); cnt = g.new((batch,), torch.int32)
+    ws = g.new((sw.sw_decode_select_workspace_bytes(batch, mb),), torch.uint8)
+    qn = torch.randn(batch, h_q, d, device="cuda").bfloat16(); kn = torch.randn(batch, h_kv, d, device="cuda").bfloat16()
+    for step in range(2):
+        sw.sw_decode_select(batch, B, mb, qn, kn, seql, signs_d, cols_d, r, 1 / math.sqrt(r), s, flags, kbc, ksc, Wc,
+                            mb * mb, rv[0] if step else None, rv[step], tau_b, tau, idx, cnt, ws)
+        g.check(f"decode selection, step {step}")
+    assert (cnt == tau).all()
+    tmax = max(ts)
+    kc = torch.randn(batch, tmax, h_kv, d, device="cuda").bfloat16(); vc = torch.randn(batch, tmax, h_kv, d, device="cuda").bfloat16()
+    out = g.new((batch, h_q, d), torch.bfloat16); lse = g.new((batch, h_q), torch.float32)
+    aws = g.new((sw.sw_decode_workspace_bytes(batch, h_q, h_kv, d, tau),), torch.uint8)
+    sw.sw_sparse_attn_decode(batch, B, qn, kc, vc, seql, idx, cnt, tau, 1 / math.sqrt(d), out, lse, aws)
+    g.check("decode attention")
+    assert torch.isfinite(out.float()).all()

@@ -138,7 +138,7 @@ def prefill_bench(pkg, args, rank, world, dist, sampler, peaks):
                        "frac": sketch_gbs / peaks.get("hbm_gbs")},
         "roofline": {"kernel": "sw_sparse_attn_prefill", "bound": "tensor", "achieved": achieved, "peak": peak,
                      "unit": "TFLOP/s", "frac": achieved / peak, "traffic": _ncu_traffic("sw_sparse_attn_prefill"),
-                     "traffic_source": _ncu_traffic("_source"),
+                     "traffic_source": _ncu_traffic("_source"), "traffic_commit": _ncu_traffic("_commit"),
                      "peak_source": f"{peaks['_source']} bf16 sustained (kernel timed inside a long step)",
                      "frac_of_sustained": achieved / peak,
                      "frac_of_burst": achieved / peaks.get("bf16_tflops", peak), "peak_burst": peaks.get("bf16_tflops"),
